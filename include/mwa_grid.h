@@ -1,0 +1,104 @@
+/* mwa_grid.h - C ABI of the B200 convolutional visibility gridder.
+ *
+ * The operation (section 2.1): "The data-set then undergoes a convolution that interpolates
+ * the samples onto a regular grid to permit the operation of the Fast Fourier Transform".  The input is
+ * the correlator output of PAPER.md:19 (section 2): ~130,000 baselines x 768 channels x 4 polarisations,
+ * complex.  Everything the paper leaves open (kernel function, support, rounding, layout, edge policy)
+ * is fixed by the readings R1-R16 of DESIGN.md; the formulas below restate them.
+ *
+ *   h = (W-1)/2, s_c = freqs[c] / 299792458.0, x = (u_m * s_c) * (1.0 / cell_du)      (fp64, RN, no FMA)
+ *   (iu, ru) = INDEX(x), (iv, rv) = INDEX(y)                                          (R4)
+ *   grid[c][p][iv+tv-h][iu+tu-h] += T[rv][tv] * T[ru][tu] * w[n][c] * V[n][c][p]      (fp32 accumulate)
+ *
+ * All entry points are plain C; no torch types.  Pointers are DEVICE pointers unless the name or the
+ * comment says host.  Functions return 0 (MWA_GRID_OK) or a negative error code; the text of the last
+ * error on the calling thread is available from mwa_grid_last_error().
+ */
+#ifndef MWA_GRID_H
+#define MWA_GRID_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mwa_grid_plan mwa_grid_plan; /* opaque */
+
+enum {
+    MWA_GRID_OK = 0,
+    MWA_GRID_ERR_INVALID = -1, /* NULL / misaligned pointer, bad size or parameter */
+    MWA_GRID_ERR_NOMEM = -2,   /* workspace allocation failed */
+    MWA_GRID_ERR_CUDA = -3     /* CUDA runtime error; text in mwa_grid_last_error() */
+};
+
+/* Gridding designs (BASELINE.json north_star asks for the comparison).
+ * AUTO picks GATHER.  All designs give the same indices and values within the fp32 tolerance. */
+enum {
+    MWA_GRID_DESIGN_AUTO = 0,
+    MWA_GRID_DESIGN_ATOMIC = 1, /* K0: memset + one global red.add per tap (bring-up / ncu baseline)        */
+    MWA_GRID_DESIGN_SMEM = 2,   /* K3a: tile-owned shared-memory accumulation (red.shared.add.f32)          */
+    MWA_GRID_DESIGN_ROMEIN = 3, /* K3b: threads own cells modulo W, register-resident, flush on cell change */
+    MWA_GRID_DESIGN_GATHER = 4  /* K3c: tile-owned, threads own a 4x2 cell block in registers (product)     */
+};
+
+/* Create a plan (R5-R8 for the table).
+ *   grid_n        N, cells per side; even, 16 <= N <= 16384, N >= 2*support_W
+ *   cell_du       wavelengths per cell, finite and > 0; the plan stores inv_du = 1.0 / cell_du (fp64)
+ *   support_W     W, odd, 1 <= W <= 15
+ *   oversample_O  O, even, 2 <= O <= 64
+ *   kernel_table  HOST pointer, (O+1)*W floats, row-major [ru][t]; T[ru][t] is the 1-D kernel at the distance
+ *                 from cell (ic + t - h) to a sample at ic + (ru - O/2)/O.  Copied; the caller keeps ownership.
+ * Returns NULL on failure.  A plan owns one workspace (grown on first use, then reused: no allocation inside
+ * a warmed-up call) and must not be used by two host threads at once; different plans are independent. */
+mwa_grid_plan* mwa_grid_plan_create(int grid_n, double cell_du, int support_W, int oversample_O,
+                                    const float* kernel_table);
+
+/* Grid one visibility set (hot path: SURVEY.md section 8(a) rows a1-a5).
+ *   uv_f64   [n_vis][2]            double, metres (u_m, v_m)                 16-byte aligned
+ *   freqs    [n_chan]              double, Hz
+ *   vis_c64  [n_vis][n_chan][4][2] float (re, im), polarisation fastest      32-byte aligned
+ *   weights  [n_vis][n_chan]       float, or NULL = all ones                 4-byte aligned
+ *   grid_out [n_chan][4][N][N][2]  float (re, im), row = v, column = u       16-byte aligned
+ *            OVERWRITTEN entirely: every cell is written, zeros where no tap lands (R10).
+ *   stream   cudaStream_t passed as void* (0 = legacy default stream)
+ * Samples whose stamp would leave the grid are dropped whole (R11); that is not an error.
+ * n_chan == 0 is a no-op; n_vis == 0 zero-fills the grid.  Asynchronous: returns after enqueue; the caller's
+ * arrays must stay valid until the stream reaches the end of the call. */
+int mwa_grid_visibilities(mwa_grid_plan* plan, const double* uv_f64, const double* freqs,
+                          const float* vis_c64, const float* weights, long long n_vis, int n_chan,
+                          float* grid_out, void* stream);
+
+/* The same call on HOST buffers (pinned memory gives full PCIe speed; pageable works): copies the inputs to a
+ * device staging area owned by the plan, grids, copies the grid back, and synchronises `stream` before
+ * returning.  Layouts as above.  This is the end-to-end entry point bench.py times. */
+int mwa_grid_visibilities_host(mwa_grid_plan* plan, const double* uv_f64, const double* freqs,
+                               const float* vis_c64, const float* weights, long long n_vis, int n_chan,
+                               float* grid_out, void* stream);
+
+/* Test hook for "indices bit-exact": runs the SAME __device__ index function the gridders use.
+ *   out_idx [n_vis][n_chan][4] int32 = (iu, iv, ru, rv), or (-1,-1,-1,-1) for a dropped sample. */
+int mwa_grid_compute_indices(mwa_grid_plan* plan, const double* uv_f64, const double* freqs,
+                             long long n_vis, int n_chan, int* out_idx, void* stream);
+
+/* Select the gridding design (MWA_GRID_DESIGN_*).  Takes effect at the next call. */
+int mwa_grid_plan_set_design(mwa_grid_plan* plan, int design);
+
+/* When enabled, every mwa_grid_visibilities call records CUDA events around its stages on `stream`.
+ * mwa_grid_plan_stage_ms then synchronises on them and writes up to `n` floats (milliseconds) of the LAST
+ * call into host array `out_ms`: [0] scale+binning (a1, a3), [1] gridding kernel(s) incl. any zero-fill
+ * (a2, a4, a5), [2] whole call.  Returns the number of values written, or a negative error code. */
+int mwa_grid_plan_set_profiling(mwa_grid_plan* plan, int enabled);
+int mwa_grid_plan_stage_ms(mwa_grid_plan* plan, float* out_ms, int n);
+
+/* Number of kernel launches (memsets included) enqueued by the last gridding call on this plan. */
+int mwa_grid_plan_last_launches(const mwa_grid_plan* plan);
+
+/* Free the table and the workspace.  NULL is a no-op. */
+void mwa_grid_plan_destroy(mwa_grid_plan* plan);
+
+/* Text of the last error raised on the calling thread ("" if none).  Never NULL. */
+const char* mwa_grid_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MWA_GRID_H */

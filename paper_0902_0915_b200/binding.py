@@ -1,0 +1,190 @@
+"""Thin ctypes binding of include/mwa_grid.h: argument marshalling only, same names as the C ABI.
+
+Every step of the hot path runs in the CUDA library; there is no CPU fallback.  Importing this module
+without the built library raises ImportError (build it with `python -m paper_0902_0915_b200._build`
+or `__graft_entry__.build()`).
+"""
+import ctypes
+import os
+
+import torch
+
+from . import _build
+
+DESIGN_AUTO, DESIGN_ATOMIC, DESIGN_SMEM, DESIGN_ROMEIN, DESIGN_GATHER = 0, 1, 2, 3, 4
+DESIGNS = {"auto": DESIGN_AUTO, "atomic": DESIGN_ATOMIC, "smem": DESIGN_SMEM, "romein": DESIGN_ROMEIN,
+           "gather": DESIGN_GATHER}
+
+if not os.path.exists(_build.LIB):
+    raise ImportError(f"{_build.LIB} is missing: the CUDA library has not been built "
+                      "(run `python -m paper_0902_0915_b200._build`); there is no CPU fallback")
+
+_lib = ctypes.CDLL(_build.LIB)
+_P, _I, _LL, _D = ctypes.c_void_p, ctypes.c_int, ctypes.c_longlong, ctypes.c_double
+
+_lib.mwa_grid_plan_create.argtypes = [_I, _D, _I, _I, _P]
+_lib.mwa_grid_plan_create.restype = _P
+_lib.mwa_grid_plan_destroy.argtypes = [_P]
+_lib.mwa_grid_plan_destroy.restype = None
+_lib.mwa_grid_visibilities.argtypes = [_P, _P, _P, _P, _P, _LL, _I, _P, _P]
+_lib.mwa_grid_visibilities.restype = _I
+_lib.mwa_grid_visibilities_host.argtypes = [_P, _P, _P, _P, _P, _LL, _I, _P, _P]
+_lib.mwa_grid_visibilities_host.restype = _I
+_lib.mwa_grid_compute_indices.argtypes = [_P, _P, _P, _LL, _I, _P, _P]
+_lib.mwa_grid_compute_indices.restype = _I
+_lib.mwa_grid_plan_set_design.argtypes = [_P, _I]
+_lib.mwa_grid_plan_set_design.restype = _I
+_lib.mwa_grid_plan_set_profiling.argtypes = [_P, _I]
+_lib.mwa_grid_plan_set_profiling.restype = _I
+_lib.mwa_grid_plan_stage_ms.argtypes = [_P, _P, _I]
+_lib.mwa_grid_plan_stage_ms.restype = _I
+_lib.mwa_grid_plan_last_launches.argtypes = [_P]
+_lib.mwa_grid_plan_last_launches.restype = _I
+_lib.mwa_grid_last_error.argtypes = []
+_lib.mwa_grid_last_error.restype = ctypes.c_char_p
+
+EXPORTS = ["mwa_grid_plan_create", "mwa_grid_plan_destroy", "mwa_grid_visibilities", "mwa_grid_visibilities_host",
+           "mwa_grid_compute_indices", "mwa_grid_plan_set_design", "mwa_grid_plan_set_profiling",
+           "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_last_error"]
+
+
+class MwaGridError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"mwa_grid error {code}: {msg}")
+        self.code = code
+
+
+def mwa_grid_last_error() -> str:
+    return _lib.mwa_grid_last_error().decode()
+
+
+def _check(rc: int) -> int:
+    if rc < 0:
+        raise MwaGridError(rc, mwa_grid_last_error())
+    return rc
+
+
+def _ptr(t, dtype, device_type, name):
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor):
+        raise TypeError(f"{name} must be a torch.Tensor")
+    if t.dtype != dtype:
+        raise TypeError(f"{name} must be {dtype}, got {t.dtype}")
+    if t.device.type != device_type:
+        raise ValueError(f"{name} must live on {device_type}, got {t.device}")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous")
+    return t.data_ptr()
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def mwa_grid_plan_create(grid_n: int, cell_du: float, support_W: int, oversample_O: int, kernel_table) -> int:
+    """kernel_table: CPU float32 tensor / array of shape [O+1, W].  Returns the opaque plan handle."""
+    tab = torch.as_tensor(kernel_table, dtype=torch.float32, device="cpu").contiguous()
+    if tab.numel() != (int(oversample_O) + 1) * int(support_W):
+        raise ValueError("kernel_table must hold (O+1)*W floats")
+    h = _lib.mwa_grid_plan_create(int(grid_n), float(cell_du), int(support_W), int(oversample_O), tab.data_ptr())
+    if not h:
+        raise MwaGridError(-1, mwa_grid_last_error())
+    return h
+
+
+def mwa_grid_plan_destroy(plan) -> None:
+    if plan:
+        _lib.mwa_grid_plan_destroy(plan)
+
+
+def mwa_grid_visibilities(plan, uv_f64, freqs, vis_c64, weights, n_vis, n_chan, grid_out, stream=None) -> None:
+    """Device tensors: uv f64 [n_vis,2], freqs f64 [n_chan], vis complex64 [n_vis,n_chan,4],
+    weights f32 [n_vis,n_chan] or None, grid_out complex64 [n_chan,4,N,N] (overwritten).  Asynchronous."""
+    _check(_lib.mwa_grid_visibilities(plan, _ptr(uv_f64, torch.float64, "cuda", "uv_f64"),
+                                      _ptr(freqs, torch.float64, "cuda", "freqs"),
+                                      _ptr(vis_c64, torch.complex64, "cuda", "vis_c64"),
+                                      _ptr(weights, torch.float32, "cuda", "weights"),
+                                      int(n_vis), int(n_chan), _ptr(grid_out, torch.complex64, "cuda", "grid_out"),
+                                      _stream_ptr(stream)))
+
+
+def mwa_grid_visibilities_host(plan, uv_f64, freqs, vis_c64, weights, n_vis, n_chan, grid_out, stream=None) -> None:
+    """The same call on HOST tensors (pinned for full PCIe speed); synchronises before returning."""
+    _check(_lib.mwa_grid_visibilities_host(plan, _ptr(uv_f64, torch.float64, "cpu", "uv_f64"),
+                                           _ptr(freqs, torch.float64, "cpu", "freqs"),
+                                           _ptr(vis_c64, torch.complex64, "cpu", "vis_c64"),
+                                           _ptr(weights, torch.float32, "cpu", "weights"),
+                                           int(n_vis), int(n_chan), _ptr(grid_out, torch.complex64, "cpu", "grid_out"),
+                                           _stream_ptr(stream)))
+
+
+def mwa_grid_compute_indices(plan, uv_f64, freqs, n_vis, n_chan, out_idx, stream=None) -> None:
+    """out_idx: device int32 [n_vis, n_chan, 4] = (iu, iv, ru, rv) or -1s."""
+    _check(_lib.mwa_grid_compute_indices(plan, _ptr(uv_f64, torch.float64, "cuda", "uv_f64"),
+                                         _ptr(freqs, torch.float64, "cuda", "freqs"), int(n_vis), int(n_chan),
+                                         _ptr(out_idx, torch.int32, "cuda", "out_idx"), _stream_ptr(stream)))
+
+
+def mwa_grid_plan_set_design(plan, design) -> None:
+    _check(_lib.mwa_grid_plan_set_design(plan, DESIGNS[design] if isinstance(design, str) else int(design)))
+
+
+def mwa_grid_plan_set_profiling(plan, enabled: bool) -> None:
+    _check(_lib.mwa_grid_plan_set_profiling(plan, 1 if enabled else 0))
+
+
+def mwa_grid_plan_stage_ms(plan):
+    """(binning_ms, gridding_ms, total_ms) of the last profiled call."""
+    buf = (ctypes.c_float * 3)()
+    _check(_lib.mwa_grid_plan_stage_ms(plan, ctypes.cast(buf, ctypes.c_void_p), 3))
+    return tuple(float(x) for x in buf)
+
+
+def mwa_grid_plan_last_launches(plan) -> int:
+    return int(_lib.mwa_grid_plan_last_launches(plan))
+
+
+class Plan:
+    """Owns a plan handle; `grid()` allocates the output on the inputs' device and calls the ABI."""
+
+    def __init__(self, grid_n, cell_du, support_W, oversample_O, kernel_table, design="auto"):
+        self.grid_n, self.support_W, self.oversample_O = int(grid_n), int(support_W), int(oversample_O)
+        self.handle = mwa_grid_plan_create(grid_n, cell_du, support_W, oversample_O, kernel_table)
+        if design != "auto":
+            mwa_grid_plan_set_design(self.handle, design)
+
+    def set_design(self, design):
+        mwa_grid_plan_set_design(self.handle, design)
+
+    def grid(self, uv, freqs, vis, weights=None, out=None, stream=None):
+        n_vis, n_chan = int(uv.shape[0]), int(freqs.shape[0])
+        if out is None:
+            out = torch.empty((n_chan, 4, self.grid_n, self.grid_n), dtype=torch.complex64, device=uv.device)
+        mwa_grid_visibilities(self.handle, uv, freqs, vis, weights, n_vis, n_chan, out, stream)
+        return out
+
+    def indices(self, uv, freqs, stream=None):
+        n_vis, n_chan = int(uv.shape[0]), int(freqs.shape[0])
+        out = torch.empty((n_vis, n_chan, 4), dtype=torch.int32, device=uv.device)
+        mwa_grid_compute_indices(self.handle, uv, freqs, n_vis, n_chan, out, stream)
+        return out
+
+    def close(self):
+        if self.handle:
+            mwa_grid_plan_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()

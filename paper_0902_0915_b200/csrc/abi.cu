@@ -1,0 +1,283 @@
+// abi.cu - the extern "C" boundary declared in include/mwa_grid.h: argument checks, workspace, dispatch.
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "../../include/mwa_grid.h"
+#include "plan.h"
+
+namespace mwa {
+
+static thread_local std::string g_last_error;
+
+void set_error(const std::string& msg) { g_last_error = msg; }
+
+bool cuda_ok(cudaError_t e, const char* what) {
+    if (e == cudaSuccess) return true;
+    set_error(std::string(what) + ": " + cudaGetErrorName(e) + " - " + cudaGetErrorString(e));
+    return false;
+}
+
+template <typename T>
+static bool ensure(T*& ptr, size_t count, const char* what) {
+    if (ptr) cudaFree(ptr);
+    ptr = nullptr;
+    if (count == 0) return true;
+    cudaError_t e = cudaMalloc((void**)&ptr, count * sizeof(T));
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        set_error(std::string("workspace allocation failed (") + what + "): " + cudaGetErrorString(e));
+        ptr = nullptr;
+        return false;
+    }
+    return true;
+}
+
+// returns 0 / MWA_GRID_ERR_NOMEM
+static int ensure_workspace(Plan* p, long long n_vis, int n_chan) {
+    Workspace& ws = p->ws;
+    if (n_chan > ws.cap_chan) {
+        if (!ensure(ws.d_scale, (size_t)n_chan, "scale")) return MWA_GRID_ERR_NOMEM;
+        ws.cap_chan = n_chan;
+    }
+    if (!ws.d_scale_ref && !ensure(ws.d_scale_ref, 1, "scale_ref")) return MWA_GRID_ERR_NOMEM;
+    const int nb = (p->geom.N + kBucketCells - 1) / kBucketCells;
+    const int n_buckets = nb * nb;
+    if (n_buckets > ws.cap_buckets) {
+        if (!ensure(ws.d_bucket_count, (size_t)n_buckets + 1, "bucket_count")) return MWA_GRID_ERR_NOMEM;
+        if (!ensure(ws.d_bucket_cursor, (size_t)n_buckets, "bucket_cursor")) return MWA_GRID_ERR_NOMEM;
+        ws.cap_buckets = n_buckets;
+    }
+    if (n_vis > ws.cap_vis) {
+        if (!ensure(ws.d_perm, (size_t)n_vis, "perm")) return MWA_GRID_ERR_NOMEM;
+        if (!ensure(ws.d_uv_sorted, (size_t)n_vis, "uv_sorted")) return MWA_GRID_ERR_NOMEM;
+        ws.cap_vis = n_vis;
+    }
+    const int nt = (p->geom.N + kTile - 1) / kTile;
+    const int n_tiles = nt * nt;
+    if (n_tiles > ws.cap_tiles) {
+        if (!ensure(ws.d_tile_order, (size_t)n_tiles, "tile_order")) return MWA_GRID_ERR_NOMEM;
+        if (!ensure(ws.d_tile_weight, (size_t)n_tiles, "tile_weight")) return MWA_GRID_ERR_NOMEM;
+        ws.cap_tiles = n_tiles;
+    }
+    if (!ws.d_misc && !ensure(ws.d_misc, 4096 + 16, "misc")) return MWA_GRID_ERR_NOMEM;
+    return MWA_GRID_OK;
+}
+
+static bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
+
+static int check_common(Plan* p, const double* uv, const double* freqs, long long n_vis, int n_chan) {
+    if (!p) { set_error("plan is NULL"); return MWA_GRID_ERR_INVALID; }
+    if (n_vis < 0 || n_chan < 0) { set_error("n_vis and n_chan must be >= 0"); return MWA_GRID_ERR_INVALID; }
+    if (n_vis > 0x7fffffffLL) { set_error("n_vis must fit in 31 bits"); return MWA_GRID_ERR_INVALID; }
+    if (n_chan > 0 && !freqs) { set_error("freqs is NULL"); return MWA_GRID_ERR_INVALID; }
+    if (n_vis > 0 && n_chan > 0 && !uv) { set_error("uv_f64 is NULL"); return MWA_GRID_ERR_INVALID; }
+    if (!aligned(uv, 16)) { set_error("uv_f64 must be 16-byte aligned"); return MWA_GRID_ERR_INVALID; }
+    if (!aligned(freqs, 8)) { set_error("freqs must be 8-byte aligned"); return MWA_GRID_ERR_INVALID; }
+    return MWA_GRID_OK;
+}
+
+static int resolve_design(const Plan* p) {
+    return p->design == MWA_GRID_DESIGN_AUTO ? MWA_GRID_DESIGN_GATHER : p->design;
+}
+
+static int grid_device(Plan* p, const double* uv, const double* freqs, const float* vis, const float* weights,
+                       long long n_vis, int n_chan, float* grid, cudaStream_t st) {
+    p->last_launches = 0;
+    if (n_chan == 0) return MWA_GRID_OK;
+    int rc = ensure_workspace(p, n_vis, n_chan);
+    if (rc != MWA_GRID_OK) return rc;
+    const bool prof = p->profiling;
+    if (prof) {
+        for (auto& e : p->ev)
+            if (!e && !cuda_ok(cudaEventCreate(&e), "cudaEventCreate")) return MWA_GRID_ERR_CUDA;
+        cudaEventRecord(p->ev[0], st);
+    }
+    if (!launch_scale(p, freqs, n_chan, st)) return MWA_GRID_ERR_CUDA;
+    const int design = resolve_design(p);
+    if (design != MWA_GRID_DESIGN_ATOMIC && n_vis > 0)
+        if (!launch_binning(p, uv, n_vis, n_chan, st)) return MWA_GRID_ERR_CUDA;
+    if (prof) cudaEventRecord(p->ev[1], st);
+    bool ok = false;
+    if (n_vis == 0) {
+        ok = cuda_ok(cudaMemsetAsync(grid, 0, (size_t)n_chan * 4 * p->geom.N * p->geom.N * 8, st), "memset grid");
+        p->last_launches += 1;
+    } else {
+        switch (design) {
+            case MWA_GRID_DESIGN_ATOMIC: ok = launch_atomic(p, uv, vis, weights, n_vis, n_chan, grid, st); break;
+            case MWA_GRID_DESIGN_SMEM: ok = launch_smem(p, vis, weights, n_vis, n_chan, grid, st); break;
+            case MWA_GRID_DESIGN_ROMEIN: ok = launch_romein(p, vis, weights, n_vis, n_chan, grid, st); break;
+            case MWA_GRID_DESIGN_GATHER: ok = launch_gather(p, vis, weights, n_vis, n_chan, grid, st); break;
+            default: set_error("unknown design"); return MWA_GRID_ERR_INVALID;
+        }
+    }
+    if (!ok) return MWA_GRID_ERR_CUDA;
+    if (prof) {
+        cudaEventRecord(p->ev[2], st);
+        p->ev_valid = true;
+    }
+    return MWA_GRID_OK;
+}
+
+}  // namespace mwa
+
+using namespace mwa;
+
+extern "C" {
+
+const char* mwa_grid_last_error(void) { return g_last_error.c_str(); }
+
+mwa_grid_plan* mwa_grid_plan_create(int grid_n, double cell_du, int support_W, int oversample_O,
+                                    const float* kernel_table) {
+    g_last_error.clear();
+    if (grid_n < 16 || grid_n > 16384 || (grid_n & 1)) { set_error("grid_n must be even and in [16, 16384]"); return nullptr; }
+    if (support_W < 1 || support_W > 15 || !(support_W & 1)) { set_error("support_W must be odd and in [1, 15]"); return nullptr; }
+    if (grid_n < 2 * support_W) { set_error("grid_n must be >= 2 * support_W"); return nullptr; }
+    if (oversample_O < 2 || oversample_O > 64 || (oversample_O & 1)) { set_error("oversample_O must be even and in [2, 64]"); return nullptr; }
+    if (!(cell_du > 0.0) || !std::isfinite(cell_du)) { set_error("cell_du must be finite and > 0"); return nullptr; }
+    if (!kernel_table) { set_error("kernel_table is NULL"); return nullptr; }
+    Plan* p = new (std::nothrow) Plan();
+    if (!p) { set_error("out of host memory"); return nullptr; }
+    p->geom.N = grid_n;
+    p->geom.W = support_W;
+    p->geom.h = (support_W - 1) / 2;
+    p->geom.O = oversample_O;
+    p->geom.inv_du = 1.0 / cell_du;
+    p->cell_du = cell_du;
+    const size_t n = (size_t)(oversample_O + 1) * support_W;
+    p->h_table = new (std::nothrow) float[n];
+    if (!p->h_table) { set_error("out of host memory"); delete p; return nullptr; }
+    std::memcpy(p->h_table, kernel_table, n * sizeof(float));
+    if (!cuda_ok(cudaGetDevice(&p->device), "cudaGetDevice") ||
+        !cuda_ok(cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, p->device), "sm count") ||
+        !cuda_ok(cudaMalloc((void**)&p->d_table, n * sizeof(float)), "cudaMalloc table") ||
+        !cuda_ok(cudaMemcpy(p->d_table, kernel_table, n * sizeof(float), cudaMemcpyHostToDevice), "copy table")) {
+        mwa_grid_plan_destroy(reinterpret_cast<mwa_grid_plan*>(p));
+        return nullptr;
+    }
+    return reinterpret_cast<mwa_grid_plan*>(p);
+}
+
+void mwa_grid_plan_destroy(mwa_grid_plan* plan) {
+    if (!plan) return;
+    Plan* p = reinterpret_cast<Plan*>(plan);
+    Workspace& ws = p->ws;
+    void* ptrs[] = {p->d_table, ws.d_scale, ws.d_scale_ref, ws.d_bucket_count, ws.d_bucket_cursor, ws.d_perm,
+                    ws.d_uv_sorted, ws.d_tile_order, ws.d_tile_weight, ws.d_misc, ws.d_stage};
+    for (void* q : ptrs)
+        if (q) cudaFree(q);
+    for (auto& e : p->ev)
+        if (e) cudaEventDestroy(e);
+    delete[] p->h_table;
+    delete p;
+}
+
+int mwa_grid_plan_set_design(mwa_grid_plan* plan, int design) {
+    if (!plan) { set_error("plan is NULL"); return MWA_GRID_ERR_INVALID; }
+    if (design < MWA_GRID_DESIGN_AUTO || design > MWA_GRID_DESIGN_GATHER) { set_error("unknown design"); return MWA_GRID_ERR_INVALID; }
+    reinterpret_cast<Plan*>(plan)->design = design;
+    return MWA_GRID_OK;
+}
+
+int mwa_grid_plan_set_profiling(mwa_grid_plan* plan, int enabled) {
+    if (!plan) { set_error("plan is NULL"); return MWA_GRID_ERR_INVALID; }
+    Plan* p = reinterpret_cast<Plan*>(plan);
+    p->profiling = enabled != 0;
+    p->ev_valid = false;
+    return MWA_GRID_OK;
+}
+
+int mwa_grid_plan_stage_ms(mwa_grid_plan* plan, float* out_ms, int n) {
+    if (!plan || !out_ms || n < 0) { set_error("bad argument"); return MWA_GRID_ERR_INVALID; }
+    Plan* p = reinterpret_cast<Plan*>(plan);
+    if (!p->ev_valid) { set_error("no profiled call recorded"); return MWA_GRID_ERR_INVALID; }
+    if (!cuda_ok(cudaEventSynchronize(p->ev[2]), "cudaEventSynchronize")) return MWA_GRID_ERR_CUDA;
+    float v[3] = {0, 0, 0};
+    cudaEventElapsedTime(&v[0], p->ev[0], p->ev[1]);
+    cudaEventElapsedTime(&v[1], p->ev[1], p->ev[2]);
+    cudaEventElapsedTime(&v[2], p->ev[0], p->ev[2]);
+    int k = n < 3 ? n : 3;
+    for (int i = 0; i < k; ++i) out_ms[i] = v[i];
+    return k;
+}
+
+int mwa_grid_plan_last_launches(const mwa_grid_plan* plan) {
+    return plan ? reinterpret_cast<const Plan*>(plan)->last_launches : 0;
+}
+
+int mwa_grid_compute_indices(mwa_grid_plan* plan, const double* uv_f64, const double* freqs, long long n_vis,
+                             int n_chan, int* out_idx, void* stream) {
+    g_last_error.clear();
+    Plan* p = reinterpret_cast<Plan*>(plan);
+    int rc = check_common(p, uv_f64, freqs, n_vis, n_chan);
+    if (rc != MWA_GRID_OK) return rc;
+    if (n_vis == 0 || n_chan == 0) return MWA_GRID_OK;
+    if (!out_idx || !aligned(out_idx, 16)) { set_error("out_idx must be non-NULL and 16-byte aligned"); return MWA_GRID_ERR_INVALID; }
+    rc = ensure_workspace(p, n_vis, n_chan);
+    if (rc != MWA_GRID_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    p->last_launches = 0;
+    if (!launch_scale(p, freqs, n_chan, st)) return MWA_GRID_ERR_CUDA;
+    if (!launch_indices(p, uv_f64, n_vis, n_chan, out_idx, st)) return MWA_GRID_ERR_CUDA;
+    return MWA_GRID_OK;
+}
+
+int mwa_grid_visibilities(mwa_grid_plan* plan, const double* uv_f64, const double* freqs, const float* vis_c64,
+                          const float* weights, long long n_vis, int n_chan, float* grid_out, void* stream) {
+    g_last_error.clear();
+    Plan* p = reinterpret_cast<Plan*>(plan);
+    int rc = check_common(p, uv_f64, freqs, n_vis, n_chan);
+    if (rc != MWA_GRID_OK) return rc;
+    if (n_chan == 0) { p->last_launches = 0; return MWA_GRID_OK; }
+    if (!grid_out || !aligned(grid_out, 16)) { set_error("grid_out must be non-NULL and 16-byte aligned"); return MWA_GRID_ERR_INVALID; }
+    if (n_vis > 0 && (!vis_c64 || !aligned(vis_c64, 32))) { set_error("vis_c64 must be non-NULL and 32-byte aligned"); return MWA_GRID_ERR_INVALID; }
+    if (!aligned(weights, 4)) { set_error("weights must be 4-byte aligned"); return MWA_GRID_ERR_INVALID; }
+    return grid_device(p, uv_f64, freqs, vis_c64, weights, n_vis, n_chan, grid_out, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int mwa_grid_visibilities_host(mwa_grid_plan* plan, const double* uv_f64, const double* freqs, const float* vis_c64,
+                               const float* weights, long long n_vis, int n_chan, float* grid_out, void* stream) {
+    g_last_error.clear();
+    Plan* p = reinterpret_cast<Plan*>(plan);
+    int rc = check_common(p, uv_f64, freqs, n_vis, n_chan);
+    if (rc != MWA_GRID_OK) return rc;
+    if (n_chan == 0) { p->last_launches = 0; return MWA_GRID_OK; }
+    if (!grid_out) { set_error("grid_out is NULL"); return MWA_GRID_ERR_INVALID; }
+    if (n_vis > 0 && !vis_c64) { set_error("vis_c64 is NULL"); return MWA_GRID_ERR_INVALID; }
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    auto up = [](size_t b) { return (b + 255) & ~size_t(255); };
+    const size_t samples = (size_t)n_vis * n_chan;
+    const size_t b_uv = up((size_t)n_vis * 16), b_fr = up((size_t)n_chan * 8), b_vis = up(samples * 32);
+    const size_t b_w = weights ? up(samples * 4) : 0;
+    const size_t b_grid = (size_t)n_chan * 4 * p->geom.N * p->geom.N * 8;
+    const size_t total = b_uv + b_fr + b_vis + b_w + up(b_grid);
+    if (total > p->ws.cap_stage) {
+        if (p->ws.d_stage) cudaFree(p->ws.d_stage);
+        p->ws.d_stage = nullptr;
+        p->ws.cap_stage = 0;
+        cudaError_t e = cudaMalloc(&p->ws.d_stage, total);
+        if (e != cudaSuccess) { cudaGetLastError(); set_error("staging allocation failed"); return MWA_GRID_ERR_NOMEM; }
+        p->ws.cap_stage = total;
+    }
+    char* base = (char*)p->ws.d_stage;
+    double* d_uv = (double*)base;
+    double* d_fr = (double*)(base + b_uv);
+    float* d_vis = (float*)(base + b_uv + b_fr);
+    float* d_w = weights ? (float*)(base + b_uv + b_fr + b_vis) : nullptr;
+    float* d_grid = (float*)(base + b_uv + b_fr + b_vis + b_w);
+    if (n_vis > 0) {
+        if (!cuda_ok(cudaMemcpyAsync(d_uv, uv_f64, (size_t)n_vis * 16, cudaMemcpyHostToDevice, st), "H2D uv")) return MWA_GRID_ERR_CUDA;
+        if (!cuda_ok(cudaMemcpyAsync(d_vis, vis_c64, samples * 32, cudaMemcpyHostToDevice, st), "H2D vis")) return MWA_GRID_ERR_CUDA;
+        if (weights && !cuda_ok(cudaMemcpyAsync(d_w, weights, samples * 4, cudaMemcpyHostToDevice, st), "H2D weights")) return MWA_GRID_ERR_CUDA;
+    }
+    if (!cuda_ok(cudaMemcpyAsync(d_fr, freqs, (size_t)n_chan * 8, cudaMemcpyHostToDevice, st), "H2D freqs")) return MWA_GRID_ERR_CUDA;
+    rc = grid_device(p, d_uv, d_fr, d_vis, d_w, n_vis, n_chan, d_grid, st);
+    if (rc != MWA_GRID_OK) return rc;
+    if (!cuda_ok(cudaMemcpyAsync(grid_out, d_grid, b_grid, cudaMemcpyDeviceToHost, st), "D2H grid")) return MWA_GRID_ERR_CUDA;
+    if (!cuda_ok(cudaStreamSynchronize(st), "stream synchronize")) return MWA_GRID_ERR_CUDA;
+    return MWA_GRID_OK;
+}
+
+}  // extern "C"

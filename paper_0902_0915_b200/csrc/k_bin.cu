@@ -1,0 +1,157 @@
+// k_bin.cu - a3: counting sort of the n_vis baseline rows by uv bucket (hard part 1).
+//
+// u_lambda = u_m * nu / c is a pure radial scaling, so the rows are binned ONCE per call, at the largest
+// channel scale s_ref of the call, into kBucketCells-wide buckets.  A (tile, channel) work item of the
+// gridder back-projects its tile (plus the stamp halo) to the reference scale, walks the few buckets
+// that overlap it, and decides membership with the exact index function; the buckets only have to be
+// conservative.  n_vis items are sorted, not n_vis * n_chan.
+#include "plan.h"
+
+namespace mwa {
+
+__device__ __forceinline__ int bucket_coord(double metres, double s_ref, double inv_du, int N, int nb) {
+    const double cx = metres * s_ref * inv_du + (double)(N / 2);     // cells from the low grid edge
+    if (!(cx > 0.0)) return 0;                                        // also NaN
+    const double b = floor(cx * (1.0 / kBucketCells));
+    return b >= (double)(nb - 1) ? nb - 1 : (int)b;
+}
+
+__global__ void bin_count_kernel(GridGeom g, const double2* __restrict__ uv, const double* __restrict__ s_ref_p,
+                                 int n_vis, int nb, int* __restrict__ count) {
+    const double s_ref = *s_ref_p;
+    for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < n_vis; n += gridDim.x * blockDim.x) {
+        const double2 p = uv[n];
+        const int bx = bucket_coord(p.x, s_ref, g.inv_du, g.N, nb);
+        const int by = bucket_coord(p.y, s_ref, g.inv_du, g.N, nb);
+        atomicAdd(&count[by * nb + bx], 1);
+    }
+}
+
+// Exclusive scan of count[0..n] in place (count[n] receives the total); one block, 1024 threads.
+__global__ void bin_scan_kernel(int* __restrict__ count, int n, int* __restrict__ cursor) {
+    __shared__ int warp_sum[32];
+    __shared__ int carry_s;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    for (int base = 0; base < n; base += 1024 * 4) {
+        const int i0 = base + threadIdx.x * 4;
+        int v[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) v[k] = (i0 + k < n) ? count[i0 + k] : 0;
+        const int tsum = v[0] + v[1] + v[2] + v[3];
+        int inc = tsum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) warp_sum[wid] = inc;
+        __syncthreads();
+        if (wid == 0) {
+            int ws = warp_sum[lane];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, ws, o);
+                if (lane >= o) ws += t;
+            }
+            warp_sum[lane] = ws;                 // inclusive over warps
+        }
+        __syncthreads();
+        const int carry = carry_s;
+        int excl = carry + (wid > 0 ? warp_sum[wid - 1] : 0) + inc - tsum;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (i0 + k < n) { count[i0 + k] = excl; cursor[i0 + k] = excl; }
+            excl += v[k];
+        }
+        __syncthreads();
+        if (threadIdx.x == 1023) carry_s = carry + warp_sum[31];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) count[n] = carry_s;
+}
+
+__global__ void bin_scatter_kernel(GridGeom g, const double2* __restrict__ uv, const double* __restrict__ s_ref_p,
+                                   int n_vis, int nb, int* __restrict__ cursor, int* __restrict__ perm,
+                                   double2* __restrict__ uv_sorted) {
+    const double s_ref = *s_ref_p;
+    for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < n_vis; n += gridDim.x * blockDim.x) {
+        const double2 p = uv[n];
+        const int bx = bucket_coord(p.x, s_ref, g.inv_du, g.N, nb);
+        const int by = bucket_coord(p.y, s_ref, g.inv_du, g.N, nb);
+        const int pos = atomicAdd(&cursor[by * nb + bx], 1);
+        perm[pos] = n;
+        uv_sorted[pos] = p;
+    }
+}
+
+// Tile weights (rows whose reference-scale bucket lies under the tile) and a heaviest-first tile order by a
+// counting sort on the clipped weight.  Only a scheduling heuristic: any order gives the same grid.
+constexpr int kWeightBins = 1024;
+
+__global__ void tile_weight_kernel(const int* __restrict__ bucket_start, int nb, int nt, int* __restrict__ weight,
+                                   int* __restrict__ hist) {
+    const int per = kTile / kBucketCells;
+    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < nt * nt; t += gridDim.x * blockDim.x) {
+        const int ty = t / nt, tx = t - ty * nt;
+        int w = 0;
+        for (int dy = 0; dy < per; ++dy) {
+            const int by = ty * per + dy;
+            if (by >= nb) break;
+            const int b0 = by * nb + tx * per;
+            const int b1 = by * nb + min(nb, tx * per + per);
+            if (b0 < b1) w += bucket_start[b1] - bucket_start[b0];
+        }
+        weight[t] = w;
+        atomicAdd(&hist[kWeightBins - 1 - min(w, kWeightBins - 1)], 1);   // descending
+    }
+}
+
+__global__ void tile_order_scan_kernel(int* __restrict__ hist) {   // one block of kWeightBins threads
+    __shared__ int s[kWeightBins];
+    s[threadIdx.x] = hist[threadIdx.x];
+    __syncthreads();
+    for (int o = 1; o < kWeightBins; o <<= 1) {
+        const int t = threadIdx.x >= o ? s[threadIdx.x - o] : 0;
+        __syncthreads();
+        s[threadIdx.x] += t;
+        __syncthreads();
+    }
+    hist[threadIdx.x] = s[threadIdx.x] - hist[threadIdx.x];         // exclusive
+}
+
+__global__ void tile_order_scatter_kernel(const int* __restrict__ weight, int n_tiles, int* __restrict__ hist,
+                                          int* __restrict__ order) {
+    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < n_tiles; t += gridDim.x * blockDim.x) {
+        const int pos = atomicAdd(&hist[kWeightBins - 1 - min(weight[t], kWeightBins - 1)], 1);
+        order[pos] = t;
+    }
+}
+
+bool launch_binning(Plan* p, const double* uv, long long n_vis, int /*n_chan*/, cudaStream_t st) {
+    Workspace& ws = p->ws;
+    const int nb = (p->geom.N + kBucketCells - 1) / kBucketCells;
+    const int n_buckets = nb * nb;
+    const int nt = (p->geom.N + kTile - 1) / kTile;
+    if (!cuda_ok(cudaMemsetAsync(ws.d_bucket_count, 0, ((size_t)n_buckets + 1) * sizeof(int), st), "memset buckets"))
+        return false;
+    if (!cuda_ok(cudaMemsetAsync(ws.d_misc, 0, (4096 + 16) * sizeof(int), st), "memset misc")) return false;
+    int blocks = (int)((n_vis + 255) / 256);
+    if (blocks > p->sm_count * 8) blocks = p->sm_count * 8;
+    bin_count_kernel<<<blocks, 256, 0, st>>>(p->geom, (const double2*)uv, ws.d_scale_ref, (int)n_vis, nb,
+                                             ws.d_bucket_count);
+    bin_scan_kernel<<<1, 1024, 0, st>>>(ws.d_bucket_count, n_buckets, ws.d_bucket_cursor);
+    bin_scatter_kernel<<<blocks, 256, 0, st>>>(p->geom, (const double2*)uv, ws.d_scale_ref, (int)n_vis, nb,
+                                               ws.d_bucket_cursor, ws.d_perm, ws.d_uv_sorted);
+    int* hist = ws.d_misc + 16;
+    int tblocks = (nt * nt + 255) / 256;
+    if (tblocks > p->sm_count * 8) tblocks = p->sm_count * 8;
+    tile_weight_kernel<<<tblocks, 256, 0, st>>>(ws.d_bucket_count, nb, nt, ws.d_tile_weight, hist);
+    tile_order_scan_kernel<<<1, kWeightBins, 0, st>>>(hist);
+    tile_order_scatter_kernel<<<tblocks, 256, 0, st>>>(ws.d_tile_weight, nt * nt, hist, ws.d_tile_order);
+    p->last_launches += 8;
+    return cuda_ok(cudaGetLastError(), "binning kernels");
+}
+
+}  // namespace mwa

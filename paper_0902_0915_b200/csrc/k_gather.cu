@@ -1,0 +1,353 @@
+// k_gather.cu - K3c, the product gridder: tile-owned, register-resident accumulation (a2 + a4 + a5 fused).
+//
+// One WARP owns one 16x16-cell tile of one channel (all 4 polarisations) from its first tap to its single
+// write-out, so there are no atomics on grid data anywhere and every grid cell is written exactly once,
+// zeros included (R10; SURVEY.md section 7 hard part 2).  Inside the warp every lane owns a 4x2 block
+// of cells: 8 cells x 4 pol x (re, im) = 64 fp32 accumulators in registers.  PAPER.md:49 calls this the
+// "gather" form ("a thread collects the values for a particular memory location"); what is new here is
+// how a lane finds its values without scanning everything:
+//
+//   phase A (lane = candidate row): walk the buckets of k_bin.cu that can reach the tile at this channel's
+//            scale, run the exact index function (index.cuh) on each candidate, keep the rows whose WxW
+//            stamp overlaps the tile; per hit store w*V, the table offsets and a 32-bit mask of the lanes
+//            (4x2 blocks) the stamp overlaps.
+//   transpose: a 32x32 bit-matrix transpose by warp shuffles turns "blocks per hit" into "hits per block".
+//   phase B (lane = block owner): each lane walks ITS OWN hit list; all 32 lanes do useful FMAs on
+//            different hits.  Per hit a lane reads w*V (2 x LDS.128), 4 u-taps (LDS.128) and 2 v-taps (LDS.64)
+//            from zero-padded, pre-shifted copies of the kernel table, and issues 32 packed fma.rn.f32x2.
+//   write-out: 16 x STG.128 per lane, streaming (evict-first) so the grid does not push vis lines out of L2.
+//
+// Work items (tile, channel) are taken from a global counter, channel fastest, tiles heaviest first.
+#include "plan.h"
+
+namespace mwa {
+
+constexpr int kWarpsPerCta = 4;
+constexpr int kCap = 128;                 // hits buffered per warp before they are consumed
+constexpr int kBlocksX = 4, kBlocksY = 8; // lane -> block (bx = lane & 3, by = lane >> 2); block = 4 x 2 cells
+
+struct GatherParams {
+    GridGeom g;
+    const double* scale;        // [n_chan]
+    const double* scale_ref;    // [1]
+    const int* bucket_start;    // [nb*nb + 1]
+    const int* perm;            // [n_vis]
+    const double2* uv_sorted;   // [n_vis]
+    const int* tile_order;      // [nt*nt]
+    int* counter;               // work counter
+    const float4* vis;          // [n_vis][n_chan][2] float4
+    const float* weights;       // [n_vis][n_chan] or null
+    const float* table;         // [(O+1)][W]
+    float* grid;                // [n_chan][4][N][N][2]
+    int n_chan, nb, nt;
+    int rlu, rlv;               // padded row lengths of the shifted table copies
+    long long n_items;
+};
+
+typedef unsigned long long u64;
+
+__device__ __forceinline__ u64 pack2(float a, float b) {
+    u64 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
+    return r;
+}
+__device__ __forceinline__ void unpack2(u64 v, float& a, float& b) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v));
+}
+__device__ __forceinline__ void ffma2(u64& d, u64 a, u64 b) {        // d = a * b + d, two fp32 lanes
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(a), "l"(b));
+}
+__device__ __forceinline__ void st_stream_v4(float* p, float a, float b, float c, float d) {
+    asm volatile("st.global.cs.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+
+// 32x32 bit-matrix transpose across the warp: in = row `lane`, out bit h = bit `lane` of lane h's input.
+__device__ __forceinline__ unsigned transpose32(unsigned x, int lane) {
+#pragma unroll
+    for (int s = 0; s < 5; ++s) {
+        const int j = 16 >> s;
+        const unsigned m = s == 0 ? 0x0000FFFFu : s == 1 ? 0x00FF00FFu : s == 2 ? 0x0F0F0F0Fu : s == 3 ? 0x33333333u : 0x55555555u;
+        const unsigned y = __shfl_xor_sync(0xffffffffu, x, j);
+        x = (lane & j) ? ((x & ~m) | ((y >> j) & m)) : ((x & m) | ((y << j) & ~m));
+    }
+    return x;
+}
+
+struct WarpSmem {
+    float4 z[kCap][2];      // w*V: {XX.re, XX.im, XY.re, XY.im}, {YX.re, YX.im, YY.re, YY.im}
+    unsigned geo[kCap];     // (byte offset into u copies + bias) | (byte offset into v copies + bias) << 16
+    unsigned mask[kCap];    // lanes (blocks) the stamp overlaps
+    int row[kCap];          // original row id (vis / weights index)
+};
+
+constexpr int kBiasU = 16, kBiasV = 16;   // floats; keep the stored offsets non-negative
+
+__global__ void __launch_bounds__(kWarpsPerCta * 32)
+gather_kernel(const GatherParams P) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const GridGeom g = P.g;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // ---- shifted, zero-padded table copies (built once per CTA)
+    //   tu[s][r][q] = Tp_u[r][q + s], Tp_u[r][3 + t] = T[r][t]      s = 0..3, q = 0..rlu-1
+    //   tv[s][r][q] = Tp_v[r][q + s], Tp_v[r][1 + t] = T[r][t]      s = 0..1, q = 0..rlv-1
+    float* tu = reinterpret_cast<float*>(smem_raw);
+    const int n_tu = 4 * (g.O + 1) * P.rlu;
+    const int n_tv = 2 * (g.O + 1) * P.rlv;
+    float* tv = tu + n_tu;
+    WarpSmem* wsm = reinterpret_cast<WarpSmem*>(smem_raw + (((size_t)(n_tu + n_tv) * 4 + 15) & ~size_t(15))) + warp;
+    for (int k = threadIdx.x; k < n_tu; k += blockDim.x) {
+        const int q = k % P.rlu, r = (k / P.rlu) % (g.O + 1), s = k / (P.rlu * (g.O + 1));
+        const int t = q + s - 3;
+        tu[k] = (t >= 0 && t < g.W) ? P.table[r * g.W + t] : 0.0f;
+    }
+    for (int k = threadIdx.x; k < n_tv; k += blockDim.x) {
+        const int q = k % P.rlv, r = (k / P.rlv) % (g.O + 1), s = k / (P.rlv * (g.O + 1));
+        const int t = q + s - 1;
+        tv[k] = (t >= 0 && t < g.W) ? P.table[r * g.W + t] : 0.0f;
+    }
+    __syncthreads();
+
+    const int bx = lane & 3, by = lane >> 2;
+    const unsigned tu_s = (unsigned)__cvta_generic_to_shared(tu);
+    const unsigned tv_s = (unsigned)__cvta_generic_to_shared(tv);
+    const unsigned z_s = (unsigned)__cvta_generic_to_shared(&wsm->z[0][0]);
+    const unsigned geo_s = (unsigned)__cvta_generic_to_shared(&wsm->geo[0]);
+    // lane constants of the table addresses: offset (floats) = stored - bias + 4*bx  (u), + 2*by (v)
+    const unsigned cu = tu_s + (unsigned)((4 * bx - kBiasU) * 4);
+    const unsigned cv = tv_s + (unsigned)((2 * by - kBiasV) * 4);
+    const double s_ref = *P.scale_ref;
+    const size_t plane = (size_t)g.N * g.N;
+    const unsigned lt_mask = (1u << lane) - 1u;
+
+    long long item = 0;
+    if (lane == 0) item = (long long)atomicAdd(P.counter, 1);
+    item = __shfl_sync(0xffffffffu, item, 0);
+
+    while (item < P.n_items) {
+        long long next_item = 0;
+        if (lane == 0) next_item = (long long)atomicAdd(P.counter, 1);      // latency hidden behind this item
+        const int trank = (int)(item / P.n_chan);
+        const int c = (int)(item - (long long)trank * P.n_chan);
+        const int tile = P.tile_order[trank];
+        const int ty = tile / P.nt, tx = tile - ty * P.nt;
+        const int X0 = tx * kTile, Y0 = ty * kTile;
+        const double sc = P.scale[c];
+
+        // ---- candidate buckets: back-project [X0 - h - 1, X0 + 15 + h + 1] (cells from the centre) to s_ref
+        int bx0 = 0, bx1 = P.nb - 1, by0 = 0, by1 = P.nb - 1;
+        {
+            const double rho = sc / s_ref;                       // <= 1 for positive frequencies
+            if (rho > 1e-3 && rho <= 1.0 + 1e-9) {
+                const double half = (double)(g.N / 2), pad = (double)g.h + 1.25, inv = 1.0 / rho;
+                const double lox = ((double)X0 - pad - half) * inv + half, hix = ((double)(X0 + kTile - 1) + pad - half) * inv + half;
+                const double loy = ((double)Y0 - pad - half) * inv + half, hiy = ((double)(Y0 + kTile - 1) + pad - half) * inv + half;
+                const double ib = 1.0 / kBucketCells, top = (double)(P.nb - 1);
+                bx0 = (int)fmin(fmax(floor(lox * ib), 0.0), top);
+                bx1 = (int)fmin(fmax(floor(hix * ib), 0.0), top);
+                by0 = (int)fmin(fmax(floor(loy * ib), 0.0), top);
+                by1 = (int)fmin(fmax(floor(hiy * ib), 0.0), top);
+            }
+        }
+
+        u64 acc[2][4][4];   // [row i][col j][pol] = (re, im)
+#pragma unroll
+        for (int i = 0; i < 2; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+#pragma unroll
+                for (int p = 0; p < 4; ++p) acc[i][j][p] = 0ull;
+
+        int n_buf = 0;
+
+        // consume the buffered hits: loads of w*V, transpose, per-lane walk
+        auto consume = [&](int n) {
+            __syncwarp();
+            // pass 2: lane = hit; visibility + weight loads, all independent
+#pragma unroll
+            for (int b = 0; b < kCap / 32; ++b) {
+                const int hidx = b * 32 + lane;
+                if (hidx < n) {
+                    const size_t sidx = (size_t)wsm->row[hidx] * P.n_chan + c;
+                    const float4 va = __ldg(P.vis + 2 * sidx), vb = __ldg(P.vis + 2 * sidx + 1);
+                    const float wt = P.weights ? __ldg(P.weights + sidx) : 1.0f;
+                    wsm->z[hidx][0] = make_float4(wt * va.x, wt * va.y, wt * va.z, wt * va.w);
+                    wsm->z[hidx][1] = make_float4(wt * vb.x, wt * vb.y, wt * vb.z, wt * vb.w);
+                }
+            }
+            unsigned mw[kCap / 32];
+#pragma unroll
+            for (int b = 0; b < kCap / 32; ++b) {
+                const int hidx = b * 32 + lane;
+                const unsigned m = (b * 32 < n) ? ((hidx < n) ? wsm->mask[hidx] : 0u) : 0u;
+                mw[b] = (b * 32 < n) ? transpose32(m, lane) : 0u;
+            }
+            __syncwarp();
+            unsigned m = mw[0];
+            int w = 0;
+            while (true) {
+                if (m == 0u) {
+#pragma unroll
+                    for (int b = 1; b < kCap / 32; ++b)
+                        if (m == 0u && w < b) { w = b; m = mw[b]; }
+                }
+                const bool act = (m != 0u);
+                if (!__any_sync(0xffffffffu, act)) break;
+                if (act) {
+                    const int bit = __ffs(m) - 1;
+                    m &= m - 1u;
+                    const int hidx = w * 32 + bit;
+                    unsigned geo;
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(geo) : "r"(geo_s + 4u * hidx));
+                    float ku0, ku1, ku2, ku3, kv0, kv1;
+                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(ku0), "=f"(ku1), "=f"(ku2), "=f"(ku3) : "r"(cu + (geo & 0xffffu)));
+                    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(kv0), "=f"(kv1) : "r"(cv + (geo >> 16)));
+                    u64 z0, z1, z2, z3;
+                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(z0), "=l"(z1) : "r"(z_s + 32u * hidx));
+                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(z2), "=l"(z3) : "r"(z_s + 32u * hidx + 16u));
+                    const float ku[4] = {ku0, ku1, ku2, ku3};
+                    const float kv[2] = {kv0, kv1};
+#pragma unroll
+                    for (int i = 0; i < 2; ++i)
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            const float k = kv[i] * ku[j];
+                            const u64 kk = pack2(k, k);
+                            ffma2(acc[i][j][0], kk, z0);
+                            ffma2(acc[i][j][1], kk, z1);
+                            ffma2(acc[i][j][2], kk, z2);
+                            ffma2(acc[i][j][3], kk, z3);
+                        }
+                }
+            }
+            __syncwarp();
+        };
+
+        // ---- phase A, pass 1: lane = candidate
+        for (int byb = by0; byb <= by1; ++byb) {
+            const int k0 = __ldg(P.bucket_start + byb * P.nb + bx0);
+            const int k1 = __ldg(P.bucket_start + byb * P.nb + bx1 + 1);
+            for (int kb = k0; kb < k1; kb += 32) {
+                const int k = kb + lane;
+                bool hit = false;
+                unsigned geo = 0, mask = 0;
+                int row = 0;
+                if (k < k1) {
+                    const double2 p = __ldg(P.uv_sorted + k);
+                    SampleIndex s;
+                    if (sample_index(p.x, p.y, sc, g, s)) {
+                        const int ou = s.iu - g.h - X0, ov = s.iv - g.h - Y0;     // stamp origin relative to the tile
+                        if (ou > -g.W && ou < kTile && ov > -g.W && ov < kTile) {
+                            hit = true;
+                            row = __ldg(P.perm + k);
+                            const int su = (3 - ou) & 3, sv = (1 - ov) & 1;
+                            const int offu = (su * (g.O + 1) + s.ru) * P.rlu + (3 - ou - su) + kBiasU;
+                            const int offv = (sv * (g.O + 1) + s.rv) * P.rlv + (1 - ov - sv) + kBiasV;
+                            geo = (unsigned)(offu * 4) | ((unsigned)(offv * 4) << 16);
+                            const int bxl = max(0, ou >> 2), bxh = min(kBlocksX - 1, (ou + g.W - 1) >> 2);
+                            const int byl = max(0, ov >> 1), byh = min(kBlocksY - 1, (ov + g.W - 1) >> 1);
+                            const unsigned m4 = (2u << bxh) - (1u << bxl);
+                            const unsigned rows = 0x11111111u & (0xFFFFFFFFu >> (28 - 4 * byh)) & (0xFFFFFFFFu << (4 * byl));
+                            mask = rows * m4;
+                        }
+                    }
+                }
+                const unsigned ball = __ballot_sync(0xffffffffu, hit);
+                const int cnt = __popc(ball);
+                if (cnt == 0) continue;
+                if (n_buf + cnt > kCap) { consume(n_buf); n_buf = 0; }
+                if (hit) {
+                    const int slot = n_buf + __popc(ball & lt_mask);
+                    wsm->geo[slot] = geo;
+                    wsm->mask[slot] = mask;
+                    wsm->row[slot] = row;
+                }
+                n_buf += cnt;
+            }
+        }
+        if (n_buf > 0) consume(n_buf);
+
+        // ---- a5: write the lane's 4x2 block of all 4 planes, once
+        {
+            const int x = X0 + 4 * bx;
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const int y = Y0 + 2 * by + i;
+                if (y < g.N) {
+#pragma unroll
+                    for (int p = 0; p < 4; ++p) {
+                        float* dst = P.grid + (((size_t)c * 4 + p) * plane + (size_t)y * g.N + x) * 2;
+                        float a0, a1, a2, a3;
+                        if (x + 1 < g.N) {
+                            unpack2(acc[i][0][p], a0, a1);
+                            unpack2(acc[i][1][p], a2, a3);
+                            st_stream_v4(dst, a0, a1, a2, a3);
+                        }
+                        if (x + 3 < g.N) {
+                            unpack2(acc[i][2][p], a0, a1);
+                            unpack2(acc[i][3][p], a2, a3);
+                            st_stream_v4(dst + 4, a0, a1, a2, a3);
+                        }
+                    }
+                }
+            }
+        }
+        item = __shfl_sync(0xffffffffu, next_item, 0);
+    }
+}
+
+bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
+                   cudaStream_t st) {
+    (void)n_vis;
+    GatherParams P;
+    P.g = p->geom;
+    P.scale = p->ws.d_scale;
+    P.scale_ref = p->ws.d_scale_ref;
+    P.bucket_start = p->ws.d_bucket_count;
+    P.perm = p->ws.d_perm;
+    P.uv_sorted = p->ws.d_uv_sorted;
+    P.tile_order = p->ws.d_tile_order;
+    P.counter = p->ws.d_misc;
+    P.vis = (const float4*)vis;
+    P.weights = w;
+    P.table = p->d_table;
+    P.grid = grid;
+    P.n_chan = n_chan;
+    P.nb = (p->geom.N + kBucketCells - 1) / kBucketCells;
+    P.nt = (p->geom.N + kTile - 1) / kTile;
+    P.rlu = (p->geom.W + 6 + 3) & ~3;
+    P.rlv = (p->geom.W + 2 + 1) & ~1;
+    P.n_items = (long long)P.nt * P.nt * n_chan;
+    const size_t tbl = ((size_t)(4 * P.rlu + 2 * P.rlv) * (p->geom.O + 1) * 4 + 15) & ~size_t(15);
+    const size_t smem = tbl + sizeof(WarpSmem) * kWarpsPerCta;
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (!cuda_ok(cudaFuncSetAttribute(gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024),
+                     "gather smem attribute"))
+            return false;
+        attr_set = true;
+    }
+    int ctas_per_sm = 0;
+    if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, gather_kernel, kWarpsPerCta * 32, smem),
+                 "gather occupancy"))
+        return false;
+    if (ctas_per_sm < 1) { set_error("gather kernel does not fit on an SM"); return false; }
+    long long want = (P.n_items + kWarpsPerCta - 1) / kWarpsPerCta;
+    long long blocks = (long long)p->sm_count * ctas_per_sm;
+    if (blocks > want) blocks = want;
+    if (blocks < 1) blocks = 1;
+    gather_kernel<<<(unsigned)blocks, kWarpsPerCta * 32, smem, st>>>(P);
+    p->last_launches += 1;
+    return cuda_ok(cudaGetLastError(), "gather_kernel");
+}
+
+// placeholders until the comparison designs land
+bool launch_smem(Plan*, const float*, const float*, long long, int, float*, cudaStream_t) {
+    set_error("design SMEM is not built yet");
+    return false;
+}
+bool launch_romein(Plan*, const float*, const float*, long long, int, float*, cudaStream_t) {
+    set_error("design ROMEIN is not built yet");
+    return false;
+}
+
+}  // namespace mwa

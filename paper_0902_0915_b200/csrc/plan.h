@@ -1,0 +1,67 @@
+// plan.h - the plan object behind the C ABI and the launchers of the individual kernels.
+#pragma once
+#include <cuda_runtime.h>
+#include <string>
+#include "index.cuh"
+
+namespace mwa {
+
+// Binning geometry (a3).  Rows are sorted once per call by the bucket of their position at the TOP
+// frequency of the call (largest extent); every channel's position is a radial contraction of that one.
+constexpr int kBucketCells = 8;     // bucket side in cells at the reference scale
+constexpr int kTile = 16;           // gridding tile side in cells (one warp owns one tile of one channel)
+
+struct Workspace {
+    // a1
+    double* d_scale = nullptr;       // [n_chan]
+    int cap_chan = 0;
+    // a3
+    double* d_scale_ref = nullptr;   // [1] max over channels of s_c
+    int* d_bucket_count = nullptr;   // [nb*nb + 1] histogram, then exclusive scan = bucket_start
+    int* d_bucket_cursor = nullptr;  // [nb*nb] scatter cursors
+    int cap_buckets = 0;
+    int* d_perm = nullptr;           // [n_vis] row ids sorted by bucket
+    double2* d_uv_sorted = nullptr;  // [n_vis] uv of the sorted rows
+    long long cap_vis = 0;
+    int* d_tile_order = nullptr;     // [n_tiles] tile ids, heaviest first
+    int* d_tile_weight = nullptr;    // [n_tiles]
+    int* d_misc = nullptr;           // small counters
+    int cap_tiles = 0;
+    // host-buffer entry point staging
+    void* d_stage = nullptr;
+    size_t cap_stage = 0;
+};
+
+struct Plan {
+    GridGeom geom{};
+    double cell_du = 0.0;
+    float* d_table = nullptr;        // [(O+1)][W] as given
+    float* h_table = nullptr;        // host copy
+    int design = 0;
+    int device = 0;
+    int sm_count = 148;
+    Workspace ws;
+    // profiling
+    bool profiling = false;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    bool ev_valid = false;
+    int last_launches = 0;
+};
+
+void set_error(const std::string& msg);
+bool cuda_ok(cudaError_t e, const char* what);
+
+// launchers (each returns false after set_error on failure and adds its launches to plan->last_launches)
+bool launch_scale(Plan* p, const double* freqs, int n_chan, cudaStream_t st);
+bool launch_indices(Plan* p, const double* uv, long long n_vis, int n_chan, int* out_idx, cudaStream_t st);
+bool launch_atomic(Plan* p, const double* uv, const float* vis, const float* w, long long n_vis, int n_chan,
+                   float* grid, cudaStream_t st);
+bool launch_binning(Plan* p, const double* uv, long long n_vis, int n_chan, cudaStream_t st);
+bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
+                   cudaStream_t st);
+bool launch_smem(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
+                 cudaStream_t st);
+bool launch_romein(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
+                   cudaStream_t st);
+
+}  // namespace mwa

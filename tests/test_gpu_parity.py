@@ -1,0 +1,220 @@
+"""GPU parity: the CUDA library (through the C ABI binding) against the fp64 CPU oracle, same seeded inputs.
+
+Indices must match bit for bit; grid values within the north_star tolerance (tests/parity.py).
+Sizes: C1 and cut-down C2/C5 shapes element by element; C3 whole; C4 and C5 at FULL size on sampled
+channels (a channel owns its grid, so a whole channel is compared element by element).
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from gen import CONFIGS, generate, make_kernel_table, scaled
+from parity import assert_parity
+
+pytestmark = pytest.mark.gpu
+C = 299792458.0
+DESIGNS = ["atomic", "gather"]
+
+
+@pytest.fixture(scope="module")
+def lib():
+    import paper_0902_0915_b200 as m
+    return m
+
+
+def _plan(lib, g, design="auto"):
+    cfg = g.cfg
+    return lib.Plan(cfg.grid_n, g.cell_du, cfg.support_W, cfg.oversample_O, g.kernel_table, design=design)
+
+
+def _oracle(g, chans=None):
+    cfg = g.cfg
+    uv, fr, vis, w = g.uv.cpu(), g.freqs.cpu(), g.vis, g.weights
+    if chans is not None:
+        fr = fr[chans]
+        vis = vis[:, chans]
+        w = w[:, chans]
+    return oracle.grid(uv, fr, vis.cpu(), w.cpu(), cfg.grid_n, g.cell_du, cfg.support_W, cfg.oversample_O,
+                       g.kernel_table)
+
+
+def _to_dev(g):
+    g.uv, g.freqs, g.vis, g.weights = (t.cuda().contiguous() for t in (g.uv, g.freqs, g.vis, g.weights))
+    return g
+
+
+# ---------------------------------------------------------------------------- indices: bit-exact
+@pytest.mark.parametrize("cfg", [CONFIGS["C1"], scaled(CONFIGS["C2"], n_ant=48, n_chan=7),
+                                 scaled(CONFIGS["C5"], n_ant=24, core_ant=12, n_chan=5, grid_n=512),
+                                 scaled(CONFIGS["C4"], n_ant=40, core_ant=20, n_chan=48, oversample_O=6)])
+def test_indices_bit_exact(lib, cfg):
+    g = generate(cfg)
+    want = oracle.compute_indices(g.uv, g.freqs, cfg.grid_n, g.cell_du, cfg.support_W, cfg.oversample_O)
+    _to_dev(g)
+    with _plan(lib, g) as p:
+        got = p.indices(g.uv, g.freqs).cpu().numpy()
+    assert np.array_equal(got, want)
+
+
+def test_indices_lattice_halfway_edges_and_nonfinite(lib):
+    # positions on the 1/(2O) lattice hit every rounding tie; s = 1, du = 1 so x = u_m exactly
+    N, W, O = 256, 7, 8
+    lat = np.arange(-130 * 2 * O, 130 * 2 * O + 1) / (2.0 * O)
+    rs = np.random.RandomState(3)
+    extra = np.concatenate([rs.uniform(-130, 130, 5000), [np.nan, np.inf, -np.inf, 1e300, -0.0, 0.0, 124.5, 124.5625]])
+    u = np.concatenate([lat, extra])
+    uv = np.stack([u, u[::-1]], axis=1).copy()
+    fr = np.array([C, 0.5 * C, 150e6])
+    want = oracle.compute_indices(uv, fr, N, 1.0, W, O)
+    with lib.Plan(N, 1.0, W, O, make_kernel_table(W, O)) as p:
+        got = p.indices(torch.from_numpy(uv).cuda(), torch.from_numpy(fr).cuda()).cpu().numpy()
+    assert np.array_equal(got, want)
+    assert (want[:, 0, 0] == -1).any() and (want[:, 0, 0] >= 0).any()
+
+
+# ---------------------------------------------------------------------------- values
+@pytest.mark.parametrize("design", DESIGNS)
+def test_c1_whole_grid(lib, design):
+    g = generate(CONFIGS["C1"])
+    G, A, _ = _oracle(g)
+    _to_dev(g)
+    with _plan(lib, g, design) as p:
+        out = p.grid(g.uv, g.freqs, g.vis, g.weights)
+        torch.cuda.synchronize()
+        assert_parity(out.cpu().numpy(), G, A, design)
+        out2 = p.grid(g.uv, g.freqs, g.vis, None)                 # NULL weights = ones (R12)
+        assert_parity(out2.cpu().numpy(), G, A, design + " null weights")
+
+
+@pytest.mark.parametrize("design", DESIGNS)
+@pytest.mark.parametrize("name,kw", [
+    ("C2", dict(n_ant=64, n_chan=6)),                              # several tiles, several channels
+    ("C5", dict(n_ant=20, core_ant=10, n_chan=3, grid_n=512)),     # W = 15, O = 16, random weights, rotation
+    ("C4", dict(n_ant=64, core_ant=32, n_chan=16, grid_n=250)),    # grid not a multiple of the tile: ragged tail
+])
+def test_cut_down_configs(lib, design, name, kw):
+    g = generate(scaled(CONFIGS[name], **kw))
+    G, A, _ = _oracle(g)
+    _to_dev(g)
+    with _plan(lib, g, design) as p:
+        out = p.grid(g.uv, g.freqs, g.vis, g.weights)
+        torch.cuda.synchronize()
+    assert_parity(out.cpu().numpy(), G, A, f"{name} {design}")
+
+
+@pytest.mark.parametrize("design", DESIGNS)
+def test_c3_whole(lib, design):
+    g = generate(CONFIGS["C3"], device="cuda")
+    G, A, _ = _oracle(g)
+    with _plan(lib, g, design) as p:
+        out = p.grid(g.uv, g.freqs, g.vis, g.weights)
+        torch.cuda.synchronize()
+    assert_parity(out.cpu().numpy(), G, A, f"C3 {design}")
+
+
+def test_c2_whole(lib):
+    g = generate(CONFIGS["C2"], device="cuda")
+    with _plan(lib, g) as p:
+        out = p.grid(g.uv, g.freqs, g.vis, g.weights)
+        torch.cuda.synchronize()
+    for c0 in range(0, 32, 8):
+        ch = list(range(c0, c0 + 8))
+        G, A, _ = _oracle(g, ch)
+        assert_parity(out[c0:c0 + 8].cpu().numpy(), G, A, f"C2 channels {c0}..")
+
+
+def test_single_visibility_stamp_and_dropped_rows(lib):
+    N, W, O, h = 256, 7, 8, 3
+    T = make_kernel_table(W, O)
+    uv = np.array([[10.0625, -10.25], [124.5625, 0.0], [0.0, -126.0], [-124.5, 124.5]])
+    vis = np.zeros((4, 1, 4), dtype=np.complex64)
+    vis[0, 0] = [1 + 0j, 2j, -3.0, 0.5 - 0.25j]
+    vis[1:] = 7.0                                                  # rows 1, 2 are dropped whole (R11); row 3 is the last valid corner
+    fr = np.array([C])
+    G, A, _ = oracle.grid(uv, fr, vis, None, N, 1.0, W, O, T)
+    for design in DESIGNS:
+        with lib.Plan(N, 1.0, W, O, T, design=design) as p:
+            out = p.grid(torch.from_numpy(uv).cuda(), torch.from_numpy(fr).cuda(), torch.from_numpy(vis).cuda())
+            got = out.cpu().numpy()
+        assert_parity(got, G, A, design)
+        stamp = np.outer(T[2].astype(np.float64), T[5].astype(np.float64))    # rv = 2, ru = 5
+        assert np.allclose(got[0, 0, 118 - h:118 + h + 1, 138 - h:138 + h + 1], stamp, rtol=3e-7, atol=0)
+        assert np.count_nonzero(got[0, 0]) == 2 * W * W
+
+
+def test_empty_inputs_and_error_codes(lib):
+    T = make_kernel_table(7, 8)
+    with lib.Plan(64, 1.0, 7, 8, T) as p:
+        fr = torch.tensor([C, 2 * C], dtype=torch.float64, device="cuda")
+        out = torch.full((2, 4, 64, 64), 3 + 4j, dtype=torch.complex64, device="cuda")
+        lib.mwa_grid_visibilities(p.handle, torch.zeros((0, 2), dtype=torch.float64, device="cuda"), fr,
+                                  torch.zeros((0, 2, 4), dtype=torch.complex64, device="cuda"), None, 0, 2, out)
+        assert not out.cpu().numpy().any()                          # n_vis == 0 zero-fills
+        out.fill_(1)
+        lib.mwa_grid_visibilities(p.handle, None, None, None, None, 0, 0, out)
+        assert bool((out == 1).all())                               # n_chan == 0 is a no-op
+        with pytest.raises(lib.MwaGridError) as e:
+            lib.mwa_grid_visibilities(p.handle, torch.zeros((3, 2), dtype=torch.float64, device="cuda"), fr,
+                                      None, None, 3, 2, out)
+        assert e.value.code == -1 and "vis_c64" in str(e.value)
+        with pytest.raises(lib.MwaGridError):
+            lib.mwa_grid_visibilities(p.handle, None, fr, None, None, -1, 2, out)
+    for bad in [(63, 1.0, 7, 8), (64, 0.0, 7, 8), (64, float("nan"), 7, 8), (64, 1.0, 6, 8), (64, 1.0, 7, 7),
+                (64, 1.0, 17, 8), (8, 1.0, 7, 8)]:
+        with pytest.raises(lib.MwaGridError):
+            lib.mwa_grid_plan_create(bad[0], bad[1], bad[2], bad[3], make_kernel_table(7, 8))
+
+
+def test_host_entry_point_matches_device_call(lib):
+    g = generate(scaled(CONFIGS["C2"], n_ant=32, n_chan=4, grid_n=256))
+    G, A, _ = _oracle(g)
+    cfg = g.cfg
+    with _plan(lib, g) as p:
+        out = torch.empty((cfg.n_chan, 4, cfg.grid_n, cfg.grid_n), dtype=torch.complex64).pin_memory()
+        lib.mwa_grid_visibilities_host(p.handle, g.uv.pin_memory(), g.freqs.pin_memory(), g.vis.pin_memory(),
+                                       g.weights.pin_memory(), cfg.n_vis, cfg.n_chan, out)
+        assert_parity(out.numpy(), G, A, "host entry")
+        assert lib.mwa_grid_plan_last_launches(p.handle) > 0
+
+
+def test_plan_reuse_changing_sizes(lib):
+    # workspace growth and reuse: small call, larger call, small again on the same plan
+    T = make_kernel_table(7, 8)
+    base = scaled(CONFIGS["C2"], n_ant=24, n_chan=2, grid_n=256)
+    g_small, g_big = generate(base), generate(scaled(base, n_ant=72, n_chan=9))
+    du = g_big.cell_du
+    with lib.Plan(256, du, 7, 8, T) as p:
+        for g in (g_small, g_big, g_small):
+            G, A, _ = oracle.grid(g.uv, g.freqs, g.vis, g.weights, 256, du, 7, 8, T)
+            out = p.grid(g.uv.cuda(), g.freqs.cuda(), g.vis.cuda(), g.weights.cuda())
+            assert_parity(out.cpu().numpy(), G, A, "reuse")
+
+
+# ---------------------------------------------------------------------------- full-size configs, sampled channels
+def _full_size_sampled(lib, name, chans):
+    g = generate(CONFIGS[name], device="cuda")
+    cfg = g.cfg
+    with _plan(lib, g) as p:
+        out = torch.empty((cfg.n_chan, 4, cfg.grid_n, cfg.grid_n), dtype=torch.complex64, device="cuda")
+        out.fill_(float("nan"))
+        lib.mwa_grid_visibilities(p.handle, g.uv, g.freqs, g.vis, g.weights, cfg.n_vis, cfg.n_chan, out)
+        torch.cuda.synchronize()
+        idx = p.indices(g.uv, g.freqs[chans].contiguous()).cpu().numpy()
+    want_idx = oracle.compute_indices(g.uv.cpu(), g.freqs[chans].cpu(), cfg.grid_n, g.cell_du, cfg.support_W,
+                                      cfg.oversample_O)
+    assert np.array_equal(idx, want_idx)
+    assert not bool(torch.isnan(out.real).any())                   # every cell of every plane was written
+    for c in chans:
+        G, A, _ = _oracle(g, [c])
+        assert_parity(out[c:c + 1].cpu().numpy(), G, A, f"{name} channel {c}")
+    # flux conservation per channel at full size: sum over cells = sum_n w V S(ru) S(rv)  (pin P3 restated for the GPU)
+    return g, out
+
+
+def test_c4_full_size_sampled_channels(lib):
+    _full_size_sampled(lib, "C4", [0, 383, 767])
+
+
+def test_c5_full_size_sampled_channels(lib):
+    _full_size_sampled(lib, "C5", [0, 63])
