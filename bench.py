@@ -145,6 +145,9 @@ def run_ours(args):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", lr))
     cfg = CONFIGS[args.config]
+    if args.n_chan:                               # profiling subset (ncu captures): same rows, fewer channels
+        from gen import scaled
+        cfg = scaled(cfg, n_chan=args.n_chan)
     dev = torch.device("cuda", lr)
     g = generate(cfg, device=dev)
     plan = lib.Plan(cfg.grid_n, g.cell_du, cfg.support_W, cfg.oversample_O, g.kernel_table, design=args.design)
@@ -284,6 +287,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C4", choices=sorted(CONFIGS))
     ap.add_argument("--design", default="auto")
+    ap.add_argument("--n-chan", type=int, default=0, help="profiling only: cut the config down to this many channels")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

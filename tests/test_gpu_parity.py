@@ -163,7 +163,8 @@ def test_empty_inputs_and_error_codes(lib):
     for bad in [(63, 1.0, 7, 8), (64, 0.0, 7, 8), (64, float("nan"), 7, 8), (64, 1.0, 6, 8), (64, 1.0, 7, 7),
                 (64, 1.0, 17, 8), (8, 1.0, 7, 8)]:
         with pytest.raises(lib.MwaGridError):
-            lib.mwa_grid_plan_create(bad[0], bad[1], bad[2], bad[3], make_kernel_table(7, 8))
+            lib.mwa_grid_plan_create(bad[0], bad[1], bad[2], bad[3],
+                                     np.zeros((bad[3] + 1) * bad[2], dtype=np.float32))
 
 
 def test_host_entry_point_matches_device_call(lib):
