@@ -189,6 +189,7 @@ def run_ours(args):
         stage.append(lib.mwa_grid_plan_stage_ms(plan.handle))
         launches += lib.mwa_grid_plan_last_launches(plan.handle)
     barrier()
+    ran = lib.mwa_grid_plan_last_design(plan.handle)           # resolves AUTO (device-side choice)
     clocks = sampler.stop() if rank == 0 else None
     t = torch.tensor([tot_ms], dtype=torch.float64, device=dev)
     if dist is not None:
@@ -239,13 +240,13 @@ def run_ours(args):
         "config": {"workload": f"{cfg.name}: {cfg.n_ant} antennas, {cfg.n_vis} rows x {cfg.n_chan} channels x 4 pol, "
                                f"grid {cfg.grid_n}^2 per channel and pol, kernel {cfg.support_W}x{cfg.support_W} "
                                f"oversampling {cfg.oversample_O}",
-                   "design": args.design, "per_gpu": "one full snapshot per rank",
+                   "design": args.design, "design_ran": ran, "per_gpu": "one full snapshot per rank",
                    "cache": "256 MB L2 flush before every step" if small else
                             f"inputs+outputs {alg_bytes / 1e9:.1f} GB >> 126 MB L2, no flush"},
         "kernel_tap_updates_per_sec": value * cfg.support_W ** 2,
         "stage_ms": {"scale_and_binning": bin_ms, "gridding": grid_ms},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None, "peak_source": peak_src, "kernel": "gather_kernel" if args.design in ("auto", "gather") else args.design,
+                     "traffic": None, "peak_source": peak_src, "kernel": {"gather": "gather_kernel", "chan": "chan_kernel", "atomic": "atomic_grid_kernel"}.get(ran, ran),
                      "algorithmic_bytes_per_launch": alg_bytes,
                      "whole_call_frac": alg_bytes / (ms_per_step * 1e-3) / 1e9 / peak,
                      "fp32_time_ms_at_74.45_TFLOPs": cfg.tap_updates() * 4 / 74.45e12 * 1e3},

@@ -31,13 +31,16 @@ enum {
 };
 
 /* Gridding designs (BASELINE.json north_star asks for the comparison).
- * AUTO picks GATHER.  All designs give the same indices and values within the fp32 tolerance. */
+ * AUTO picks CHAN when the call has >= 8 channels and every group of 32 adjacent channels moves a baseline
+ * by at most 6 cells at the grid edge (decided on the device from freqs), else GATHER.
+ * All designs give the same indices and values within the fp32 tolerance. */
 enum {
     MWA_GRID_DESIGN_AUTO = 0,
     MWA_GRID_DESIGN_ATOMIC = 1, /* K0: memset + one global red.add per tap (bring-up / ncu baseline)        */
     MWA_GRID_DESIGN_SMEM = 2,   /* K3a: tile-owned shared-memory accumulation (red.shared.add.f32)          */
     MWA_GRID_DESIGN_ROMEIN = 3, /* K3b: threads own cells modulo W, register-resident, flush on cell change */
-    MWA_GRID_DESIGN_GATHER = 4  /* K3c: tile-owned, threads own a 4x2 cell block in registers (product)     */
+    MWA_GRID_DESIGN_GATHER = 4, /* K3c: tile-owned, lane = 4x2 cell block of one channel, registers              */
+    MWA_GRID_DESIGN_CHAN = 5    /* K5: tile-owned, lane = channel (32 adjacent channels per warp), registers     */
 };
 
 /* Create a plan (R5-R8 for the table).
@@ -81,6 +84,10 @@ int mwa_grid_compute_indices(mwa_grid_plan* plan, const double* uv_f64, const do
 
 /* Select the gridding design (MWA_GRID_DESIGN_*).  Takes effect at the next call. */
 int mwa_grid_plan_set_design(mwa_grid_plan* plan, int design);
+
+/* The design the last gridding call on this plan actually ran (MWA_GRID_DESIGN_*).  For AUTO this reads the
+ * device-side decision back and therefore synchronises with the device; negative on error. */
+int mwa_grid_plan_last_design(mwa_grid_plan* plan);
 
 /* When enabled, every mwa_grid_visibilities call records CUDA events around its stages on `stream`.
  * mwa_grid_plan_stage_ms then synchronises on them and writes up to `n` floats (milliseconds) of the LAST

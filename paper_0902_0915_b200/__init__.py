@@ -8,14 +8,14 @@ import os as _os
 
 from . import _build
 
-if _os.path.exists(_build.LIB):
+if _os.path.exists(_build.LIB) and not _build.needs_build():
     from .binding import *  # noqa: F401,F403
     from .binding import Plan, MwaGridError, DESIGNS, EXPORTS  # noqa: F401
 else:
     def __getattr__(name):
-        if _os.path.exists(_build.LIB):      # built since the package was imported
+        if _os.path.exists(_build.LIB) and not _build.needs_build():      # built since the package was imported
             from . import binding
             globals().update({k: getattr(binding, k) for k in dir(binding) if not k.startswith("__")})
             return globals()[name]
-        raise ImportError(f"{_build.LIB} is missing: the CUDA library has not been built "
+        raise ImportError(f"{_build.LIB} is missing or older than its sources: the CUDA library has not been built "
                           "(run `python -m paper_0902_0915_b200._build`); there is no CPU fallback")

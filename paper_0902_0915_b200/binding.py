@@ -11,9 +11,9 @@ import torch
 
 from . import _build
 
-DESIGN_AUTO, DESIGN_ATOMIC, DESIGN_SMEM, DESIGN_ROMEIN, DESIGN_GATHER = 0, 1, 2, 3, 4
+DESIGN_AUTO, DESIGN_ATOMIC, DESIGN_SMEM, DESIGN_ROMEIN, DESIGN_GATHER, DESIGN_CHAN = 0, 1, 2, 3, 4, 5
 DESIGNS = {"auto": DESIGN_AUTO, "atomic": DESIGN_ATOMIC, "smem": DESIGN_SMEM, "romein": DESIGN_ROMEIN,
-           "gather": DESIGN_GATHER}
+           "gather": DESIGN_GATHER, "chan": DESIGN_CHAN}
 
 if not os.path.exists(_build.LIB):
     raise ImportError(f"{_build.LIB} is missing: the CUDA library has not been built "
@@ -40,12 +40,14 @@ _lib.mwa_grid_plan_stage_ms.argtypes = [_P, _P, _I]
 _lib.mwa_grid_plan_stage_ms.restype = _I
 _lib.mwa_grid_plan_last_launches.argtypes = [_P]
 _lib.mwa_grid_plan_last_launches.restype = _I
+_lib.mwa_grid_plan_last_design.argtypes = [_P]
+_lib.mwa_grid_plan_last_design.restype = _I
 _lib.mwa_grid_last_error.argtypes = []
 _lib.mwa_grid_last_error.restype = ctypes.c_char_p
 
 EXPORTS = ["mwa_grid_plan_create", "mwa_grid_plan_destroy", "mwa_grid_visibilities", "mwa_grid_visibilities_host",
            "mwa_grid_compute_indices", "mwa_grid_plan_set_design", "mwa_grid_plan_set_profiling",
-           "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_last_error"]
+           "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_plan_last_design", "mwa_grid_last_error"]
 
 
 class MwaGridError(RuntimeError):
@@ -145,6 +147,12 @@ def mwa_grid_plan_stage_ms(plan):
 
 def mwa_grid_plan_last_launches(plan) -> int:
     return int(_lib.mwa_grid_plan_last_launches(plan))
+
+
+def mwa_grid_plan_last_design(plan) -> str:
+    """Name of the design the last gridding call ran (resolves AUTO; synchronises)."""
+    code = _check(_lib.mwa_grid_plan_last_design(plan))
+    return {v: k for k, v in DESIGNS.items()}[code]
 
 
 class Plan:

@@ -1,6 +1,7 @@
 // abi.cu - the extern "C" boundary declared in include/mwa_grid.h: argument checks, workspace, dispatch.
 #include <cmath>
 #include <cstdint>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -43,6 +44,7 @@ static int ensure_workspace(Plan* p, long long n_vis, int n_chan) {
         ws.cap_chan = n_chan;
     }
     if (!ws.d_scale_ref && !ensure(ws.d_scale_ref, 1, "scale_ref")) return MWA_GRID_ERR_NOMEM;
+    if (!ws.d_dispatch && !ensure(ws.d_dispatch, 1, "dispatch")) return MWA_GRID_ERR_NOMEM;
     const int nb = (p->geom.N + kBucketCells - 1) / kBucketCells;
     const int n_buckets = nb * nb;
     if (n_buckets > ws.cap_buckets) {
@@ -79,9 +81,6 @@ static int check_common(Plan* p, const double* uv, const double* freqs, long lon
     return MWA_GRID_OK;
 }
 
-static int resolve_design(const Plan* p) {
-    return p->design == MWA_GRID_DESIGN_AUTO ? MWA_GRID_DESIGN_GATHER : p->design;
-}
 
 static int grid_device(Plan* p, const double* uv, const double* freqs, const float* vis, const float* weights,
                        long long n_vis, int n_chan, float* grid, cudaStream_t st) {
@@ -96,7 +95,7 @@ static int grid_device(Plan* p, const double* uv, const double* freqs, const flo
         cudaEventRecord(p->ev[0], st);
     }
     if (!launch_scale(p, freqs, n_chan, st)) return MWA_GRID_ERR_CUDA;
-    const int design = resolve_design(p);
+    const int design = p->design;
     if (design != MWA_GRID_DESIGN_ATOMIC && n_vis > 0)
         if (!launch_binning(p, uv, n_vis, n_chan, st)) return MWA_GRID_ERR_CUDA;
     if (prof) cudaEventRecord(p->ev[1], st);
@@ -109,7 +108,15 @@ static int grid_device(Plan* p, const double* uv, const double* freqs, const flo
             case MWA_GRID_DESIGN_ATOMIC: ok = launch_atomic(p, uv, vis, weights, n_vis, n_chan, grid, st); break;
             case MWA_GRID_DESIGN_SMEM: ok = launch_smem(p, vis, weights, n_vis, n_chan, grid, st); break;
             case MWA_GRID_DESIGN_ROMEIN: ok = launch_romein(p, vis, weights, n_vis, n_chan, grid, st); break;
-            case MWA_GRID_DESIGN_GATHER: ok = launch_gather(p, vis, weights, n_vis, n_chan, grid, st); break;
+            case MWA_GRID_DESIGN_GATHER: ok = launch_gather(p, vis, weights, n_vis, n_chan, grid, nullptr, st); break;
+            case MWA_GRID_DESIGN_CHAN: ok = launch_chan(p, vis, weights, n_vis, n_chan, grid, nullptr, st); break;
+            case MWA_GRID_DESIGN_AUTO:
+                // the choice is made on the device by scale_kernel (the host never reads freqs): both kernels
+                // are enqueued and the one that was not picked returns at once
+                ok = true;
+                if (chan_supported(p, n_chan)) ok = launch_chan(p, vis, weights, n_vis, n_chan, grid, p->ws.d_dispatch, st);
+                ok = ok && launch_gather(p, vis, weights, n_vis, n_chan, grid, p->ws.d_dispatch, st);
+                break;
             default: set_error("unknown design"); return MWA_GRID_ERR_INVALID;
         }
     }
@@ -144,8 +151,15 @@ mwa_grid_plan* mwa_grid_plan_create(int grid_n, double cell_du, int support_W, i
     p->geom.W = support_W;
     p->geom.h = (support_W - 1) / 2;
     p->geom.O = oversample_O;
+    p->geom.o_shift = -1;
+    for (int k = 1; k <= 6; ++k)
+        if ((1 << k) == oversample_O) p->geom.o_shift = k;
     p->geom.inv_du = 1.0 / cell_du;
     p->cell_du = cell_du;
+    if (const char* e = std::getenv("MWA_GRID_CHAN_PASSES")) {      // tuning knob for experiments: 1, 2 or 4
+        const int v = std::atoi(e);
+        if (v == 1 || v == 2 || v == 4) p->chan_passes = v;
+    }
     const size_t n = (size_t)(oversample_O + 1) * support_W;
     p->h_table = new (std::nothrow) float[n];
     if (!p->h_table) { set_error("out of host memory"); delete p; return nullptr; }
@@ -165,7 +179,7 @@ void mwa_grid_plan_destroy(mwa_grid_plan* plan) {
     Plan* p = reinterpret_cast<Plan*>(plan);
     Workspace& ws = p->ws;
     void* ptrs[] = {p->d_table, ws.d_scale, ws.d_scale_ref, ws.d_bucket_count, ws.d_bucket_cursor, ws.d_perm,
-                    ws.d_uv_sorted, ws.d_tile_order, ws.d_tile_weight, ws.d_misc, ws.d_stage};
+                    ws.d_uv_sorted, ws.d_tile_order, ws.d_tile_weight, ws.d_misc, ws.d_dispatch, ws.d_stage};
     for (void* q : ptrs)
         if (q) cudaFree(q);
     for (auto& e : p->ev)
@@ -176,7 +190,7 @@ void mwa_grid_plan_destroy(mwa_grid_plan* plan) {
 
 int mwa_grid_plan_set_design(mwa_grid_plan* plan, int design) {
     if (!plan) { set_error("plan is NULL"); return MWA_GRID_ERR_INVALID; }
-    if (design < MWA_GRID_DESIGN_AUTO || design > MWA_GRID_DESIGN_GATHER) { set_error("unknown design"); return MWA_GRID_ERR_INVALID; }
+    if (design < MWA_GRID_DESIGN_AUTO || design > MWA_GRID_DESIGN_CHAN) { set_error("unknown design"); return MWA_GRID_ERR_INVALID; }
     reinterpret_cast<Plan*>(plan)->design = design;
     return MWA_GRID_OK;
 }
@@ -205,6 +219,16 @@ int mwa_grid_plan_stage_ms(mwa_grid_plan* plan, float* out_ms, int n) {
 
 int mwa_grid_plan_last_launches(const mwa_grid_plan* plan) {
     return plan ? reinterpret_cast<const Plan*>(plan)->last_launches : 0;
+}
+
+int mwa_grid_plan_last_design(mwa_grid_plan* plan) {
+    if (!plan) { set_error("plan is NULL"); return MWA_GRID_ERR_INVALID; }
+    Plan* p = reinterpret_cast<Plan*>(plan);
+    if (p->design != MWA_GRID_DESIGN_AUTO) return p->design;
+    if (!p->ws.d_dispatch) { set_error("no gridding call recorded"); return MWA_GRID_ERR_INVALID; }
+    int v = 0;
+    if (!cuda_ok(cudaMemcpy(&v, p->ws.d_dispatch, sizeof(int), cudaMemcpyDeviceToHost), "read dispatch")) return MWA_GRID_ERR_CUDA;
+    return v == 1 ? MWA_GRID_DESIGN_CHAN : MWA_GRID_DESIGN_GATHER;
 }
 
 int mwa_grid_compute_indices(mwa_grid_plan* plan, const double* uv_f64, const double* freqs, long long n_vis,

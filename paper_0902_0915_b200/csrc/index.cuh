@@ -17,6 +17,7 @@ struct GridGeom {
     int W;          // kernel support (odd)
     int h;          // (W - 1) / 2
     int O;          // oversampling (even)
+    int o_shift;    // log2(O) when O is a power of two, else -1 (the division below then takes the generic path)
     double inv_du;  // 1.0 / cell_du, computed once on the host in fp64
 };
 
@@ -35,8 +36,9 @@ __device__ __forceinline__ bool index_1d(double x, const GridGeom& g, int& i, in
     const int sgn = (__double2hiint(x) < 0) ? -1 : 1;        // signbit, so -0.0 behaves like the CPU's signbit()
     const double shifted = __dadd_rn(__dmul_rn(a, (double)g.O), 0.5);
     const int ka = __double2int_rd(shifted);                 // floor; < N/2 * O + 1 <= 2^20, fits easily
-    int q = ka / g.O;
-    int rem = ka - q * g.O;
+    int q, rem;                                              // non-negative integer division ka = q * O + rem
+    if (g.o_shift >= 0) { q = ka >> g.o_shift; rem = ka & (g.O - 1); }
+    else { q = ka / g.O; rem = ka - q * g.O; }
     if (rem > g.O / 2) { q += 1; rem -= g.O; }
     const int ii = g.N / 2 + sgn * q;
     if (ii - g.h < 0 || ii + g.h > g.N - 1) return false;    // R11: whole stamp must be inside

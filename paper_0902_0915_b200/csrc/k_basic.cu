@@ -8,15 +8,33 @@
 
 namespace mwa {
 
-__global__ void scale_kernel(const double* __restrict__ freqs, int n_chan, double* __restrict__ scale,
-                             double* __restrict__ scale_ref) {
+// Also picks the gridder for MWA_GRID_DESIGN_AUTO on the device (the host never reads freqs): K5 (k_chan.cu)
+// needs the 32 channels of a group to see a baseline at almost the same cell.  drift = largest displacement,
+// in cells at the grid edge, between the extreme channels of any group.
+constexpr double kChanMaxDriftCells = 6.0;
+constexpr int kChanMinChannels = 8;
+
+__global__ void scale_kernel(const double* __restrict__ freqs, int n_chan, int half_n, int chan_ok,
+                             double* __restrict__ scale, double* __restrict__ scale_ref, int* __restrict__ dispatch) {
     // one block; also reduces max(s_c) for the binning reference scale
     __shared__ double smax[32];
+    __shared__ int bad;
+    if (threadIdx.x == 0) bad = 0;
+    __syncthreads();
     double m = 0.0;
     for (int c = threadIdx.x; c < n_chan; c += blockDim.x) {
         const double s = channel_scale(freqs[c]);
         scale[c] = s;
         m = fmax(m, fabs(s));
+    }
+    for (int g0 = threadIdx.x * 32; g0 < n_chan; g0 += blockDim.x * 32) {      // one 32-channel group per thread
+        double lo = channel_scale(freqs[g0]), hi = lo;
+        for (int c = g0 + 1; c < min(n_chan, g0 + 32); ++c) {
+            const double s = channel_scale(freqs[c]);
+            lo = fmin(lo, s);
+            hi = fmax(hi, s);
+        }
+        if (!(lo > 0.0) || !((hi - lo) / hi * (double)half_n <= kChanMaxDriftCells)) atomicOr(&bad, 1);
     }
     for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
     if ((threadIdx.x & 31) == 0) smax[threadIdx.x >> 5] = m;
@@ -24,12 +42,16 @@ __global__ void scale_kernel(const double* __restrict__ freqs, int n_chan, doubl
     if (threadIdx.x < 32) {
         m = (threadIdx.x < (blockDim.x >> 5)) ? smax[threadIdx.x] : 0.0;
         for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
-        if (threadIdx.x == 0) *scale_ref = m;
+        if (threadIdx.x == 0) {
+            *scale_ref = m;
+            *dispatch = (chan_ok && n_chan >= kChanMinChannels && !bad) ? 1 : 0;
+        }
     }
 }
 
 bool launch_scale(Plan* p, const double* freqs, int n_chan, cudaStream_t st) {
-    scale_kernel<<<1, 256, 0, st>>>(freqs, n_chan, p->ws.d_scale, p->ws.d_scale_ref);
+    scale_kernel<<<1, 256, 0, st>>>(freqs, n_chan, p->geom.N / 2, chan_supported(p, n_chan) ? 1 : 0, p->ws.d_scale,
+                                    p->ws.d_scale_ref, p->ws.d_dispatch);
     p->last_launches += 1;
     return cuda_ok(cudaGetLastError(), "scale_kernel");
 }

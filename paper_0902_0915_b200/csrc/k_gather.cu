@@ -35,6 +35,7 @@ struct GatherParams {
     const double2* uv_sorted;   // [n_vis]
     const int* tile_order;      // [nt*nt]
     int* counter;               // work counter
+    const int* dispatch;        // AUTO: run only if *dispatch == 0 (see scale_kernel); null = always
     const float4* vis;          // [n_vis][n_chan][2] float4
     const float* weights;       // [n_vis][n_chan] or null
     const float* table;         // [(O+1)][W]
@@ -84,6 +85,7 @@ constexpr int kBiasU = 16, kBiasV = 16;   // floats; keep the stored offsets non
 
 __global__ void __launch_bounds__(kWarpsPerCta * 32)
 gather_kernel(const GatherParams P) {
+    if (P.dispatch != nullptr && *P.dispatch != 0) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const GridGeom g = P.g;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -296,7 +298,7 @@ gather_kernel(const GatherParams P) {
 }
 
 bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
-                   cudaStream_t st) {
+                   const int* dispatch, cudaStream_t st) {
     (void)n_vis;
     GatherParams P;
     P.g = p->geom;
@@ -307,6 +309,7 @@ bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, i
     P.uv_sorted = p->ws.d_uv_sorted;
     P.tile_order = p->ws.d_tile_order;
     P.counter = p->ws.d_misc;
+    P.dispatch = dispatch;
     P.vis = (const float4*)vis;
     P.weights = w;
     P.table = p->d_table;

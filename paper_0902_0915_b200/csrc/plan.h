@@ -26,6 +26,7 @@ struct Workspace {
     int* d_tile_order = nullptr;     // [n_tiles] tile ids, heaviest first
     int* d_tile_weight = nullptr;    // [n_tiles]
     int* d_misc = nullptr;           // small counters
+    int* d_dispatch = nullptr;       // [1] design picked on the device for AUTO: 0 = gather (K3c), 1 = chan (K5)
     int cap_tiles = 0;
     // host-buffer entry point staging
     void* d_stage = nullptr;
@@ -38,6 +39,7 @@ struct Plan {
     float* d_table = nullptr;        // [(O+1)][W] as given
     float* h_table = nullptr;        // host copy
     int design = 0;
+    int chan_passes = 2;             // K5 tile height = 4 * chan_passes (1, 2 or 4)
     int device = 0;
     int sm_count = 148;
     Workspace ws;
@@ -58,7 +60,10 @@ bool launch_atomic(Plan* p, const double* uv, const float* vis, const float* w, 
                    float* grid, cudaStream_t st);
 bool launch_binning(Plan* p, const double* uv, long long n_vis, int n_chan, cudaStream_t st);
 bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
-                   cudaStream_t st);
+                   const int* dispatch, cudaStream_t st);
+bool chan_supported(const Plan* p, int n_chan);
+bool launch_chan(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
+                 const int* dispatch, cudaStream_t st);
 bool launch_smem(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                  cudaStream_t st);
 bool launch_romein(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,

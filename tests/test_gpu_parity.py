@@ -14,7 +14,7 @@ from parity import assert_parity
 
 pytestmark = pytest.mark.gpu
 C = 299792458.0
-DESIGNS = ["atomic", "gather"]
+DESIGNS = ["atomic", "gather", "chan"]
 
 
 @pytest.fixture(scope="module")
@@ -111,6 +111,48 @@ def test_c3_whole(lib, design):
         out = p.grid(g.uv, g.freqs, g.vis, g.weights)
         torch.cuda.synchronize()
     assert_parity(out.cpu().numpy(), G, A, f"C3 {design}")
+
+
+@pytest.mark.parametrize("design", ["chan", "auto"])
+@pytest.mark.parametrize("kw", [
+    dict(n_ant=96, core_ant=48, n_chan=70, grid_n=512),            # 3 channel groups, the last one ragged (6 channels)
+    dict(n_ant=200, core_ant=100, n_chan=33, grid_n=250),          # dense core -> multi-batch tiles; ragged grid edge
+])
+def test_fine_channels_c4_shape(lib, design, kw):
+    # C4's 40 kHz channel spacing: the regime K5 (lane = channel) is built for, and the one AUTO must pick it in
+    cfg = scaled(CONFIGS["C4"], **kw)
+    cfg = scaled(cfg, f_lo_hz=155e6, f_hi_hz=155e6 + 40e3 * (cfg.n_chan - 1))
+    g = generate(cfg)
+    G, A, _ = _oracle(g)
+    _to_dev(g)
+    with _plan(lib, g, design) as p:
+        out = p.grid(g.uv, g.freqs, g.vis, g.weights)
+        torch.cuda.synchronize()
+        assert lib.mwa_grid_plan_last_design(p.handle) == "chan"
+        assert_parity(out.cpu().numpy(), G, A, f"fine channels {design}")
+        out2 = p.grid(g.uv, g.freqs, g.vis, None)
+        assert_parity(out2.cpu().numpy(), G, A, f"fine channels {design} null weights")
+
+
+def test_auto_picks_gather_for_coarse_channels(lib):
+    g = generate(scaled(CONFIGS["C2"], n_ant=32, n_chan=16, grid_n=256))     # 16 channels over 140-170 MHz
+    _to_dev(g)
+    with _plan(lib, g, "auto") as p:
+        p.grid(g.uv, g.freqs, g.vis, g.weights)
+        assert lib.mwa_grid_plan_last_design(p.handle) == "gather"
+
+
+@pytest.mark.parametrize("passes", ["1", "4"])
+def test_chan_other_tile_heights(lib, passes, monkeypatch):
+    monkeypatch.setenv("MWA_GRID_CHAN_PASSES", passes)
+    cfg = scaled(CONFIGS["C5"], n_ant=24, core_ant=12, n_chan=40, grid_n=512, f_lo_hz=150e6, f_hi_hz=150e6 + 39 * 40e3)
+    g = generate(cfg)
+    G, A, _ = _oracle(g)
+    _to_dev(g)
+    with _plan(lib, g, "chan") as p:
+        out = p.grid(g.uv, g.freqs, g.vis, g.weights)
+        torch.cuda.synchronize()
+    assert_parity(out.cpu().numpy(), G, A, f"chan passes={passes}")
 
 
 def test_c2_whole(lib):
