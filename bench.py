@@ -138,6 +138,9 @@ def run_ours(args):
     ws, rank, lr = _dist()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    from paper_0902_0915_b200 import _build
+    if rank == 0:
+        _build.build()                            # no-op when the in-tree library is newer than its sources
     import paper_0902_0915_b200 as lib
     torch.cuda.set_device(lr)
     dist = None
@@ -145,9 +148,10 @@ def run_ours(args):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", lr))
     cfg = CONFIGS[args.config]
-    if args.n_chan:                               # profiling subset (ncu captures): same rows, fewer channels
-        from gen import scaled
-        cfg = scaled(cfg, n_chan=args.n_chan)
+    if args.n_chan:                               # profiling subset (ncu captures): same rows, the TOP n channels
+        from gen import scaled                    # of the band at the config's own channel spacing (same du)
+        step_hz = (cfg.f_hi_hz - cfg.f_lo_hz) / max(cfg.n_chan - 1, 1)
+        cfg = scaled(cfg, n_chan=args.n_chan, f_lo_hz=cfg.f_hi_hz - step_hz * (args.n_chan - 1))
     dev = torch.device("cuda", lr)
     g = generate(cfg, device=dev)
     plan = lib.Plan(cfg.grid_n, g.cell_du, cfg.support_W, cfg.oversample_O, g.kernel_table, design=args.design)

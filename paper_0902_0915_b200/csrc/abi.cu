@@ -156,10 +156,6 @@ mwa_grid_plan* mwa_grid_plan_create(int grid_n, double cell_du, int support_W, i
         if ((1 << k) == oversample_O) p->geom.o_shift = k;
     p->geom.inv_du = 1.0 / cell_du;
     p->cell_du = cell_du;
-    if (const char* e = std::getenv("MWA_GRID_CHAN_PASSES")) {      // tuning knob for experiments: 1, 2 or 4
-        const int v = std::atoi(e);
-        if (v == 1 || v == 2 || v == 4) p->chan_passes = v;
-    }
     const size_t n = (size_t)(oversample_O + 1) * support_W;
     p->h_table = new (std::nothrow) float[n];
     if (!p->h_table) { set_error("out of host memory"); delete p; return nullptr; }

@@ -39,7 +39,6 @@ struct Plan {
     float* d_table = nullptr;        // [(O+1)][W] as given
     float* h_table = nullptr;        // host copy
     int design = 0;
-    int chan_passes = 2;             // K5 tile height = 4 * chan_passes (1, 2 or 4)
     int device = 0;
     int sm_count = 148;
     Workspace ws;
