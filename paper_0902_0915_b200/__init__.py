@@ -1,21 +1,16 @@
 """B200-native convolutional visibility gridding (arXiv 0902.0915) behind a C ABI.
 
 `binding` mirrors include/mwa_grid.h one to one; `Plan` is a convenience holder for a plan handle.
-There is no CPU path.  Without the built CUDA library only `_build` (the nvcc build step) is importable;
-touching anything else raises ImportError.
+There is no CPU path.  Importing the package builds the CUDA library in-tree when it is missing or older
+than its sources (nvcc, sm_100a only - `_build.py`); if that fails the import fails: nothing here works
+without the built library.
 """
-import os as _os
-
 from . import _build
 
-if _os.path.exists(_build.LIB) and not _build.needs_build():
-    from .binding import *  # noqa: F401,F403
-    from .binding import Plan, MwaGridError, DESIGNS, EXPORTS  # noqa: F401
-else:
-    def __getattr__(name):
-        if _os.path.exists(_build.LIB) and not _build.needs_build():      # built since the package was imported
-            from . import binding
-            globals().update({k: getattr(binding, k) for k in dir(binding) if not k.startswith("__")})
-            return globals()[name]
-        raise ImportError(f"{_build.LIB} is missing or older than its sources: the CUDA library has not been built "
-                          "(run `python -m paper_0902_0915_b200._build`); there is no CPU fallback")
+try:
+    _build.build()
+except Exception as _e:  # no nvcc, compile error, ...
+    raise ImportError(f"{_build.LIB} could not be built ({_e!r}); there is no CPU fallback") from _e
+
+from .binding import *  # noqa: F401,F403,E402
+from .binding import Plan, MwaGridError, DESIGNS, EXPORTS  # noqa: F401,E402

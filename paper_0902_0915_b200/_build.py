@@ -30,7 +30,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     """Compile every CUDA source for sm_100a into one shared library; returns its path."""
     if force or needs_build():
         srcs = [os.path.join(CSRC, s) for s in SOURCES if os.path.exists(os.path.join(CSRC, s))]
-        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + srcs
+        extra = os.environ.get("MWA_EXTRA_NVCC", "").split()          # e.g. -DMWA_CHAN_TIMING (debug builds only)
+        cmd = [_nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + srcs
         subprocess.run(cmd, check=True, cwd=CSRC)
     return LIB
 

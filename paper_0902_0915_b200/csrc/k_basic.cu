@@ -15,9 +15,11 @@ constexpr double kChanMaxDriftCells = 6.0;
 constexpr int kChanMinChannels = 8;
 
 __global__ void scale_kernel(const double* __restrict__ freqs, int n_chan, int half_n, int chan_ok,
-                             double* __restrict__ scale, double* __restrict__ scale_ref, int* __restrict__ dispatch) {
+                             double* __restrict__ scale, double* __restrict__ scale_ref, int* __restrict__ dispatch,
+                             double4* __restrict__ group) {
     // one block; also reduces max(s_c) for the binning reference scale
     __shared__ double smax[32];
+    __shared__ double sref;
     __shared__ int bad;
     if (threadIdx.x == 0) bad = 0;
     __syncthreads();
@@ -44,14 +46,30 @@ __global__ void scale_kernel(const double* __restrict__ freqs, int n_chan, int h
         for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
         if (threadIdx.x == 0) {
             *scale_ref = m;
+            sref = m;
             *dispatch = (chan_ok && n_chan >= kChanMinChannels && !bad) ? 1 : 0;
         }
+    }
+    __syncthreads();
+    // per 32-channel group (K5): {s_lo, s_hi, s_ref / s_lo, s_ref / s_hi}; the last two are NaN when the group cannot
+    // be back-projected to the reference scale (non-positive scales), which makes K5 scan every bucket
+    for (int g0 = threadIdx.x * 32; g0 < n_chan; g0 += blockDim.x * 32) {
+        double lo = channel_scale(freqs[g0]), hi = lo;
+        for (int c = g0 + 1; c < min(n_chan, g0 + 32); ++c) {
+            const double s = channel_scale(freqs[c]);
+            lo = fmin(lo, s);
+            hi = fmax(hi, s);
+        }
+        const double rl = lo / sref, rh = hi / sref;
+        const bool ok = rl > 1e-3 && rh <= 1.0 + 1e-9;
+        const double nan = __longlong_as_double(0x7ff8000000000000LL);
+        group[g0 >> 5] = make_double4(lo, hi, ok ? 1.0 / rl : nan, ok ? 1.0 / rh : nan);
     }
 }
 
 bool launch_scale(Plan* p, const double* freqs, int n_chan, cudaStream_t st) {
     scale_kernel<<<1, 256, 0, st>>>(freqs, n_chan, p->geom.N / 2, chan_supported(p, n_chan) ? 1 : 0, p->ws.d_scale,
-                                    p->ws.d_scale_ref, p->ws.d_dispatch);
+                                    p->ws.d_scale_ref, p->ws.d_dispatch, (double4*)p->ws.d_group);
     p->last_launches += 1;
     return cuda_ok(cudaGetLastError(), "scale_kernel");
 }

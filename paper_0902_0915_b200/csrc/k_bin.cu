@@ -74,7 +74,7 @@ __global__ void bin_scan_kernel(int* __restrict__ count, int n, int* __restrict_
 
 __global__ void bin_scatter_kernel(GridGeom g, const double2* __restrict__ uv, const double* __restrict__ s_ref_p,
                                    int n_vis, int nb, int* __restrict__ cursor, int* __restrict__ perm,
-                                   double2* __restrict__ uv_sorted) {
+                                   double2* __restrict__ uv_sorted, double4* __restrict__ row_sorted) {
     const double s_ref = *s_ref_p;
     for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < n_vis; n += gridDim.x * blockDim.x) {
         const double2 p = uv[n];
@@ -83,6 +83,7 @@ __global__ void bin_scatter_kernel(GridGeom g, const double2* __restrict__ uv, c
         const int pos = atomicAdd(&cursor[by * nb + bx], 1);
         perm[pos] = n;
         uv_sorted[pos] = p;
+        row_sorted[pos] = make_double4(p.x, p.y, (double)n, 0.0);      // K5: uv and row id in one 32 B record
     }
 }
 
@@ -143,7 +144,7 @@ bool launch_binning(Plan* p, const double* uv, long long n_vis, int /*n_chan*/, 
                                              ws.d_bucket_count);
     bin_scan_kernel<<<1, 1024, 0, st>>>(ws.d_bucket_count, n_buckets, ws.d_bucket_cursor);
     bin_scatter_kernel<<<blocks, 256, 0, st>>>(p->geom, (const double2*)uv, ws.d_scale_ref, (int)n_vis, nb,
-                                               ws.d_bucket_cursor, ws.d_perm, ws.d_uv_sorted);
+                                               ws.d_bucket_cursor, ws.d_perm, ws.d_uv_sorted, (double4*)ws.d_row_sorted);
     int* hist = ws.d_misc + 16;
     int tblocks = (nt * nt + 255) / 256;
     if (tblocks > p->sm_count * 8) tblocks = p->sm_count * 8;

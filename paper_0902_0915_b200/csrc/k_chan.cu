@@ -4,53 +4,59 @@
 // at almost the same (u, v) (u_lambda = u_m * nu / c moves by 2.6e-4 of its radius per channel), and every
 // channel owns its own grid (BASELINE.json configs[3]).  K5 turns that into SIMD lanes:
 //
-//   CTA  = one 16 x 8 cell tile  x  one group of 32 adjacent channels (all 4 polarisations); 16 warps
+//   CTA  = one 16 x 4 cell tile x one SUPER-GROUP of 4 x 32 adjacent channels; 8 warps, 2 CTAs per SM
 //   warp = one 4x2-cell block of the tile
-//   lane = one channel of the group; the lane keeps 8 cells x 4 pol x (re, im) = 64 fp32 accumulators
-//          of ITS channel's grid in registers.
+//   lane = one channel of the current 32-channel group; the lane keeps 8 cells x 4 pol x (re, im) = 64 fp32
+//          accumulators of ITS channel's grid in registers.
 //
 // All 32 lanes of a warp therefore walk (almost) the same list of baseline rows - the walk is balanced by
 // construction, where K3c (k_gather.cu: lane = block, same channel) leaves 23 of 32 lanes idle on Poisson
 // noise (profiles/r01_gather_v0_c4x64.md).  A lane whose stamp misses the block at its own channel reads
 // zeros from the padded kernel table, so there is no divergence in the FMA body at all.
 //
-//   A1 (thread = candidate row): walk the uv buckets (k_bin.cu) that can reach the tile at ANY scale of the
-//       channel group, keep the rows whose stamp can overlap the tile (conservative fp64 interval test);
-//       compaction is by ballot + prefix, so the hit order - and with it every fp32 sum - is deterministic.
-//   A2 (warp = hit, lane = channel): coalesced load of the hit's 32 visibilities (1 KB) and weights, w*V
-//       staged in shared memory; the exact index function (index.cuh) per (row, channel) gives the lane a
-//       packed pair of kernel-table offsets ("geo"); per hit a bit mask of the blocks any lane touches.
+//   A1 (thread = candidate row, once per super-group): walk the uv buckets (k_bin.cu) that can reach the tile
+//       at ANY scale of the 128 channels, keep the rows whose stamp can overlap the tile (conservative fp64
+//       interval test).  Then, per 32-channel group:
+//   F  (thread = list entry): the same interval test against the group's own scale range, from shared memory.
+//       Compaction is by ballot + prefix in both steps, so the hit order is a pure function of the sorted rows.
+//   A2 (warp = hit, lane = channel): cp.async of the hit's 32 visibilities (1 KB) and weights into shared
+//       memory; while they fly, the exact index function (index.cuh) per (row, channel) gives the lane a packed
+//       pair of kernel-table offsets ("geo") and the hit a bit mask of the blocks any lane touches; then w*V
+//       in place.
 //   B  (warp = block, lane = channel): for every hit that touches the block: 2 x LDS.128 of w*V, LDS.128 +
 //       LDS.64 of kernel taps from shifted zero-padded table copies, 8 FMUL, 32 FFMA2 (fma.rn.f32x2).
 //   write-out: registers -> padded shared-memory stage (aliasing the w*V batch) -> full 128 B lines of one
 //       (channel, pol, row) with streaming stores; every cell of grid_out is written exactly once, zeros
 //       included (R10).
 //
-// No atomics on grid data, no fp64 in phase B, no global loads in phase B.
+// No atomics on grid data, no fp64 and no global loads in phase B.  A tile too dense for the list falls back
+// to one A1 sweep per group with flushes.  Two co-resident CTAs hide each other's barriers and load latency.
+#include <cstdio>
 #include "plan.h"
 
 namespace mwa {
 
-constexpr int kcWarps = 16;
+constexpr int kcWarps = 8;
 constexpr int kcThreads = kcWarps * 32;
 constexpr int kcLanes = 32;            // channels per group
-constexpr int kcTileX = 16, kcTileY = 8;
-constexpr int kcListCap = 1024;        // candidate hits kept per A1 sweep (row id + uv)
-constexpr int kcBatch = 128;           // hits per A2/B batch (w*V: 128 KB, geo: 16 KB)
+constexpr int kcSuper = 4;             // groups per super-group (one A1 sweep serves them all)
+constexpr int kcTileX = 16, kcTileY = 4;
+constexpr int kcListCap = 512;         // candidate hits kept per A1 sweep (row id + uv)
+constexpr int kcBatch = 64;            // hits per A2/B batch (w*V: 64 KB, geo: 8 KB)
+constexpr int kcGroupCap = 64;         // channel groups whose scale table is cached in shared memory (2048 channels)
 constexpr int kcPadU = 20;             // zero padding (floats) in front of a u table row
 constexpr int kcPadV = kcTileY;        // ... of a v table row
 constexpr int kcZeroFloats = 32;       // all-zero block behind each table (target of an invalid lane's geo)
-constexpr int kcChanStride = 4 * kcTileY * 128 + 16;   // stage bytes per channel: 4 pol x 8 rows x 128 B, +16 B so
+constexpr int kcChanStride = 4 * kcTileY * 128 + 16;   // stage bytes per channel: 4 pol x 4 rows x 128 B, +16 B so
                                                        // that the 8 lanes of an STS.128 quarter-warp hit all 32 banks
-constexpr int kcStageBytes = kcLanes * kcChanStride;   // 131,584 B >= the 131,072 B of a w*V batch
+constexpr int kcStageBytes = kcLanes * kcChanStride;   // 66,048 B >= the 65,536 B of a w*V batch
 
 struct ChanParams {
     GridGeom g;
     const double* scale;        // [n_chan]
-    const double* scale_ref;    // [1]
+    const double4* group;       // [n_groups] s_lo, s_hi, s_ref / s_lo, s_ref / s_hi (scale_kernel)
     const int* bucket_start;    // [nb*nb + 1]
-    const int* perm;            // [n_vis]
-    const double2* uv_sorted;   // [n_vis]
+    const double4* row_sorted;  // [n_vis] (u, v, row id, 0) of the bucket-sorted rows
     const int* tile_order;      // [nt*nt] 16x16 super-tiles, heaviest first
     int* counter;               // work counter
     const int* dispatch;        // device-side design choice (AUTO): run only if *dispatch == dispatch_want; null = always
@@ -83,19 +89,25 @@ __device__ __forceinline__ void c_st_stream_v4(float* p, float4 v) {
     asm volatile("st.global.cs.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
 }
 
+
 struct ChanSmem {                 // fixed part; the table copies follow it in dynamic shared memory
     __align__(16) unsigned char zs[kcStageBytes];   // w*V of the batch [hit][lane][8 floats]; aliased by the write-out stage
     unsigned geo[kcBatch * kcLanes];
-    double2 hit_uv[kcListCap];
+    float wts[kcBatch * kcLanes];                   // weights of the batch [hit][lane] (cp.async target)
+    double2 hit_uv[kcListCap];                      // the list: uv (metres) and original row of each candidate hit
     int hit_row[kcListCap];
+    unsigned short sel[kcListCap];                  // list entries selected for the current group, in list order
     unsigned hit_mask[kcBatch];
     unsigned char vlist[kcWarps][kcBatch];          // per warp: the batch hits that touch its block, in order
+    unsigned char lut_u[32], lut_v[32];             // block masks by stamp origin: [ou + W - 1] -> bx bits, [ov + W - 1] -> by bits (x16)
     int warp_cnt[2][kcWarps];
-    int next_item;
+    int next_item, next_tile;
+    double4 group[kcGroupCap];                      // copy of the per-group scale table (scale_kernel)
+    double sc[kcSuper][kcLanes];                    // channel scales s_c of the current super-group
 };
 
 template <bool HAS_W>
-__global__ void __launch_bounds__(kcThreads, 1)
+__global__ void __launch_bounds__(kcThreads, 2)
 chan_kernel(const __grid_constant__ ChanParams P) {
     if (P.dispatch != nullptr && *P.dispatch != P.dispatch_want) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -126,7 +138,28 @@ chan_kernel(const __grid_constant__ ChanParams P) {
         }
         tv[k] = v;
     }
-    if (tid == 0) S.next_item = atomicAdd(P.counter, 1);
+    if (tid < 32) {                                                  // W <= 15: ou + W - 1 <= 29, ov + W - 1 <= 17
+        const int ou = tid - (W - 1);
+        unsigned mu = 0u, mv = 0u;
+        if (ou < kcTileX) {
+            const int bxl = max(0, ou >> 2), bxh = min(kcTileX / 4 - 1, (ou + W - 1) >> 2);
+            mu = (2u << bxh) - (1u << bxl);
+        }
+        if (ou < kcTileY) {                                           // same index reused as ov
+            const int bl = max(0, ou >> 1), bh = min(kcTileY / 2 - 1, (ou + W - 1) >> 1);
+            for (int b = bl; b <= bh; ++b) mv |= 1u << (4 * b);
+        }
+        S.lut_u[tid] = (unsigned char)mu;
+        S.lut_v[tid] = (unsigned char)mv;
+    }
+    for (int k = tid; k < min(P.n_groups, kcGroupCap); k += kcThreads) S.group[k] = P.group[k];
+    const double4* group = P.n_groups <= kcGroupCap ? S.group : P.group;
+    const int n_sg = (P.n_groups + kcSuper - 1) / kcSuper;
+    if (tid == 0) {
+        const int it = atomicAdd(P.counter, 1);
+        S.next_item = it;
+        S.next_tile = it < P.n_items ? P.tile_order[(it / n_sg) >> 2] : 0;
+    }
     __syncthreads();
 
     const int bx = warp & 3, by = warp >> 2;
@@ -135,44 +168,55 @@ chan_kernel(const __grid_constant__ ChanParams P) {
     const unsigned tv_s = (unsigned)__cvta_generic_to_shared(tv) + 8u * by;
     const unsigned zs_s = (unsigned)__cvta_generic_to_shared(S.zs) + 32u * lane;
     const unsigned geo_s = (unsigned)__cvta_generic_to_shared(S.geo) + 4u * lane;
+    const unsigned wt_s = (unsigned)__cvta_generic_to_shared(S.wts) + 4u * lane;
     const unsigned zero_geo = (unsigned)(P.n_tu * 4) | ((unsigned)(P.n_tv * 4) << 16);
     const size_t plane = (size_t)N * N;
     const unsigned lt_mask = (1u << lane) - 1u;
     const unsigned full = 0xffffffffu;
 
+#ifdef MWA_CHAN_TIMING
+    long long tph[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, tlast = clock64();
+#define TPH(k) { const long long tn = clock64(); tph[k] += tn - tlast; tlast = tn; }
+#else
+#define TPH(k)
+#endif
     int item = S.next_item;
     while (item < P.n_items) {
-        int next_item = 0;
+        int next_item = 0, next_tile = 0;
+        bool have_next_tile = false;
         if (tid == 0) next_item = atomicAdd(P.counter, 1);           // latency hidden behind this item
-        const int grp = item % P.n_groups;
-        const int ts = item / P.n_groups;
-        const int tile = P.tile_order[ts >> 1];
+        const int sgi = item % n_sg;
+        const int ts = item / n_sg;
+        const int tile = S.next_tile;
+        if (warp < kcSuper)      // channel scales of the super-group; visible after the barriers of the sweep
+            S.sc[warp][lane] = P.scale[min((sgi * kcSuper + warp) * kcLanes + lane, P.n_chan - 1)];
         const int ty = tile / P.nt, tx = tile - ty * P.nt;
-        const int X0 = tx * kcTileX, Y0 = ty * 16 + (ts & 1) * kcTileY;
-        const int c0 = grp * kcLanes;
-        const bool cvalid = c0 + lane < P.n_chan;
-        const int cc = cvalid ? c0 + lane : P.n_chan - 1;
+        const int X0 = tx * kcTileX, Y0 = ty * 16 + (ts & 3) * kcTileY;
         if (Y0 < N) {
-            const double sc = P.scale[cc];
+            // per-group state (set in the group loop below, captured by reference)
+            int c0 = 0, cc = 0, gslot = 0;
+            bool cvalid = false;
             u64 acc[2][4][4];   // [row i][col j][pol] = (re, im) of the lane's channel
-#pragma unroll
-            for (int i = 0; i < 2; ++i)
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-#pragma unroll
-                    for (int p = 0; p < 4; ++p) acc[i][j][p] = 0ull;
 
-            // ---- A2: hits [b0, b0 + n) of the list, warp = hit, lane = channel
+            // ---- A2: n hits starting at selection entry b0, warp = hit, lane = channel
             auto phase_a2 = [&](int b0, int n) {
+                // (i) cp.async the warp's visibilities (32 lanes x 32 B = 1 KB per hit) and weights straight into
+                //     shared memory: every copy of the batch is in flight while (ii) does the fp64 index work
                 for (int hh = warp; hh < n; hh += kcWarps) {
-                    const double2 p = S.hit_uv[b0 + hh];
-                    const size_t sidx = (size_t)S.hit_row[b0 + hh] * P.n_chan + cc;
-                    float4 va = __ldg(P.vis + 2 * sidx), vb = __ldg(P.vis + 2 * sidx + 1);
-                    float wt = 1.0f;
-                    if (HAS_W) wt = __ldg(P.weights + sidx);
+                    const size_t sidx = (size_t)S.hit_row[S.sel[b0 + hh]] * P.n_chan + cc;
+                    const float4* src = P.vis + 2 * sidx;
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(zs_s + 1024u * hh), "l"(src) : "memory");
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(zs_s + 1024u * hh + 16u), "l"(src + 1) : "memory");
+                    if (HAS_W)
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(wt_s + 128u * hh), "l"(P.weights + sidx) : "memory");
+                }
+                asm volatile("cp.async.commit_group;" ::: "memory");
+                // (ii) exact indices -> geo, block mask
+                const double sc = S.sc[gslot][lane];
+                for (int hh = warp; hh < n; hh += kcWarps) {
+                    const double2 p = S.hit_uv[S.sel[b0 + hh]];
                     SampleIndex s;
-                    unsigned geo = zero_geo;
-                    int ulo = 1 << 20, uhi = -(1 << 20), vlo = 1 << 20, vhi = -(1 << 20);
+                    unsigned geo = zero_geo, mask = 0u;
                     if (cvalid && sample_index(p.x, p.y, sc, P.g, s)) {
                         const int ou = s.iu - hW - X0, ov = s.iv - hW - Y0;        // stamp origin relative to the tile
                         if (ou > -W && ou < kcTileX && ov > -W && ov < kcTileY) {
@@ -180,32 +224,26 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                             const int offu = (su * O1 + s.ru) * P.rlu + (kcPadU - ou - su);
                             const int offv = (sv * O1 + s.rv) * P.rlv + (kcPadV - ov - sv);
                             geo = (unsigned)(offu * 4) | ((unsigned)(offv * 4) << 16);
-                            ulo = uhi = ou;
-                            vlo = vhi = ov;
+                            mask = (unsigned)S.lut_v[ov + W - 1] * (unsigned)S.lut_u[ou + W - 1];
                         }
                     }
-                    // blocks touched by any lane: bounding box of the lanes' stamps (a superset costs only zeros)
-                    ulo = __reduce_min_sync(full, ulo);
-                    uhi = __reduce_max_sync(full, uhi);
-                    vlo = __reduce_min_sync(full, vlo);
-                    vhi = __reduce_max_sync(full, vhi);
-                    if (HAS_W) {
+                    mask = __reduce_or_sync(full, mask);                           // blocks touched by any lane
+                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(geo_s + 128u * hh), "r"(geo) : "memory");
+                    if (lane == 0) S.hit_mask[hh] = mask;
+                }
+                // (iii) w * V in place; each lane touches only the 36 bytes its own cp.asyncs wrote
+                asm volatile("cp.async.wait_group 0;" ::: "memory");
+                if (HAS_W) {
+                    for (int hh = warp; hh < n; hh += kcWarps) {
+                        float4 va, vb;
+                        float wt;
+                        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(va.x), "=f"(va.y), "=f"(va.z), "=f"(va.w) : "r"(zs_s + 1024u * hh));
+                        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(vb.x), "=f"(vb.y), "=f"(vb.z), "=f"(vb.w) : "r"(zs_s + 1024u * hh + 16u));
+                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(wt) : "r"(wt_s + 128u * hh));
                         va.x *= wt; va.y *= wt; va.z *= wt; va.w *= wt;
                         vb.x *= wt; vb.y *= wt; vb.z *= wt; vb.w *= wt;
-                    }
-                    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(zs_s + 1024u * hh), "f"(va.x), "f"(va.y), "f"(va.z), "f"(va.w) : "memory");
-                    asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(zs_s + 1024u * hh + 16u), "f"(vb.x), "f"(vb.y), "f"(vb.z), "f"(vb.w) : "memory");
-                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(geo_s + 128u * hh), "r"(geo) : "memory");
-                    if (lane == 0) {
-                        unsigned mask = 0u;
-                        if (ulo <= uhi) {
-                            const int bxl = max(0, ulo >> 2), bxh = min(3, (uhi + W - 1) >> 2);
-                            const int bl = max(0, vlo >> 1), bh = min(3, (vhi + W - 1) >> 1);
-                            const unsigned m4 = (2u << bxh) - (1u << bxl);
-                            const unsigned rows = 0x1111u & (0xFFFFu >> (12 - 4 * bh)) & (0xFFFFu << (4 * bl));
-                            mask = rows * m4;
-                        }
-                        S.hit_mask[hh] = mask;
+                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(zs_s + 1024u * hh), "f"(va.x), "f"(va.y), "f"(va.z), "f"(va.w) : "memory");
+                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(zs_s + 1024u * hh + 16u), "f"(vb.x), "f"(vb.y), "f"(vb.z), "f"(vb.w) : "memory");
                     }
                 }
             };
@@ -257,33 +295,65 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                 }
             };
 
-            // the first n entries of the hit list, in batches: A2 | sync | B | sync
-            auto process_list = [&](int n) {
+            // the first n selection entries, in batches: A2 | sync | B | sync
+            auto process_sel = [&](int n) {
                 for (int b0 = 0; b0 < n; b0 += kcBatch) {
                     const int nbat = min(kcBatch, n - b0);
+                    TPH(0)
                     phase_a2(b0, nbat);
+                    TPH(1)
                     __syncthreads();
+                    TPH(2)
                     phase_b(nbat);
+                    TPH(3)
                     __syncthreads();
+                    TPH(4)
                 }
             };
 
-            // ---- scale range of the group and the bucket window it implies at the reference scale
-            double s_lo = sc, s_hi = sc;
+            int par = 0;                                                   // parity of the warp_cnt buffer in use
+            // deterministic CTA-wide compaction step: returns the slot of this thread's hit (or -1) and adds the
+            // chunk's hit count to `count`; contains one __syncthreads
+            auto compact = [&](bool hit, int& count) -> int {
+                const unsigned ball = __ballot_sync(full, hit);
+                if (lane == 0) S.warp_cnt[par][warp] = __popc(ball);
+                __syncthreads();
+                const int cv = lane < kcWarps ? S.warp_cnt[par][lane] : 0;
+                int ci = cv;
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                s_lo = fmin(s_lo, __shfl_xor_sync(full, s_lo, o));
-                s_hi = fmax(s_hi, __shfl_xor_sync(full, s_hi, o));
-            }
-            const double halfN = (double)(N / 2);
-            const double cx0 = (double)X0 - halfN, cx1 = (double)(X0 + kcTileX - 1) - halfN;
-            const double cy0 = (double)Y0 - halfN, cy1 = (double)(Y0 + kcTileY - 1) - halfN;
-            int wx0 = 0, wx1 = P.nb - 1, wy0 = 0, wy1 = P.nb - 1;
-            {
-                const double s_ref = *P.scale_ref;
-                const double rl = s_lo / s_ref, rh = s_hi / s_ref;
-                if (rl > 1e-3 && rh <= 1.0 + 1e-9) {
-                    const double pad = (double)hW + 1.25, il = 1.0 / rl, ih = 1.0 / rh;
+                for (int o = 1; o < kcWarps; o <<= 1) {
+                    const int t = __shfl_up_sync(full, ci, o);
+                    if (lane >= o) ci += t;
+                }
+                const int tot = __shfl_sync(full, ci, kcWarps - 1);
+                const int wbase = __shfl_sync(full, ci - cv, warp);
+                const int slot = hit ? count + wbase + __popc(ball & lt_mask) : -1;
+                count += tot;
+                par ^= 1;
+                return slot;
+            };
+            auto reaches_tile = [&](const double2 p, double s_lo, double s_hi) -> bool {
+                const double halfN = (double)(N / 2);
+                const double cx0 = (double)X0 - halfN, cx1 = (double)(X0 + kcTileX - 1) - halfN;
+                const double cy0 = (double)Y0 - halfN, cy1 = (double)(Y0 + kcTileY - 1) - halfN;
+                const double xa = __dmul_rn(__dmul_rn(p.x, s_lo), P.g.inv_du), xb = __dmul_rn(__dmul_rn(p.x, s_hi), P.g.inv_du);
+                const double ya = __dmul_rn(__dmul_rn(p.y, s_lo), P.g.inv_du), yb = __dmul_rn(__dmul_rn(p.y, s_hi), P.g.inv_du);
+                return fmax(xa, xb) + P.reach >= cx0 && fmin(xa, xb) - P.reach <= cx1 &&
+                       fmax(ya, yb) + P.reach >= cy0 && fmin(ya, yb) - P.reach <= cy1;
+            };
+
+            // ---- A1: bucket sweep for scales in [s_lo, s_hi] (il, ih = s_ref / s_lo, s_ref / s_hi, NaN = scan all).
+            // flush = false: fill the list (entries beyond its capacity are counted but dropped -> overflow);
+            // flush = true : the list is pushed through A2 + B whenever it would overflow (one group only).
+            // Returns the number of entries in the list (or the overflowing count); n_seen totals all hits.
+            int n_seen = 0;
+            auto sweep = [&](double s_lo, double s_hi, double il, double ih, bool flush) -> int {
+                int wx0 = 0, wx1 = P.nb - 1, wy0 = 0, wy1 = P.nb - 1;
+                if (il == il && ih == ih) {
+                    const double halfN = (double)(N / 2);
+                    const double cx0 = (double)X0 - halfN, cx1 = (double)(X0 + kcTileX - 1) - halfN;
+                    const double cy0 = (double)Y0 - halfN, cy1 = (double)(Y0 + kcTileY - 1) - halfN;
+                    const double pad = (double)hW + 1.25;
                     const double ax = cx0 - pad, bxx = cx1 + pad, ay = cy0 - pad, byy = cy1 + pad;
                     const double ib = 1.0 / kBucketCells, top = (double)(P.nb - 1);
                     wx0 = (int)fmin(fmax(floor((fmin(ax * il, ax * ih) + halfN) * ib), 0.0), top);
@@ -291,93 +361,80 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                     wy0 = (int)fmin(fmax(floor((fmin(ay * il, ay * ih) + halfN) * ib), 0.0), top);
                     wy1 = (int)fmin(fmax(floor((fmax(byy * il, byy * ih) + halfN) * ib), 0.0), top);
                 }
-            }
-
-            // ---- A1: candidate rows -> hit list (flushed through A2 + B whenever it would overflow)
-            int n_local = 0, n_total = 0, par = 0;
-            for (int rg = wy0; rg <= wy1; rg += 32) {
-                int k0 = 0, len = 0;
-                if (rg + lane <= wy1) {
-                    k0 = __ldg(P.bucket_start + (rg + lane) * P.nb + wx0);
-                    len = __ldg(P.bucket_start + (rg + lane) * P.nb + wx1 + 1) - k0;
-                }
-                int incl = len;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int t = __shfl_up_sync(full, incl, o);
-                    if (lane >= o) incl += t;
-                }
-                const int total = __shfl_sync(full, incl, 31);
-                const int excl = incl - len;
-                for (int base = 0; base < total; base += kcThreads) {
-                    if (n_local + kcThreads > kcListCap) {                 // uniform: n_local is the same in all threads
-                        __syncthreads();
-                        process_list(n_local);
-                        n_local = 0;
+                int n_local = 0;
+                for (int rg = wy0; rg <= wy1; rg += 32) {
+                    int k0 = 0, len = 0;
+                    if (rg + lane <= wy1) {
+                        k0 = __ldg(P.bucket_start + (rg + lane) * P.nb + wx0);
+                        len = __ldg(P.bucket_start + (rg + lane) * P.nb + wx1 + 1) - k0;
                     }
-                    const int f = base + tid;
-                    bool hit = false;
-                    double2 p = make_double2(0.0, 0.0);
-                    int k = 0;
-                    {
-                        int lo = 0;                                         // smallest r with incl[r] > f
+                    int incl = len;
 #pragma unroll
-                        for (int st = 16; st > 0; st >>= 1) {
-                            const int t = __shfl_sync(full, incl, lo + st - 1);
-                            if (t <= f) lo += st;
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int t = __shfl_up_sync(full, incl, o);
+                        if (lane >= o) incl += t;
+                    }
+                    const int total = __shfl_sync(full, incl, 31);
+                    const int excl = incl - len;
+                    for (int base = 0; base < total; base += kcThreads) {
+                        if (flush && n_local + kcThreads > kcListCap) {       // uniform: n_local is the same in all threads
+                            __syncthreads();
+                            process_sel(n_local);
+                            n_local = 0;
                         }
-                        lo = min(lo, 31);
-                        const int rk0 = __shfl_sync(full, k0, lo), rex = __shfl_sync(full, excl, lo);
-                        k = rk0 + (f - rex);
-                    }
-                    if (f < total) {
-                        p = __ldg(P.uv_sorted + k);
-                        const double xa = __dmul_rn(__dmul_rn(p.x, s_lo), P.g.inv_du), xb = __dmul_rn(__dmul_rn(p.x, s_hi), P.g.inv_du);
-                        const double ya = __dmul_rn(__dmul_rn(p.y, s_lo), P.g.inv_du), yb = __dmul_rn(__dmul_rn(p.y, s_hi), P.g.inv_du);
-                        hit = fmax(xa, xb) + P.reach >= cx0 && fmin(xa, xb) - P.reach <= cx1 &&
-                              fmax(ya, yb) + P.reach >= cy0 && fmin(ya, yb) - P.reach <= cy1;
-                    }
-                    const unsigned ball = __ballot_sync(full, hit);
-                    if (lane == 0) S.warp_cnt[par][warp] = __popc(ball);
-                    __syncthreads();
-                    int cv = lane < kcWarps ? S.warp_cnt[par][lane] : 0, ci = cv;
+                        const int f = base + tid;
+                        bool hit = false;
+                        double2 p = make_double2(0.0, 0.0);
+                        int k = 0;
+                        {
+                            int lo = 0;                                         // smallest r with incl[r] > f
 #pragma unroll
-                    for (int o = 1; o < kcWarps; o <<= 1) {
-                        const int t = __shfl_up_sync(full, ci, o);
-                        if (lane >= o) ci += t;
+                            for (int st = 16; st > 0; st >>= 1) {
+                                const int t = __shfl_sync(full, incl, lo + st - 1);
+                                if (t <= f) lo += st;
+                            }
+                            lo = min(lo, 31);
+                            const int rk0 = __shfl_sync(full, k0, lo), rex = __shfl_sync(full, excl, lo);
+                            k = rk0 + (f - rex);
+                        }
+                        double rowd = 0.0;
+                        if (f < total) {
+                            const double4 rec = P.row_sorted[k];
+                            p = make_double2(rec.x, rec.y);
+                            rowd = rec.z;
+                            hit = reaches_tile(p, s_lo, s_hi);
+                        }
+                        const int before = n_local;
+                        const int slot = compact(hit, n_local);
+                        n_seen += n_local - before;
+                        if (slot >= 0 && slot < kcListCap) {
+                            S.hit_uv[slot] = p;
+                            S.hit_row[slot] = (int)rowd;
+                            S.sel[slot] = (unsigned short)slot;
+                        }
                     }
-                    const int tot = __shfl_sync(full, ci, kcWarps - 1);
-                    const int wbase = __shfl_sync(full, ci - cv, warp);
-                    if (hit) {
-                        const int slot = n_local + wbase + __popc(ball & lt_mask);
-                        S.hit_uv[slot] = p;
-                        S.hit_row[slot] = __ldg(P.perm + k);
-                    }
-                    n_local += tot;
-                    n_total += tot;
-                    par ^= 1;
                 }
-            }
-            __syncthreads();                                               // list complete; previous item's stage reads done
-            process_list(n_local);
+                __syncthreads();                                           // list complete and visible
+                return n_local;
+            };
 
-            // ---- a5: write the tile of all 32 channels and 4 pols, once
-            if (n_total > 0) {
+            // ---- a5: write the lane-channel tiles of the current group, once (zeros when nothing reached the tile)
+            auto write_out = [&](bool any) {
+                if (any) {
 #pragma unroll
-                for (int pol = 0; pol < 4; ++pol)
+                    for (int pol = 0; pol < 4; ++pol)
 #pragma unroll
-                    for (int i = 0; i < 2; ++i) {
-                        float a0, a1, a2, a3, b0, b1, b2, b3;
-                        c_unpack2(acc[i][0][pol], a0, a1); c_unpack2(acc[i][1][pol], a2, a3);
-                        c_unpack2(acc[i][2][pol], b0, b1); c_unpack2(acc[i][3][pol], b2, b3);
-                        unsigned char* dst = S.zs + lane * kcChanStride + (pol * kcTileY + 2 * by + i) * 128 + bx * 32;
-                        *reinterpret_cast<float4*>(dst) = make_float4(a0, a1, a2, a3);
-                        *reinterpret_cast<float4*>(dst + 16) = make_float4(b0, b1, b2, b3);
-                    }
-                __syncthreads();
-            }
-            {
-                const int j = tid & 7, row = (tid >> 3) & 7, q0 = tid >> 6;      // 16 B chunk, tile row, (channel, pol) slot
+                        for (int i = 0; i < 2; ++i) {
+                            float a0, a1, a2, a3, b0, b1, b2, b3;
+                            c_unpack2(acc[i][0][pol], a0, a1); c_unpack2(acc[i][1][pol], a2, a3);
+                            c_unpack2(acc[i][2][pol], b0, b1); c_unpack2(acc[i][3][pol], b2, b3);
+                            unsigned char* dst = S.zs + lane * kcChanStride + (pol * kcTileY + 2 * by + i) * 128 + bx * 32;
+                            *reinterpret_cast<float4*>(dst) = make_float4(a0, a1, a2, a3);
+                            *reinterpret_cast<float4*>(dst + 16) = make_float4(b0, b1, b2, b3);
+                        }
+                    __syncthreads();
+                }
+                const int j = tid & 7, row = (tid >> 3) & 3, q0 = tid >> 5;       // 16 B chunk, tile row, (channel, pol) slot
                 const int y = Y0 + row, x = X0 + 2 * j, pol = q0 & 3;
                 if (y < N && x < N) {
                     const unsigned char* src = S.zs + (q0 >> 2) * kcChanStride + (pol * kcTileY + row) * 128 + j * 16;
@@ -386,20 +443,86 @@ chan_kernel(const __grid_constant__ ChanParams P) {
 #pragma unroll 4
                     for (int ch = q0 >> 2; ch < nch; ch += 2) {
                         float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-                        if (n_total > 0) v = *reinterpret_cast<const float4*>(src);
+                        if (any) v = *reinterpret_cast<const float4*>(src);
                         c_st_stream_v4(dst, v);
                         src += 2 * kcChanStride;
                         dst += 2 * 4 * plane * 2;
                     }
                 }
+            };
+
+            // ---- the super-group: one sweep over the union of its groups' scale ranges ...
+            const int g_begin = sgi * kcSuper, g_end = min(P.n_groups, g_begin + kcSuper);
+            double u_lo = 0.0, u_hi = 0.0, u_il = 0.0, u_ih = 0.0;
+            for (int g = g_begin; g < g_end; ++g) {
+                const double4 gi = group[g];
+                if (g == g_begin) { u_lo = gi.x; u_hi = gi.y; u_il = gi.z; u_ih = gi.w; }
+                else {
+                    u_lo = fmin(u_lo, gi.x); u_hi = fmax(u_hi, gi.y);
+                    u_il = (gi.z == gi.z && u_il == u_il) ? fmax(u_il, gi.z) : gi.z + u_il;      // NaN is sticky
+                    u_ih = (gi.w == gi.w && u_ih == u_ih) ? fmin(u_ih, gi.w) : gi.w + u_ih;
+                }
+            }
+            TPH(10)
+            const int n_super = (g_end - g_begin > 1) ? sweep(u_lo, u_hi, u_il, u_ih, false) : kcListCap + 1;
+            TPH(7)
+            const bool per_group_sweep = n_super > kcListCap;              // too dense for the list (or a single group)
+            if (tid == 0 && next_item < P.n_items) next_tile = P.tile_order[(next_item / n_sg) >> 2];   // the atomic has landed by now
+            have_next_tile = true;
+
+            // ... then group by group: select, A2 + B, write
+            for (int g = g_begin; g < g_end; ++g) {
+                c0 = g * kcLanes;
+                gslot = g - g_begin;
+                cvalid = c0 + lane < P.n_chan;
+                cc = cvalid ? c0 + lane : P.n_chan - 1;
+#pragma unroll
+                for (int i = 0; i < 2; ++i)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+#pragma unroll
+                        for (int p = 0; p < 4; ++p) acc[i][j][p] = 0ull;
+                bool any;
+                if (per_group_sweep) {
+                    n_seen = 0;
+                    TPH(0)
+                    const double4 gi = group[g];
+                    const int n_left = sweep(gi.x, gi.y, gi.z, gi.w, true);
+                    TPH(6)
+                    process_sel(n_left);
+                    any = n_seen > 0;
+                } else {
+                    int n_sel = 0;
+                    const double g_lo = group[g].x, g_hi = group[g].y;
+                    for (int base = 0; base < n_super; base += kcThreads) {
+                        const int i = base + tid;
+                        const bool hit = i < n_super && reaches_tile(S.hit_uv[i], g_lo, g_hi);
+                        const int slot = compact(hit, n_sel);
+                        if (slot >= 0) S.sel[slot] = (unsigned short)i;
+                    }
+                    __syncthreads();
+                    TPH(6)
+                    process_sel(n_sel);
+                    any = n_sel > 0;
+                }
+                TPH(0)
+                write_out(any);
+                TPH(5)
             }
         }   // Y0 < N
-
+        TPH(8)
+        if (!have_next_tile && tid == 0 && next_item < P.n_items) next_tile = P.tile_order[(next_item / n_sg) >> 2];
         __syncthreads();
-        if (tid == 0) S.next_item = next_item;
+        if (tid == 0) { S.next_item = next_item; S.next_tile = next_tile; }
         __syncthreads();
         item = S.next_item;
+        TPH(9)
     }
+#ifdef MWA_CHAN_TIMING
+    if (lane == 0 && (warp == 0 || warp == 5) && (blockIdx.x % 37) == 0)
+        printf("cta %d warp %d: gaps %lld tail %lld itemsync %lld decode %lld |  sweep %lld | filter %lld | A2 %lld | bar %lld | B %lld | bar %lld | write %lld\n", blockIdx.x, warp,
+               tph[0], tph[8], tph[9], tph[10], tph[7], tph[6], tph[1], tph[2], tph[3], tph[4], tph[5]);
+#endif
 }
 
 // Geometry of the padded table copies (see the kernel header).
@@ -430,10 +553,9 @@ bool launch_chan(Plan* p, const float* vis, const float* w, long long n_vis, int
     P.g = p->geom;
     chan_table_geometry(p->geom, P);
     P.scale = p->ws.d_scale;
-    P.scale_ref = p->ws.d_scale_ref;
+    P.group = (const double4*)p->ws.d_group;
     P.bucket_start = p->ws.d_bucket_count;
-    P.perm = p->ws.d_perm;
-    P.uv_sorted = p->ws.d_uv_sorted;
+    P.row_sorted = (const double4*)p->ws.d_row_sorted;
     P.tile_order = p->ws.d_tile_order;
     P.counter = p->ws.d_misc + 1;
     P.dispatch = dispatch;
@@ -447,7 +569,8 @@ bool launch_chan(Plan* p, const float* vis, const float* w, long long n_vis, int
     P.nb = (p->geom.N + kBucketCells - 1) / kBucketCells;
     P.nt = (p->geom.N + kTile - 1) / kTile;
     P.reach = (double)p->geom.h + 0.5 + 0.5 / (double)p->geom.O + 1e-6;
-    const long long n_items = (long long)P.nt * P.nt * 2 * P.n_groups;
+    const int n_sg = (P.n_groups + kcSuper - 1) / kcSuper;
+    const long long n_items = (long long)P.nt * P.nt * (16 / kcTileY) * n_sg;
     if (n_items >= 0x7fffffffLL) { set_error("design CHAN: too many work items"); return false; }
     P.n_items = (int)n_items;
     const size_t smem = chan_smem_bytes(P);
@@ -458,7 +581,11 @@ bool launch_chan(Plan* p, const float* vis, const float* w, long long n_vis, int
             return false;
         attr_set[w ? 1 : 0] = true;
     }
-    long long blocks = p->sm_count;
+    int ctas_per_sm = 0;
+    if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, kcThreads, smem), "chan occupancy"))
+        return false;
+    if (ctas_per_sm < 1) { set_error("chan kernel does not fit on an SM"); return false; }
+    long long blocks = (long long)p->sm_count * ctas_per_sm;
     if (blocks > n_items) blocks = n_items;
     if (blocks < 1) blocks = 1;
     kern<<<(unsigned)blocks, kcThreads, smem, st>>>(P);

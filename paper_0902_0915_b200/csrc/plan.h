@@ -14,6 +14,7 @@ constexpr int kTile = 16;           // gridding tile side in cells (one warp own
 struct Workspace {
     // a1
     double* d_scale = nullptr;       // [n_chan]
+    double* d_group = nullptr;       // [ceil(n_chan / 32)][4] per channel group: s_lo, s_hi, s_ref/s_lo, s_ref/s_hi
     int cap_chan = 0;
     // a3
     double* d_scale_ref = nullptr;   // [1] max over channels of s_c
@@ -22,6 +23,7 @@ struct Workspace {
     int cap_buckets = 0;
     int* d_perm = nullptr;           // [n_vis] row ids sorted by bucket
     double2* d_uv_sorted = nullptr;  // [n_vis] uv of the sorted rows
+    double* d_row_sorted = nullptr;  // [n_vis][4] (u, v, row id, 0) of the sorted rows: one 32 B record per row (K5)
     long long cap_vis = 0;
     int* d_tile_order = nullptr;     // [n_tiles] tile ids, heaviest first
     int* d_tile_weight = nullptr;    // [n_tiles]
