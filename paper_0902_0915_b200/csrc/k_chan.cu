@@ -264,19 +264,35 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                 }
                 __syncwarp();
                 if (cnt == 0) return;
-                unsigned hh = S.vlist[warp][0];
-                unsigned geo;
-                asm volatile("ld.shared.u32 %0, [%1];" : "=r"(geo) : "r"(geo_s + 128u * hh));
+                // software pipeline: the taps and w*V of visit v+1 and the geo of visit v+2 are loaded while the
+                // 32 FFMA2 of visit v issue, so no LDS latency is exposed inside the loop
+                const unsigned char* vl = S.vlist[warp];
+                const int last = cnt - 1;
+                unsigned h1 = vl[min(1, last)], h2 = vl[min(2, last)];
+                unsigned g1;
+                u64 z0, z1, z2, z3;
+                float ku0, ku1, ku2, ku3, kv0, kv1;
+                {
+                    const unsigned h0 = vl[0];
+                    unsigned g0;
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g0) : "r"(geo_s + 128u * h0));
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g1) : "r"(geo_s + 128u * h1));
+                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(z0), "=l"(z1) : "r"(zs_s + 1024u * h0));
+                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(z2), "=l"(z3) : "r"(zs_s + 1024u * h0 + 16u));
+                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(ku0), "=f"(ku1), "=f"(ku2), "=f"(ku3) : "r"(tu_s + (g0 & 0xffffu)));
+                    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(kv0), "=f"(kv1) : "r"(tv_s + (g0 >> 16)));
+                }
                 for (int v = 0; v < cnt; ++v) {
-                    const unsigned hn = S.vlist[warp][min(v + 1, cnt - 1)];
-                    unsigned geon;
-                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(geon) : "r"(geo_s + 128u * hn));
-                    u64 z0, z1, z2, z3;
-                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(z0), "=l"(z1) : "r"(zs_s + 1024u * hh));
-                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(z2), "=l"(z3) : "r"(zs_s + 1024u * hh + 16u));
-                    float ku0, ku1, ku2, ku3, kv0, kv1;
-                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(ku0), "=f"(ku1), "=f"(ku2), "=f"(ku3) : "r"(tu_s + (geo & 0xffffu)));
-                    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(kv0), "=f"(kv1) : "r"(tv_s + (geo >> 16)));
+                    // loads of visit v+1 (harmless repeats of the last visit at the end) and geo of v+2
+                    u64 nz0, nz1, nz2, nz3;
+                    float nku0, nku1, nku2, nku3, nkv0, nkv1;
+                    unsigned g2;
+                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(nz0), "=l"(nz1) : "r"(zs_s + 1024u * h1));
+                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(nz2), "=l"(nz3) : "r"(zs_s + 1024u * h1 + 16u));
+                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(nku0), "=f"(nku1), "=f"(nku2), "=f"(nku3) : "r"(tu_s + (g1 & 0xffffu)));
+                    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(nkv0), "=f"(nkv1) : "r"(tv_s + (g1 >> 16)));
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g2) : "r"(geo_s + 128u * h2));
+                    const unsigned h3 = vl[min(v + 3, last)];
                     const float ku[4] = {ku0, ku1, ku2, ku3};
                     const float kv[2] = {kv0, kv1};
 #pragma unroll
@@ -290,8 +306,9 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                             c_ffma2(acc[i][j][2], kk, z2);
                             c_ffma2(acc[i][j][3], kk, z3);
                         }
-                    hh = hn;
-                    geo = geon;
+                    z0 = nz0; z1 = nz1; z2 = nz2; z3 = nz3;
+                    ku0 = nku0; ku1 = nku1; ku2 = nku2; ku3 = nku3; kv0 = nkv0; kv1 = nkv1;
+                    h1 = h2; h2 = h3; g1 = g2;
                 }
             };
 
