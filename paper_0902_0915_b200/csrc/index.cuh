@@ -47,11 +47,35 @@ __device__ __forceinline__ bool index_1d(double x, const GridGeom& g, int& i, in
     return true;
 }
 
+// The same INDEX(x) for a power-of-two O, written branch-free (K5's inner loop).  Identical results to index_1d:
+//   |x| * O is exact for a power of two, so fma(|x|, O, 0.5) rounds once exactly like the multiply-then-add;
+//   q' = (ka + O/2 - 1) >> log2 O carries exactly when rem > O/2;  rem' = ka - q' * O lies in [-O/2 + 1, O/2];
+//   the sign is re-applied with the two's-complement identity (v ^ m) - m, m = 0 or -1.
+// `origin` receives i - h (the first cell of the stamp); valid iff 0 <= origin <= N - W.
+__device__ __forceinline__ bool index_1d_pow2(double x, const GridGeom& g, int& origin, int& r) {
+    const double a = fabs(x);
+    const bool in = a < (double)(g.N / 2);                    // false for NaN / Inf
+    const int m = __double2hiint(x) >> 31;                    // 0 or -1 (signbit)
+    const int ka = __double2int_rd(__fma_rn(a, (double)g.O, 0.5));
+    const int q = (ka + (g.O / 2 - 1)) >> g.o_shift;
+    const int rem = ka - (q << g.o_shift);
+    origin = g.N / 2 - g.h + ((q ^ m) - m);
+    r = ((rem ^ m) - m) + g.O / 2;
+    return in && (unsigned)origin <= (unsigned)(g.N - g.W);
+}
+
 struct SampleIndex { int iu, iv, ru, rv; };
 
 __device__ __forceinline__ bool sample_index(double um, double vm, double scale, const GridGeom& g, SampleIndex& s) {
     const double x = cell_coord(um, scale, g.inv_du);
     const double y = cell_coord(vm, scale, g.inv_du);
+    if (g.o_shift >= 0) {                                     // uniform branch: every thread of a launch takes the same side
+        int ou, ov, ru, rv;
+        const bool oku = index_1d_pow2(x, g, ou, ru);
+        const bool okv = index_1d_pow2(y, g, ov, rv);
+        s.iu = ou + g.h; s.iv = ov + g.h; s.ru = ru; s.rv = rv;
+        return oku && okv;
+    }
     int iu, ru, iv, rv;
     const bool oku = index_1d(x, g, iu, ru);
     const bool okv = index_1d(y, g, iv, rv);

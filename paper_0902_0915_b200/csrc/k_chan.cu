@@ -180,6 +180,7 @@ chan_kernel(const __grid_constant__ ChanParams P) {
 #else
 #define TPH(k)
 #endif
+
     int item = S.next_item;
     while (item < P.n_items) {
         int next_item = 0, next_tile = 0;
@@ -217,35 +218,22 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                     const double2 p = S.hit_uv[S.sel[b0 + hh]];
                     SampleIndex s;
                     unsigned geo = zero_geo, mask = 0u;
-                    if (cvalid && sample_index(p.x, p.y, sc, P.g, s)) {
-                        const int ou = s.iu - hW - X0, ov = s.iv - hW - Y0;        // stamp origin relative to the tile
-                        if (ou > -W && ou < kcTileX && ov > -W && ov < kcTileY) {
-                            const int su = (kcPadU - ou) & 3, sv = (kcPadV - ov) & 1;
-                            const int offu = (su * O1 + s.ru) * P.rlu + (kcPadU - ou - su);
-                            const int offv = (sv * O1 + s.rv) * P.rlv + (kcPadV - ov - sv);
+                    if (sample_index(p.x, p.y, sc, P.g, s) && cvalid) {
+                        const int tu_ = kcPadU + hW + X0 - s.iu, tv_ = kcPadV + hW + Y0 - s.iv;   // pad - (stamp origin relative to the tile)
+                        const unsigned iu_ = (unsigned)(kcPadU + W - 1 - tu_), iv_ = (unsigned)(kcPadV + W - 1 - tv_);   // ou + W - 1, ov + W - 1
+                        if (iu_ < (unsigned)(kcTileX + W - 1) && iv_ < (unsigned)(kcTileY + W - 1)) {
+                            const int su = tu_ & 3, sv = tv_ & 1;
+                            const int offu = s.ru * P.rlu + tu_ + su * (O1 * P.rlu - 1);
+                            const int offv = s.rv * P.rlv + tv_ + sv * (O1 * P.rlv - 1);
                             geo = (unsigned)(offu * 4) | ((unsigned)(offv * 4) << 16);
-                            mask = (unsigned)S.lut_v[ov + W - 1] * (unsigned)S.lut_u[ou + W - 1];
+                            mask = (unsigned)S.lut_v[iv_] * (unsigned)S.lut_u[iu_];
                         }
                     }
                     mask = __reduce_or_sync(full, mask);                           // blocks touched by any lane
                     asm volatile("st.shared.u32 [%0], %1;" ::"r"(geo_s + 128u * hh), "r"(geo) : "memory");
                     if (lane == 0) S.hit_mask[hh] = mask;
                 }
-                // (iii) w * V in place; each lane touches only the 36 bytes its own cp.asyncs wrote
-                asm volatile("cp.async.wait_group 0;" ::: "memory");
-                if (HAS_W) {
-                    for (int hh = warp; hh < n; hh += kcWarps) {
-                        float4 va, vb;
-                        float wt;
-                        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(va.x), "=f"(va.y), "=f"(va.z), "=f"(va.w) : "r"(zs_s + 1024u * hh));
-                        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(vb.x), "=f"(vb.y), "=f"(vb.z), "=f"(vb.w) : "r"(zs_s + 1024u * hh + 16u));
-                        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(wt) : "r"(wt_s + 128u * hh));
-                        va.x *= wt; va.y *= wt; va.z *= wt; va.w *= wt;
-                        vb.x *= wt; vb.y *= wt; vb.z *= wt; vb.w *= wt;
-                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(zs_s + 1024u * hh), "f"(va.x), "f"(va.y), "f"(va.z), "f"(va.w) : "memory");
-                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(zs_s + 1024u * hh + 16u), "f"(vb.x), "f"(vb.y), "f"(vb.z), "f"(vb.w) : "memory");
-                    }
-                }
+                asm volatile("cp.async.wait_group 0;" ::: "memory");              // visible to the other warps after the barrier
             };
 
             // ---- B: the warp's block against the n hits of the batch; every lane computes, zeros where it misses
@@ -264,52 +252,58 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                 }
                 __syncwarp();
                 if (cnt == 0) return;
-                // software pipeline: the taps and w*V of visit v+1 and the geo of visit v+2 are loaded while the
-                // 32 FFMA2 of visit v issue, so no LDS latency is exposed inside the loop
+                // software pipeline, two visits per trip with two register sets (no rotation moves): the taps, the
+                // weight and the visibility of visit v+1 and the geo of visit v+2 are loaded while the 32 FFMA2 of
+                // visit v issue, so no LDS latency is exposed inside the loop
                 const unsigned char* vl = S.vlist[warp];
                 const int last = cnt - 1;
-                unsigned h1 = vl[min(1, last)], h2 = vl[min(2, last)];
-                unsigned g1;
-                u64 z0, z1, z2, z3;
-                float ku0, ku1, ku2, ku3, kv0, kv1;
+#define K5_LOAD(h, g, Z0, Z1, Z2, Z3, U0, U1, U2, U3, V0, V1, WT)                                                         \
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(Z0), "=l"(Z1) : "r"(zs_s + 1024u * (h)));                       \
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(Z2), "=l"(Z3) : "r"(zs_s + 1024u * (h) + 16u));                 \
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(U0), "=f"(U1), "=f"(U2), "=f"(U3) : "r"(tu_s + ((g) & 0xffffu))); \
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(V0), "=f"(V1) : "r"(tv_s + ((g) >> 16)));                       \
+    if (HAS_W) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(WT) : "r"(wt_s + 128u * (h)));
+#define K5_FMA(Z0, Z1, Z2, Z3, U0, U1, U2, U3, V0, V1, WT)                                                                \
+    {                                                                                                                     \
+        const float kvw[2] = {HAS_W ? V0 * WT : V0, HAS_W ? V1 * WT : V1};                                                \
+        const float kuu[4] = {U0, U1, U2, U3};                                                                            \
+        _Pragma("unroll") for (int i = 0; i < 2; ++i) _Pragma("unroll") for (int j = 0; j < 4; ++j) {                      \
+            const float k = kvw[i] * kuu[j];                                                                              \
+            const u64 kk = c_pack2(k, k);                                                                                 \
+            c_ffma2(acc[i][j][0], kk, Z0);                                                                                \
+            c_ffma2(acc[i][j][1], kk, Z1);                                                                                \
+            c_ffma2(acc[i][j][2], kk, Z2);                                                                                \
+            c_ffma2(acc[i][j][3], kk, Z3);                                                                                \
+        }                                                                                                                 \
+    }
+                u64 az0, az1, az2, az3, bz0, bz1, bz2, bz3;
+                float au0, au1, au2, au3, av0, av1, aw = 1.0f, bu0, bu1, bu2, bu3, bv0, bv1, bw = 1.0f;
+                unsigned h1 = vl[min(1, last)], h2 = vl[min(2, last)], g1, g2;
                 {
                     const unsigned h0 = vl[0];
                     unsigned g0;
                     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g0) : "r"(geo_s + 128u * h0));
                     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g1) : "r"(geo_s + 128u * h1));
-                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(z0), "=l"(z1) : "r"(zs_s + 1024u * h0));
-                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(z2), "=l"(z3) : "r"(zs_s + 1024u * h0 + 16u));
-                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(ku0), "=f"(ku1), "=f"(ku2), "=f"(ku3) : "r"(tu_s + (g0 & 0xffffu)));
-                    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(kv0), "=f"(kv1) : "r"(tv_s + (g0 >> 16)));
+                    K5_LOAD(h0, g0, az0, az1, az2, az3, au0, au1, au2, au3, av0, av1, aw)
                 }
-                for (int v = 0; v < cnt; ++v) {
-                    // loads of visit v+1 (harmless repeats of the last visit at the end) and geo of v+2
-                    u64 nz0, nz1, nz2, nz3;
-                    float nku0, nku1, nku2, nku3, nkv0, nkv1;
-                    unsigned g2;
-                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(nz0), "=l"(nz1) : "r"(zs_s + 1024u * h1));
-                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(nz2), "=l"(nz3) : "r"(zs_s + 1024u * h1 + 16u));
-                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(nku0), "=f"(nku1), "=f"(nku2), "=f"(nku3) : "r"(tu_s + (g1 & 0xffffu)));
-                    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(nkv0), "=f"(nkv1) : "r"(tv_s + (g1 >> 16)));
+#pragma unroll 1
+                for (int v = 0; v < cnt; v += 2) {
+                    // set B <- visit v+1 ; geo of v+2 ; then FMAs of visit v from set A
+                    K5_LOAD(h1, g1, bz0, bz1, bz2, bz3, bu0, bu1, bu2, bu3, bv0, bv1, bw)
                     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g2) : "r"(geo_s + 128u * h2));
                     const unsigned h3 = vl[min(v + 3, last)];
-                    const float ku[4] = {ku0, ku1, ku2, ku3};
-                    const float kv[2] = {kv0, kv1};
-#pragma unroll
-                    for (int i = 0; i < 2; ++i)
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            const float k = kv[i] * ku[j];
-                            const u64 kk = c_pack2(k, k);
-                            c_ffma2(acc[i][j][0], kk, z0);
-                            c_ffma2(acc[i][j][1], kk, z1);
-                            c_ffma2(acc[i][j][2], kk, z2);
-                            c_ffma2(acc[i][j][3], kk, z3);
-                        }
-                    z0 = nz0; z1 = nz1; z2 = nz2; z3 = nz3;
-                    ku0 = nku0; ku1 = nku1; ku2 = nku2; ku3 = nku3; kv0 = nkv0; kv1 = nkv1;
-                    h1 = h2; h2 = h3; g1 = g2;
+                    K5_FMA(az0, az1, az2, az3, au0, au1, au2, au3, av0, av1, aw)
+                    if (v + 1 >= cnt) break;
+                    // set A <- visit v+2 ; geo of v+3 ; then FMAs of visit v+1 from set B
+                    K5_LOAD(h2, g2, az0, az1, az2, az3, au0, au1, au2, au3, av0, av1, aw)
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g1) : "r"(geo_s + 128u * h3));
+                    const unsigned h4 = vl[min(v + 4, last)];
+                    K5_FMA(bz0, bz1, bz2, bz3, bu0, bu1, bu2, bu3, bv0, bv1, bw)
+                    h1 = h3;
+                    h2 = h4;
                 }
+#undef K5_LOAD
+#undef K5_FMA
             };
 
             // the first n selection entries, in batches: A2 | sync | B | sync
@@ -395,7 +389,7 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                     const int excl = incl - len;
                     for (int base = 0; base < total; base += kcThreads) {
                         if (flush && n_local + kcThreads > kcListCap) {       // uniform: n_local is the same in all threads
-                            __syncthreads();
+                                    __syncthreads();
                             process_sel(n_local);
                             n_local = 0;
                         }
@@ -457,7 +451,7 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                     const unsigned char* src = S.zs + (q0 >> 2) * kcChanStride + (pol * kcTileY + row) * 128 + j * 16;
                     float* dst = P.grid + (((size_t)(c0 + (q0 >> 2)) * 4 + pol) * plane + (size_t)y * N + x) * 2;
                     const int nch = min(kcLanes, P.n_chan - c0);
-#pragma unroll 4
+#pragma unroll 8
                     for (int ch = q0 >> 2; ch < nch; ch += 2) {
                         float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
                         if (any) v = *reinterpret_cast<const float4*>(src);
