@@ -98,7 +98,7 @@ static int grid_device(Plan* p, const double* uv, const double* freqs, const flo
     }
     if (!launch_scale(p, freqs, n_chan, st)) return MWA_GRID_ERR_CUDA;
     const int design = p->design;
-    if (design != MWA_GRID_DESIGN_ATOMIC && n_vis > 0)
+    if (design != MWA_GRID_DESIGN_ATOMIC && design != MWA_GRID_DESIGN_ROMEIN && n_vis > 0)
         if (!launch_binning(p, uv, n_vis, n_chan, st)) return MWA_GRID_ERR_CUDA;
     if (prof) cudaEventRecord(p->ev[1], st);
     bool ok = false;
@@ -109,7 +109,7 @@ static int grid_device(Plan* p, const double* uv, const double* freqs, const flo
         switch (design) {
             case MWA_GRID_DESIGN_ATOMIC: ok = launch_atomic(p, uv, vis, weights, n_vis, n_chan, grid, st); break;
             case MWA_GRID_DESIGN_SMEM: ok = launch_smem(p, vis, weights, n_vis, n_chan, grid, st); break;
-            case MWA_GRID_DESIGN_ROMEIN: ok = launch_romein(p, vis, weights, n_vis, n_chan, grid, st); break;
+            case MWA_GRID_DESIGN_ROMEIN: ok = launch_romein(p, uv, vis, weights, n_vis, n_chan, grid, st); break;
             case MWA_GRID_DESIGN_GATHER: ok = launch_gather(p, vis, weights, n_vis, n_chan, grid, nullptr, st); break;
             case MWA_GRID_DESIGN_CHAN: ok = launch_chan(p, vis, weights, n_vis, n_chan, grid, nullptr, st); break;
             case MWA_GRID_DESIGN_AUTO:

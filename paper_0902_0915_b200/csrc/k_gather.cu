@@ -343,14 +343,4 @@ bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, i
     return cuda_ok(cudaGetLastError(), "gather_kernel");
 }
 
-// placeholders until the comparison designs land
-bool launch_smem(Plan*, const float*, const float*, long long, int, float*, cudaStream_t) {
-    set_error("design SMEM is not built yet");
-    return false;
-}
-bool launch_romein(Plan*, const float*, const float*, long long, int, float*, cudaStream_t) {
-    set_error("design ROMEIN is not built yet");
-    return false;
-}
-
 }  // namespace mwa

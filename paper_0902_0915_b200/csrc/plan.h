@@ -67,7 +67,7 @@ bool launch_chan(Plan* p, const float* vis, const float* w, long long n_vis, int
                  const int* dispatch, cudaStream_t st);
 bool launch_smem(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                  cudaStream_t st);
-bool launch_romein(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
+bool launch_romein(Plan* p, const double* uv, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                    cudaStream_t st);
 
 }  // namespace mwa

@@ -14,7 +14,7 @@ from parity import assert_parity
 
 pytestmark = pytest.mark.gpu
 C = 299792458.0
-DESIGNS = ["atomic", "gather", "chan"]
+DESIGNS = ["atomic", "smem", "romein", "gather", "chan"]
 
 
 @pytest.fixture(scope="module")
