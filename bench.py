@@ -236,6 +236,8 @@ def run_ours(args):
         return
 
     peak, peak_src = _peaks()
+    fp32_ffma, fp32_ffma2 = lib.mwa_grid_probe_fp32(plan.handle)   # register-only FMA loops, measured now
+    fp32_peak = max(fp32_ffma, fp32_ffma2)
     achieved = alg_bytes / (grid_ms * 1e-3) / 1e9
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": ws, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -253,31 +255,49 @@ def run_ours(args):
                      "traffic": None, "peak_source": peak_src, "kernel": {"gather": "gather_kernel", "chan": "chan_kernel", "atomic": "atomic_grid_kernel"}.get(ran, ran),
                      "algorithmic_bytes_per_launch": alg_bytes,
                      "whole_call_frac": alg_bytes / (ms_per_step * 1e-3) / 1e9 / peak,
-                     "fp32_time_ms_at_74.45_TFLOPs": cfg.tap_updates() * 4 / 74.45e12 * 1e3},
+                     "fp32_peak_tflops_measured": {"fma.rn.f32": fp32_ffma, "fma.rn.f32x2": fp32_ffma2},
+                     "fp32_time_ms_at_measured_peak": cfg.tap_updates() * 4 / (fp32_peak * 1e12) * 1e3,
+                     "hbm_time_ms_at_peak": alg_bytes / (peak * 1e9) * 1e3},
         "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
     }
-    tr = os.path.join(ROOT, "profiles", "traffic.json")     # dram bytes per launch from the committed ncu capture
+    tr = os.path.join(ROOT, "profiles", "traffic.csv")      # dram bytes per launch from the committed ncu captures
     if os.path.exists(tr):
+        import csv
         with open(tr) as f:
-            out["roofline"]["traffic"] = json.load(f).get(f"{cfg.name}:{out['roofline']['kernel']}")
+            for row in csv.DictReader(f):
+                if row["workload:kernel"] == f"{cfg.name}:{out['roofline']['kernel']}" and not args.n_chan:
+                    out["roofline"]["traffic"] = float(row["dram_bytes_per_launch"])
+                    out["roofline"]["traffic_source"] = row["source"]
 
     if ws == 1 and not args.no_cpu:
-        import oracle  # cpu_baseline leg
+        import oracle  # cpu_baseline leg: the oracle as it stands, on the box's cores, on a bounded channel sample
         cores = os.cpu_count() or 1
-        n_ch = min(cfg.n_chan, max(2 * cores, 16))
-        chans = sorted({int(round(k * (cfg.n_chan - 1) / max(n_ch - 1, 1))) for k in range(n_ch)})
-        uv, fr = g.uv.cpu(), g.freqs.cpu()[chans]
-        vis, w = g.vis[:, chans].cpu().contiguous(), g.weights[:, chans].cpu().contiguous()
-        t0 = time.perf_counter()
-        used = 0
-        for c0 in range(0, len(chans), cores):          # bounded memory: `cores` channel grids at a time
-            sl = slice(c0, c0 + cores)
-            _, _, th = oracle.grid(uv, fr[sl], vis[:, sl].contiguous(), w[:, sl].contiguous(), cfg.grid_n, g.cell_du,
-                                   cfg.support_W, cfg.oversample_O, g.kernel_table, want_abs=False, n_threads=cores)
-            used = max(used, th)
-        dt = time.perf_counter() - t0
+        uv = g.uv.cpu()
+
+        def run_channels(chans):
+            fr = g.freqs.cpu()[chans]
+            vis, w = g.vis[:, chans].cpu().contiguous(), g.weights[:, chans].cpu().contiguous()
+            t0 = time.perf_counter()
+            used = 0
+            for c0 in range(0, len(chans), cores):        # bounded memory: `cores` channel grids at a time
+                sl = slice(c0, c0 + cores)
+                _, _, th = oracle.grid(uv, fr[sl], vis[:, sl].contiguous(), w[:, sl].contiguous(), cfg.grid_n, g.cell_du,
+                                       cfg.support_W, cfg.oversample_O, g.kernel_table, want_abs=False, n_threads=cores)
+                used = max(used, th)
+            return time.perf_counter() - t0, used
+
+        def spaced(n):
+            return sorted({int(round(k * (cfg.n_chan - 1) / max(n - 1, 1))) for k in range(n)})
+
+        probe = spaced(min(cfg.n_chan, cores))
+        t_probe, _ = run_channels(probe)                  # calibration: how many channels make ~15 s of CPU work
+        n_ch = int(min(cfg.n_chan, max(len(probe), 15.0 / max(t_probe / len(probe), 1e-6))))
+        n_ch = max(cores, (n_ch // cores) * cores) if cfg.n_chan >= cores else cfg.n_chan
+        chans = spaced(min(n_ch, cfg.n_chan))
+        dt, used = run_channels(chans)
         out["cpu_baseline"] = {"value": cfg.n_vis * len(chans) * 4 / dt, "unit": UNIT, "cores": used, "kind": "oracle",
-                               "sample": f"{len(chans)} of {cfg.n_chan} channels of {cfg.name}, all rows, {dt:.1f} s",
+                               "sample": f"{len(chans)} of {cfg.n_chan} channels of {cfg.name} evenly spaced over the band, "
+                                         f"all {cfg.n_vis} rows, fp64, {dt:.1f} s of wall time on {used} threads",
                                "host_cpus": cores}
     print(json.dumps(out))
     if dist is not None:

@@ -96,6 +96,11 @@ int mwa_grid_plan_last_design(mwa_grid_plan* plan);
 int mwa_grid_plan_set_profiling(mwa_grid_plan* plan, int enabled);
 int mwa_grid_plan_stage_ms(mwa_grid_plan* plan, float* out_ms, int n);
 
+/* Measures the FP32 FMA throughput of the device with a register-only loop (the second term of the roofline of
+ * BASELINE.json north_star needs a measured denominator): out_tflops[0] = fma.rn.f32, out_tflops[1] = fma.rn.f32x2,
+ * both in TFLOP/s (2 flop per FMA).  HOST pointer to 2 doubles.  Synchronous; takes a few milliseconds. */
+int mwa_grid_probe_fp32(mwa_grid_plan* plan, double* out_tflops, void* stream);
+
 /* Number of kernel launches (memsets included) enqueued by the last gridding call on this plan. */
 int mwa_grid_plan_last_launches(const mwa_grid_plan* plan);
 

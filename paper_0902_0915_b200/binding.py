@@ -42,12 +42,14 @@ _lib.mwa_grid_plan_last_launches.argtypes = [_P]
 _lib.mwa_grid_plan_last_launches.restype = _I
 _lib.mwa_grid_plan_last_design.argtypes = [_P]
 _lib.mwa_grid_plan_last_design.restype = _I
+_lib.mwa_grid_probe_fp32.argtypes = [_P, _P, _P]
+_lib.mwa_grid_probe_fp32.restype = _I
 _lib.mwa_grid_last_error.argtypes = []
 _lib.mwa_grid_last_error.restype = ctypes.c_char_p
 
 EXPORTS = ["mwa_grid_plan_create", "mwa_grid_plan_destroy", "mwa_grid_visibilities", "mwa_grid_visibilities_host",
            "mwa_grid_compute_indices", "mwa_grid_plan_set_design", "mwa_grid_plan_set_profiling",
-           "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_plan_last_design", "mwa_grid_last_error"]
+           "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_plan_last_design", "mwa_grid_probe_fp32", "mwa_grid_last_error"]
 
 
 class MwaGridError(RuntimeError):
@@ -153,6 +155,13 @@ def mwa_grid_plan_last_design(plan) -> str:
     """Name of the design the last gridding call ran (resolves AUTO; synchronises)."""
     code = _check(_lib.mwa_grid_plan_last_design(plan))
     return {v: k for k, v in DESIGNS.items()}[code]
+
+
+def mwa_grid_probe_fp32(plan, stream=None):
+    """(TFLOP/s of fma.rn.f32, TFLOP/s of fma.rn.f32x2) measured with a register-only loop."""
+    buf = (ctypes.c_double * 2)()
+    _check(_lib.mwa_grid_probe_fp32(plan, ctypes.cast(buf, ctypes.c_void_p), _stream_ptr(stream)))
+    return float(buf[0]), float(buf[1])
 
 
 class Plan:

@@ -215,6 +215,12 @@ int mwa_grid_plan_stage_ms(mwa_grid_plan* plan, float* out_ms, int n) {
     return k;
 }
 
+int mwa_grid_probe_fp32(mwa_grid_plan* plan, double* out_tflops, void* stream) {
+    if (!plan || !out_tflops) { set_error("bad argument"); return MWA_GRID_ERR_INVALID; }
+    return probe_fp32(reinterpret_cast<Plan*>(plan), &out_tflops[0], &out_tflops[1], reinterpret_cast<cudaStream_t>(stream))
+               ? MWA_GRID_OK : MWA_GRID_ERR_CUDA;
+}
+
 int mwa_grid_plan_last_launches(const mwa_grid_plan* plan) {
     return plan ? reinterpret_cast<const Plan*>(plan)->last_launches : 0;
 }

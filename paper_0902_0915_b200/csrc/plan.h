@@ -62,6 +62,7 @@ bool launch_atomic(Plan* p, const double* uv, const float* vis, const float* w, 
 bool launch_binning(Plan* p, const double* uv, long long n_vis, int n_chan, cudaStream_t st);
 bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                    const int* dispatch, cudaStream_t st);
+bool probe_fp32(Plan* p, double* tflops_ffma, double* tflops_ffma2, cudaStream_t st);
 bool chan_supported(const Plan* p, int n_chan);
 bool launch_chan(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                  const int* dispatch, cudaStream_t st);
