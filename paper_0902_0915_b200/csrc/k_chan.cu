@@ -41,9 +41,9 @@ constexpr int kcThreads = kcWarps * 32;
 constexpr int kcLanes = 32;            // channels per group
 constexpr int kcSuper = 4;             // groups per super-group (one A1 sweep serves them all)
 constexpr int kcTileX = 16, kcTileY = 4;
-constexpr int kcListCap = 512;         // candidate hits kept per A1 sweep (row id + uv)
+constexpr int kcListCap = 640;         // candidate hits kept per A1 sweep chunk (row id + uv)
 constexpr int kcBatch = 64;            // hits per A2/B batch (w*V: 64 KB, geo: 8 KB)
-constexpr int kcGroupCap = 64;         // channel groups whose scale table is cached in shared memory (2048 channels)
+constexpr int kcGroupCap = 32;         // channel groups whose scale table is cached in shared memory (1024 channels)
 constexpr int kcPadU = 20;             // zero padding (floats) in front of a u table row
 constexpr int kcPadV = kcTileY;        // ... of a v table row
 constexpr int kcZeroFloats = 32;       // all-zero block behind each table (target of an invalid lane's geo)
@@ -96,11 +96,12 @@ struct ChanSmem {                 // fixed part; the table copies follow it in d
     float wts[kcBatch * kcLanes];                   // weights of the batch [hit][lane] (cp.async target)
     double2 hit_uv[kcListCap];                      // the list: uv (metres) and original row of each candidate hit
     int hit_row[kcListCap];
-    unsigned short sel[kcListCap];                  // list entries selected for the current group, in list order
+    unsigned short sel[kcSuper][kcListCap];         // per group of the super-group: the list entries that reach the tile, in list order
+    int sel_cnt[kcSuper];
     unsigned hit_mask[kcBatch];
     unsigned char vlist[kcWarps][kcBatch];          // per warp: the batch hits that touch its block, in order
     unsigned char lut_u[32], lut_v[32];             // block masks by stamp origin: [ou + W - 1] -> bx bits, [ov + W - 1] -> by bits (x16)
-    int warp_cnt[2][kcWarps];
+    int warp_cnt[2][kcSuper][kcWarps];
     int next_item, next_tile;
     double4 group[kcGroupCap];                      // copy of the per-group scale table (scale_kernel)
     double sc[kcSuper][kcLanes];                    // channel scales s_c of the current super-group
@@ -196,6 +197,7 @@ chan_kernel(const __grid_constant__ ChanParams P) {
         if (Y0 < N) {
             // per-group state (set in the group loop below, captured by reference)
             int c0 = 0, cc = 0, gslot = 0;
+            const unsigned short* sel = S.sel[0];                        // selection in use (group slot, or slot 0 after a dense sweep)
             bool cvalid = false;
             u64 acc[2][4][4];   // [row i][col j][pol] = (re, im) of the lane's channel
 
@@ -204,7 +206,7 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                 // (i) cp.async the warp's visibilities (32 lanes x 32 B = 1 KB per hit) and weights straight into
                 //     shared memory: every copy of the batch is in flight while (ii) does the fp64 index work
                 for (int hh = warp; hh < n; hh += kcWarps) {
-                    const size_t sidx = (size_t)S.hit_row[S.sel[b0 + hh]] * P.n_chan + cc;
+                    const size_t sidx = (size_t)S.hit_row[sel[b0 + hh]] * P.n_chan + cc;
                     const float4* src = P.vis + 2 * sidx;
                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(zs_s + 1024u * hh), "l"(src) : "memory");
                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(zs_s + 1024u * hh + 16u), "l"(src + 1) : "memory");
@@ -215,7 +217,7 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                 // (ii) exact indices -> geo, block mask
                 const double sc = S.sc[gslot][lane];
                 for (int hh = warp; hh < n; hh += kcWarps) {
-                    const double2 p = S.hit_uv[S.sel[b0 + hh]];
+                    const double2 p = S.hit_uv[sel[b0 + hh]];
                     SampleIndex s;
                     unsigned geo = zero_geo, mask = 0u;
                     if (sample_index(p.x, p.y, sc, P.g, s) && cvalid) {
@@ -323,25 +325,34 @@ chan_kernel(const __grid_constant__ ChanParams P) {
             };
 
             int par = 0;                                                   // parity of the warp_cnt buffer in use
-            // deterministic CTA-wide compaction step: returns the slot of this thread's hit (or -1) and adds the
-            // chunk's hit count to `count`; contains one __syncthreads
-            auto compact = [&](bool hit, int& count) -> int {
-                const unsigned ball = __ballot_sync(full, hit);
-                if (lane == 0) S.warp_cnt[par][warp] = __popc(ball);
-                __syncthreads();
-                const int cv = lane < kcWarps ? S.warp_cnt[par][lane] : 0;
-                int ci = cv;
+            // deterministic CTA-wide compaction step for up to kcSuper independent selections at once: slot[q] receives
+            // the slot of this thread's hit in selection q (or -1) and count[q] grows by the chunk's hits; ONE __syncthreads
+            auto compact = [&](const bool (&hit)[kcSuper], int nq, int (&count)[kcSuper], int (&slot)[kcSuper]) {
+                unsigned ball[kcSuper];
 #pragma unroll
-                for (int o = 1; o < kcWarps; o <<= 1) {
-                    const int t = __shfl_up_sync(full, ci, o);
-                    if (lane >= o) ci += t;
+                for (int q = 0; q < kcSuper; ++q) {
+                    ball[q] = q < nq ? __ballot_sync(full, hit[q]) : 0u;
+                    if (lane == 0 && q < nq) S.warp_cnt[par][q][warp] = __popc(ball[q]);
                 }
-                const int tot = __shfl_sync(full, ci, kcWarps - 1);
-                const int wbase = __shfl_sync(full, ci - cv, warp);
-                const int slot = hit ? count + wbase + __popc(ball & lt_mask) : -1;
-                count += tot;
+                __syncthreads();
+#pragma unroll
+                for (int q = 0; q < kcSuper; ++q) {
+                    slot[q] = -1;
+                    if (q < nq) {
+                        const int cv = lane < kcWarps ? S.warp_cnt[par][q][lane] : 0;
+                        int ci = cv;
+#pragma unroll
+                        for (int o = 1; o < kcWarps; o <<= 1) {
+                            const int t = __shfl_up_sync(full, ci, o);
+                            if (lane >= o) ci += t;
+                        }
+                        const int tot = __shfl_sync(full, ci, kcWarps - 1);
+                        const int wbase = __shfl_sync(full, ci - cv, warp);
+                        if (hit[q]) slot[q] = count[q] + wbase + __popc(ball[q] & lt_mask);
+                        count[q] += tot;
+                    }
+                }
                 par ^= 1;
-                return slot;
             };
             auto reaches_tile = [&](const double2 p, double s_lo, double s_hi) -> bool {
                 const double halfN = (double)(N / 2);
@@ -353,12 +364,10 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                        fmax(ya, yb) + P.reach >= cy0 && fmin(ya, yb) - P.reach <= cy1;
             };
 
-            // ---- A1: bucket sweep for scales in [s_lo, s_hi] (il, ih = s_ref / s_lo, s_ref / s_hi, NaN = scan all).
-            // flush = false: fill the list (entries beyond its capacity are counted but dropped -> overflow);
-            // flush = true : the list is pushed through A2 + B whenever it would overflow (one group only).
-            // Returns the number of entries in the list (or the overflowing count); n_seen totals all hits.
-            int n_seen = 0;
-            auto sweep = [&](double s_lo, double s_hi, double il, double ih, bool flush) -> int {
+            // ---- A1: bucket sweep for scales in [s_lo, s_hi] (il, ih = s_ref / s_lo, s_ref / s_hi, NaN = scan all buckets).
+            // Resumable: fills the list (identity selection in sel slot 0) from position (rg, base) of the scan until the
+            // next chunk of kcThreads candidates might not fit, and returns the number of entries; done = scan finished.
+            auto sweep = [&](double s_lo, double s_hi, double il, double ih, int& rg, int& base, bool& done) -> int {
                 int wx0 = 0, wx1 = P.nb - 1, wy0 = 0, wy1 = P.nb - 1;
                 if (il == il && ih == ih) {
                     const double halfN = (double)(N / 2);
@@ -372,8 +381,10 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                     wy0 = (int)fmin(fmax(floor((fmin(ay * il, ay * ih) + halfN) * ib), 0.0), top);
                     wy1 = (int)fmin(fmax(floor((fmax(byy * il, byy * ih) + halfN) * ib), 0.0), top);
                 }
-                int n_local = 0;
-                for (int rg = wy0; rg <= wy1; rg += 32) {
+                if (rg < 0) { rg = wy0; base = 0; }
+                int count[kcSuper] = {0, 0, 0, 0};
+                bool full_list = false;
+                for (; rg <= wy1 && !full_list; rg += 32, base = 0) {
                     int k0 = 0, len = 0;
                     if (rg + lane <= wy1) {
                         k0 = __ldg(P.bucket_start + (rg + lane) * P.nb + wx0);
@@ -387,14 +398,10 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                     }
                     const int total = __shfl_sync(full, incl, 31);
                     const int excl = incl - len;
-                    for (int base = 0; base < total; base += kcThreads) {
-                        if (flush && n_local + kcThreads > kcListCap) {       // uniform: n_local is the same in all threads
-                                    __syncthreads();
-                            process_sel(n_local);
-                            n_local = 0;
-                        }
+                    for (; base < total; base += kcThreads) {
+                        if (count[0] + kcThreads > kcListCap) { full_list = true; break; }   // uniform; resume here next time
                         const int f = base + tid;
-                        bool hit = false;
+                        bool hit[kcSuper] = {false, false, false, false};
                         double2 p = make_double2(0.0, 0.0);
                         int k = 0;
                         {
@@ -413,20 +420,21 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                             const double4 rec = P.row_sorted[k];
                             p = make_double2(rec.x, rec.y);
                             rowd = rec.z;
-                            hit = reaches_tile(p, s_lo, s_hi);
+                            hit[0] = reaches_tile(p, s_lo, s_hi);
                         }
-                        const int before = n_local;
-                        const int slot = compact(hit, n_local);
-                        n_seen += n_local - before;
-                        if (slot >= 0 && slot < kcListCap) {
-                            S.hit_uv[slot] = p;
-                            S.hit_row[slot] = (int)rowd;
-                            S.sel[slot] = (unsigned short)slot;
+                        int slot[kcSuper];
+                        compact(hit, 1, count, slot);
+                        if (slot[0] >= 0) {
+                            S.hit_uv[slot[0]] = p;
+                            S.hit_row[slot[0]] = (int)rowd;
+                            S.sel[0][slot[0]] = (unsigned short)slot[0];
                         }
                     }
+                    if (full_list) break;                                      // keep rg and base for the resume
                 }
+                done = !full_list;
                 __syncthreads();                                           // list complete and visible
-                return n_local;
+                return count[0];
             };
 
             // ---- a5: write the lane-channel tiles of the current group, once (zeros when nothing reached the tile)
@@ -475,50 +483,72 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                 }
             }
             TPH(10)
-            const int n_super = (g_end - g_begin > 1) ? sweep(u_lo, u_hi, u_il, u_ih, false) : kcListCap + 1;
-            TPH(7)
-            const bool per_group_sweep = n_super > kcListCap;              // too dense for the list (or a single group)
+            int rg = -1, base = 0;
+            bool done = false;
+            int n_super = 0;
+            if (g_end - g_begin > 1) n_super = sweep(u_lo, u_hi, u_il, u_ih, rg, base, done);
+            const bool dense = !done;                                      // list too small for the tile (or a single group)
             if (tid == 0 && next_item < P.n_items) next_tile = P.tile_order[(next_item / n_sg) >> 2];   // the atomic has landed by now
             have_next_tile = true;
 
-            // ... then group by group: select, A2 + B, write
+            // ... F: one pass over the list selects, for every group of the super-group, the entries that reach the tile
+            if (!dense) {
+                const int nq = g_end - g_begin;
+                int count[kcSuper] = {0, 0, 0, 0};
+                for (int b0 = 0; b0 < n_super; b0 += kcThreads) {
+                    const int i = b0 + tid;
+                    bool hit[kcSuper] = {false, false, false, false};
+                    if (i < n_super) {
+                        const double2 p = S.hit_uv[i];
+#pragma unroll
+                        for (int q = 0; q < kcSuper; ++q)
+                            if (q < nq) hit[q] = reaches_tile(p, group[g_begin + q].x, group[g_begin + q].y);
+                    }
+                    int slot[kcSuper];
+                    compact(hit, nq, count, slot);
+#pragma unroll
+                    for (int q = 0; q < kcSuper; ++q)
+                        if (slot[q] >= 0) S.sel[q][slot[q]] = (unsigned short)i;
+                }
+                if (tid == 0) {
+#pragma unroll
+                    for (int q = 0; q < kcSuper; ++q) S.sel_cnt[q] = count[q];
+                }
+                __syncthreads();
+            }
+
+            // ... then group by group: A2 + B over the selection (or, for a dense tile, over resumable sweeps), write
             for (int g = g_begin; g < g_end; ++g) {
                 c0 = g * kcLanes;
                 gslot = g - g_begin;
                 cvalid = c0 + lane < P.n_chan;
                 cc = cvalid ? c0 + lane : P.n_chan - 1;
+                sel = dense ? S.sel[0] : S.sel[gslot];
 #pragma unroll
                 for (int i = 0; i < 2; ++i)
 #pragma unroll
                     for (int j = 0; j < 4; ++j)
 #pragma unroll
                         for (int p = 0; p < 4; ++p) acc[i][j][p] = 0ull;
-                bool any;
-                if (per_group_sweep) {
-                    n_seen = 0;
-                    TPH(0)
-                    const double4 gi = group[g];
-                    const int n_left = sweep(gi.x, gi.y, gi.z, gi.w, true);
-                    TPH(6)
-                    process_sel(n_left);
-                    any = n_seen > 0;
-                } else {
-                    int n_sel = 0;
-                    const double g_lo = group[g].x, g_hi = group[g].y;
-                    for (int base = 0; base < n_super; base += kcThreads) {
-                        const int i = base + tid;
-                        const bool hit = i < n_super && reaches_tile(S.hit_uv[i], g_lo, g_hi);
-                        const int slot = compact(hit, n_sel);
-                        if (slot >= 0) S.sel[slot] = (unsigned short)i;
+                bool any = false, more = true;
+                rg = -1;
+                while (more) {
+                    int n;
+                    if (dense) {
+                        const double4 gi = group[g];
+                        bool fin = false;
+                        n = sweep(gi.x, gi.y, gi.z, gi.w, rg, base, fin);
+                        more = !fin;
+                    } else {
+                        n = S.sel_cnt[gslot];
+                        more = false;
                     }
-                    __syncthreads();
-                    TPH(6)
-                    process_sel(n_sel);
-                    any = n_sel > 0;
+                    if (n > 0) {
+                        process_sel(n);                                        // the only call site: A2 | sync | B | sync per batch
+                        any = true;
+                    }
                 }
-                TPH(0)
                 write_out(any);
-                TPH(5)
             }
         }   // Y0 < N
         TPH(8)
