@@ -57,7 +57,6 @@ struct ChanParams {
     const double4* group;       // [n_groups] s_lo, s_hi, s_ref / s_lo, s_ref / s_hi (scale_kernel)
     const int* bucket_start;    // [nb*nb + 1]
     const double4* row_sorted;  // [n_vis] (u, v, row id, 0) of the bucket-sorted rows
-    const int* tile_order;      // [nt*nt] 16x16 super-tiles, heaviest first
     int* counter;               // work counter
     const int* dispatch;        // device-side design choice (AUTO): run only if *dispatch == dispatch_want; null = always
     int dispatch_want;
@@ -102,7 +101,7 @@ struct ChanSmem {                 // fixed part; the table copies follow it in d
     unsigned char vlist[kcWarps][kcBatch];          // per warp: the batch hits that touch its block, in order
     unsigned char lut_u[32], lut_v[32];             // block masks by stamp origin: [ou + W - 1] -> bx bits, [ov + W - 1] -> by bits (x16)
     int warp_cnt[2][kcSuper][kcWarps];
-    int next_item, next_tile;
+    int next_item;
     double4 group[kcGroupCap];                      // copy of the per-group scale table (scale_kernel)
     double sc[kcSuper][kcLanes];                    // channel scales s_c of the current super-group
 };
@@ -156,11 +155,7 @@ chan_kernel(const __grid_constant__ ChanParams P) {
     for (int k = tid; k < min(P.n_groups, kcGroupCap); k += kcThreads) S.group[k] = P.group[k];
     const double4* group = P.n_groups <= kcGroupCap ? S.group : P.group;
     const int n_sg = (P.n_groups + kcSuper - 1) / kcSuper;
-    if (tid == 0) {
-        const int it = atomicAdd(P.counter, 1);
-        S.next_item = it;
-        S.next_tile = it < P.n_items ? P.tile_order[(it / n_sg) >> 2] : 0;
-    }
+    if (tid == 0) S.next_item = atomicAdd(P.counter, 1);
     __syncthreads();
 
     const int bx = warp & 3, by = warp >> 2;
@@ -184,12 +179,11 @@ chan_kernel(const __grid_constant__ ChanParams P) {
 
     int item = S.next_item;
     while (item < P.n_items) {
-        int next_item = 0, next_tile = 0;
-        bool have_next_tile = false;
+        int next_item = 0;
         if (tid == 0) next_item = atomicAdd(P.counter, 1);           // latency hidden behind this item
         const int sgi = item % n_sg;
         const int ts = item / n_sg;
-        const int tile = S.next_tile;
+        const int tile = ts >> 2;                                    // row-major over the 16x16 super-tiles: neighbours in time share visibility rows in L2
         if (warp < kcSuper)      // channel scales of the super-group; visible after the barriers of the sweep
             S.sc[warp][lane] = P.scale[min((sgi * kcSuper + warp) * kcLanes + lane, P.n_chan - 1)];
         const int ty = tile / P.nt, tx = tile - ty * P.nt;
@@ -488,8 +482,6 @@ chan_kernel(const __grid_constant__ ChanParams P) {
             int n_super = 0;
             if (g_end - g_begin > 1) n_super = sweep(u_lo, u_hi, u_il, u_ih, rg, base, done);
             const bool dense = !done;                                      // list too small for the tile (or a single group)
-            if (tid == 0 && next_item < P.n_items) next_tile = P.tile_order[(next_item / n_sg) >> 2];   // the atomic has landed by now
-            have_next_tile = true;
 
             // ... F: one pass over the list selects, for every group of the super-group, the entries that reach the tile
             if (!dense) {
@@ -552,9 +544,8 @@ chan_kernel(const __grid_constant__ ChanParams P) {
             }
         }   // Y0 < N
         TPH(8)
-        if (!have_next_tile && tid == 0 && next_item < P.n_items) next_tile = P.tile_order[(next_item / n_sg) >> 2];
         __syncthreads();
-        if (tid == 0) { S.next_item = next_item; S.next_tile = next_tile; }
+        if (tid == 0) S.next_item = next_item;
         __syncthreads();
         item = S.next_item;
         TPH(9)
@@ -597,7 +588,6 @@ bool launch_chan(Plan* p, const float* vis, const float* w, long long n_vis, int
     P.group = (const double4*)p->ws.d_group;
     P.bucket_start = p->ws.d_bucket_count;
     P.row_sorted = (const double4*)p->ws.d_row_sorted;
-    P.tile_order = p->ws.d_tile_order;
     P.counter = p->ws.d_misc + 1;
     P.dispatch = dispatch;
     P.dispatch_want = 1;
