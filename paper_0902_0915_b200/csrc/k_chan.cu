@@ -17,21 +17,22 @@
 //   A1 (thread = candidate row, once per super-group): walk the uv buckets (k_bin.cu) that can reach the tile
 //       at ANY scale of the 128 channels, keep the rows whose stamp can overlap the tile (conservative fp64
 //       interval test).  Then, per 32-channel group:
-//   F  (thread = list entry): the same interval test against the group's own scale range, from shared memory.
-//       Compaction is by ballot + prefix in both steps, so the hit order is a pure function of the sorted rows.
+//   F  (thread = list entry, once per super-group): the same test against each group's own scale range, from
+//       shared memory -> one selection per group.  Compaction is by ballot + prefix in both steps, so the hit
+//       order is a pure function of the sorted rows.
 //   A2 (warp = hit, lane = channel): cp.async of the hit's 32 visibilities (1 KB) and weights into shared
 //       memory; while they fly, the exact index function (index.cuh) per (row, channel) gives the lane a packed
-//       pair of kernel-table offsets ("geo") and the hit a bit mask of the blocks any lane touches; then w*V
-//       in place.
-//   B  (warp = block, lane = channel): for every hit that touches the block: 2 x LDS.128 of w*V, LDS.128 +
-//       LDS.64 of kernel taps from shifted zero-padded table copies, 8 FMUL, 32 FFMA2 (fma.rn.f32x2).
+//       pair of kernel-table offsets ("geo") and the hit a bit mask of the blocks any lane touches.
+//   B  (warp = block, lane = channel): for every hit that touches the block: 2 x LDS.128 of V, one LDS of w
+//       (folded into the two v taps), LDS.128 + LDS.64 of kernel taps from shifted zero-padded table copies,
+//       8 FMUL, 32 FFMA2 (fma.rn.f32x2); software-pipelined over two register sets.
 //   write-out: registers -> padded shared-memory stage (aliasing the w*V batch) -> full 128 B lines of one
 //       (channel, pol, row) with streaming stores; every cell of grid_out is written exactly once, zeros
 //       included (R10).
 //
-// No atomics on grid data, no fp64 and no global loads in phase B.  A tile too dense for the list falls back
-// to one A1 sweep per group with flushes.  Two co-resident CTAs hide each other's barriers and load latency.
-#include <cstdio>
+// No atomics on grid data, no fp64 and no global loads in phase B.  A tile too dense for the list is served by
+// resumable A1 sweeps per group.  Two co-resident CTAs hide part of each other's barriers and load latency.
+// Tiles are walked row-major (neighbouring tiles share visibility rows in L2), super-groups fastest.
 #include "plan.h"
 
 namespace mwa {
@@ -170,12 +171,6 @@ chan_kernel(const __grid_constant__ ChanParams P) {
     const unsigned lt_mask = (1u << lane) - 1u;
     const unsigned full = 0xffffffffu;
 
-#ifdef MWA_CHAN_TIMING
-    long long tph[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, tlast = clock64();
-#define TPH(k) { const long long tn = clock64(); tph[k] += tn - tlast; tlast = tn; }
-#else
-#define TPH(k)
-#endif
 
     int item = S.next_item;
     while (item < P.n_items) {
@@ -306,15 +301,10 @@ chan_kernel(const __grid_constant__ ChanParams P) {
             auto process_sel = [&](int n) {
                 for (int b0 = 0; b0 < n; b0 += kcBatch) {
                     const int nbat = min(kcBatch, n - b0);
-                    TPH(0)
                     phase_a2(b0, nbat);
-                    TPH(1)
                     __syncthreads();
-                    TPH(2)
                     phase_b(nbat);
-                    TPH(3)
                     __syncthreads();
-                    TPH(4)
                 }
             };
 
@@ -476,7 +466,6 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                     u_ih = (gi.w == gi.w && u_ih == u_ih) ? fmin(u_ih, gi.w) : gi.w + u_ih;
                 }
             }
-            TPH(10)
             int rg = -1, base = 0;
             bool done = false;
             int n_super = 0;
@@ -543,18 +532,11 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                 write_out(any);
             }
         }   // Y0 < N
-        TPH(8)
         __syncthreads();
         if (tid == 0) S.next_item = next_item;
         __syncthreads();
         item = S.next_item;
-        TPH(9)
     }
-#ifdef MWA_CHAN_TIMING
-    if (lane == 0 && (warp == 0 || warp == 5) && (blockIdx.x % 37) == 0)
-        printf("cta %d warp %d: gaps %lld tail %lld itemsync %lld decode %lld |  sweep %lld | filter %lld | A2 %lld | bar %lld | B %lld | bar %lld | write %lld\n", blockIdx.x, warp,
-               tph[0], tph[8], tph[9], tph[10], tph[7], tph[6], tph[1], tph[2], tph[3], tph[4], tph[5]);
-#endif
 }
 
 // Geometry of the padded table copies (see the kernel header).
