@@ -55,6 +55,7 @@ static int ensure_workspace(Plan* p, long long n_vis, int n_chan) {
     }
     if (n_vis > ws.cap_vis) {
         if (!ensure(ws.d_perm, (size_t)n_vis, "perm")) return MWA_GRID_ERR_NOMEM;
+        if (!ensure(ws.d_perm_tmp, (size_t)n_vis, "perm_tmp")) return MWA_GRID_ERR_NOMEM;
         if (!ensure(ws.d_uv_sorted, (size_t)n_vis, "uv_sorted")) return MWA_GRID_ERR_NOMEM;
         if (!ensure(ws.d_row_sorted, (size_t)n_vis * 4, "row_sorted")) return MWA_GRID_ERR_NOMEM;
         ws.cap_vis = n_vis;
@@ -176,7 +177,7 @@ void mwa_grid_plan_destroy(mwa_grid_plan* plan) {
     if (!plan) return;
     Plan* p = reinterpret_cast<Plan*>(plan);
     Workspace& ws = p->ws;
-    void* ptrs[] = {p->d_table, ws.d_scale, ws.d_group, ws.d_scale_ref, ws.d_bucket_count, ws.d_bucket_cursor, ws.d_perm,
+    void* ptrs[] = {p->d_table, ws.d_scale, ws.d_group, ws.d_scale_ref, ws.d_bucket_count, ws.d_bucket_cursor, ws.d_perm, ws.d_perm_tmp,
                     ws.d_uv_sorted, ws.d_row_sorted, ws.d_tile_order, ws.d_tile_weight, ws.d_misc, ws.d_dispatch, ws.d_stage};
     for (void* q : ptrs)
         if (q) cudaFree(q);

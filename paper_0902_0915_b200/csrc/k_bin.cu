@@ -73,17 +73,36 @@ __global__ void bin_scan_kernel(int* __restrict__ count, int n, int* __restrict_
 }
 
 __global__ void bin_scatter_kernel(GridGeom g, const double2* __restrict__ uv, const double* __restrict__ s_ref_p,
-                                   int n_vis, int nb, int* __restrict__ cursor, int* __restrict__ perm,
-                                   double2* __restrict__ uv_sorted, double4* __restrict__ row_sorted) {
+                                   int n_vis, int nb, int* __restrict__ cursor, int* __restrict__ perm_tmp) {
     const double s_ref = *s_ref_p;
     for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < n_vis; n += gridDim.x * blockDim.x) {
         const double2 p = uv[n];
         const int bx = bucket_coord(p.x, s_ref, g.inv_du, g.N, nb);
         const int by = bucket_coord(p.y, s_ref, g.inv_du, g.N, nb);
-        const int pos = atomicAdd(&cursor[by * nb + bx], 1);
-        perm[pos] = n;
-        uv_sorted[pos] = p;
-        row_sorted[pos] = make_double4(p.x, p.y, (double)n, 0.0);      // K5: uv and row id in one 32 B record
+        perm_tmp[atomicAdd(&cursor[by * nb + bx], 1)] = n;            // order inside a bucket: whatever the atomics gave
+    }
+}
+
+// One warp per bucket puts the bucket's rows in ascending row order (rank = number of smaller row ids; buckets hold
+// ~8 rows on average, a few hundred in the core) and writes the sorted copies.  With this the bucket-sorted order is a
+// pure function of the input, so K3c and K5 - which add the taps of a cell in list order, with no atomics - give
+// bit-identical grids from run to run.
+__global__ void bin_order_kernel(const double2* __restrict__ uv, const int* __restrict__ bucket_start, int n_buckets,
+                                 const int* __restrict__ perm_tmp, int* __restrict__ perm,
+                                 double2* __restrict__ uv_sorted, double4* __restrict__ row_sorted) {
+    const int lane = threadIdx.x & 31;
+    const int warps = (gridDim.x * blockDim.x) >> 5;
+    for (int b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; b < n_buckets; b += warps) {
+        const int k0 = bucket_start[b], k1 = bucket_start[b + 1];
+        for (int i = k0 + lane; i < k1; i += 32) {
+            const int row = perm_tmp[i];
+            int rank = 0;
+            for (int j = k0; j < k1; ++j) rank += perm_tmp[j] < row;
+            const double2 p = uv[row];
+            perm[k0 + rank] = row;
+            uv_sorted[k0 + rank] = p;
+            row_sorted[k0 + rank] = make_double4(p.x, p.y, (double)row, 0.0);      // K5: uv and row id in one 32 B record
+        }
     }
 }
 
@@ -144,14 +163,20 @@ bool launch_binning(Plan* p, const double* uv, long long n_vis, int /*n_chan*/, 
                                              ws.d_bucket_count);
     bin_scan_kernel<<<1, 1024, 0, st>>>(ws.d_bucket_count, n_buckets, ws.d_bucket_cursor);
     bin_scatter_kernel<<<blocks, 256, 0, st>>>(p->geom, (const double2*)uv, ws.d_scale_ref, (int)n_vis, nb,
-                                               ws.d_bucket_cursor, ws.d_perm, ws.d_uv_sorted, (double4*)ws.d_row_sorted);
+                                               ws.d_bucket_cursor, ws.d_perm_tmp);
+    {
+        long long oblocks = ((long long)n_buckets * 32 + 255) / 256;
+        if (oblocks > p->sm_count * 16) oblocks = p->sm_count * 16;
+        bin_order_kernel<<<(unsigned)oblocks, 256, 0, st>>>((const double2*)uv, ws.d_bucket_count, n_buckets, ws.d_perm_tmp, ws.d_perm,
+                                                            ws.d_uv_sorted, (double4*)ws.d_row_sorted);
+    }
     int* hist = ws.d_misc + 16;
     int tblocks = (nt * nt + 255) / 256;
     if (tblocks > p->sm_count * 8) tblocks = p->sm_count * 8;
     tile_weight_kernel<<<tblocks, 256, 0, st>>>(ws.d_bucket_count, nb, nt, ws.d_tile_weight, hist);
     tile_order_scan_kernel<<<1, kWeightBins, 0, st>>>(hist);
     tile_order_scatter_kernel<<<tblocks, 256, 0, st>>>(ws.d_tile_weight, nt * nt, hist, ws.d_tile_order);
-    p->last_launches += 8;
+    p->last_launches += 9;
     return cuda_ok(cudaGetLastError(), "binning kernels");
 }
 

@@ -21,7 +21,8 @@ struct Workspace {
     int* d_bucket_count = nullptr;   // [nb*nb + 1] histogram, then exclusive scan = bucket_start
     int* d_bucket_cursor = nullptr;  // [nb*nb] scatter cursors
     int cap_buckets = 0;
-    int* d_perm = nullptr;           // [n_vis] row ids sorted by bucket
+    int* d_perm = nullptr;           // [n_vis] row ids sorted by bucket, ascending inside a bucket
+    int* d_perm_tmp = nullptr;       // [n_vis] scatter target before the in-bucket ordering
     double2* d_uv_sorted = nullptr;  // [n_vis] uv of the sorted rows
     double* d_row_sorted = nullptr;  // [n_vis][4] (u, v, row id, 0) of the sorted rows: one 32 B record per row (K5)
     long long cap_vis = 0;
