@@ -452,6 +452,9 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                         dst += 2 * 4 * plane * 2;
                     }
                 }
+                // the stage aliases the visibility batch: nobody may start the next group's cp.async (A2) while a slower
+                // warp is still copying this group's stage out
+                if (any) __syncthreads();
             };
 
             // ---- the super-group: one sweep over the union of its groups' scale ranges ...

@@ -161,6 +161,20 @@ def test_run_to_run_bit_identical(lib, design):
         assert torch.equal(outs[0].view(torch.float32), o.view(torch.float32))
 
 
+def test_dense_tile_many_calls_on_one_plan(lib):
+    # regression: the write-out stage of K5 aliases the visibility batch; without a barrier after the copy-out a
+    # fast warp's cp.async for the next group could overwrite a slower warp's stage (seen once in ~10 calls)
+    cfg = scaled(CONFIGS["C4"], n_ant=200, core_ant=100, n_chan=33, grid_n=250)
+    cfg = scaled(cfg, f_lo_hz=155e6, f_hi_hz=155e6 + 40e3 * (cfg.n_chan - 1))
+    g = generate(cfg)
+    G, A, _ = _oracle(g)
+    _to_dev(g)
+    with _plan(lib, g, "auto") as p:
+        for k in range(12):
+            out = p.grid(g.uv, g.freqs, g.vis, g.weights if k % 3 == 0 else None)
+            assert_parity(out.cpu().numpy(), G, A, f"dense tile, call {k}")
+
+
 def test_chan_wide_kernel_repeated_calls(lib):
     # W = 15, O = 16 through K5; a second call on the same plan must pass parity too (workspace reuse)
     cfg = scaled(CONFIGS["C5"], n_ant=24, core_ant=12, n_chan=40, grid_n=512, f_lo_hz=150e6, f_hi_hz=150e6 + 39 * 40e3)
