@@ -4,7 +4,7 @@
 // at almost the same (u, v) (u_lambda = u_m * nu / c moves by 2.6e-4 of its radius per channel), and every
 // channel owns its own grid (BASELINE.json configs[3]).  K5 turns that into SIMD lanes:
 //
-//   CTA  = one 16 x 4 cell tile x one SUPER-GROUP of 4 x 32 adjacent channels; 8 warps, 2 CTAs per SM
+//   CTA  = one 16 x 4 cell tile x one SUPER-GROUP of 6 x 32 adjacent channels; 8 warps, 2 CTAs per SM
 //   warp = one 4x2-cell block of the tile
 //   lane = one channel of the current 32-channel group; the lane keeps 8 cells x 4 pol x (re, im) = 64 fp32
 //          accumulators of ITS channel's grid in registers.
@@ -15,7 +15,7 @@
 // zeros from the padded kernel table, so there is no divergence in the FMA body at all.
 //
 //   A1 (thread = candidate row, once per super-group): walk the uv buckets (k_bin.cu) that can reach the tile
-//       at ANY scale of the 128 channels, keep the rows whose stamp can overlap the tile (conservative fp64
+//       at ANY scale of the 192 channels, keep the rows whose stamp can overlap the tile (conservative fp64
 //       interval test).  Then, per 32-channel group:
 //   F  (thread = list entry, once per super-group): the same test against each group's own scale range, from
 //       shared memory -> one selection per group.  Compaction is by ballot + prefix in both steps, so the hit
@@ -40,7 +40,7 @@ namespace mwa {
 constexpr int kcWarps = 8;
 constexpr int kcThreads = kcWarps * 32;
 constexpr int kcLanes = 32;            // channels per group
-constexpr int kcSuper = 4;             // groups per super-group (one A1 sweep serves them all)
+constexpr int kcSuper = 6;             // groups per super-group (one A1 sweep serves them all)
 constexpr int kcTileX = 16, kcTileY = 4;
 constexpr int kcListCap = 640;         // candidate hits kept per A1 sweep chunk (row id + uv)
 constexpr int kcBatch = 64;            // hits per A2/B batch (w*V: 64 KB, geo: 8 KB)
@@ -205,6 +205,7 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                 asm volatile("cp.async.commit_group;" ::: "memory");
                 // (ii) exact indices -> geo, block mask
                 const double sc = S.sc[gslot][lane];
+#pragma unroll 2
                 for (int hh = warp; hh < n; hh += kcWarps) {
                     const double2 p = S.hit_uv[sel[b0 + hh]];
                     SampleIndex s;
@@ -366,7 +367,7 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                     wy1 = (int)fmin(fmax(floor((fmax(byy * il, byy * ih) + halfN) * ib), 0.0), top);
                 }
                 if (rg < 0) { rg = wy0; base = 0; }
-                int count[kcSuper] = {0, 0, 0, 0};
+                int count[kcSuper] = {};
                 bool full_list = false;
                 for (; rg <= wy1 && !full_list; rg += 32, base = 0) {
                     int k0 = 0, len = 0;
@@ -385,7 +386,7 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                     for (; base < total; base += kcThreads) {
                         if (count[0] + kcThreads > kcListCap) { full_list = true; break; }   // uniform; resume here next time
                         const int f = base + tid;
-                        bool hit[kcSuper] = {false, false, false, false};
+                        bool hit[kcSuper] = {};
                         double2 p = make_double2(0.0, 0.0);
                         int k = 0;
                         {
@@ -478,10 +479,10 @@ chan_kernel(const __grid_constant__ ChanParams P) {
             // ... F: one pass over the list selects, for every group of the super-group, the entries that reach the tile
             if (!dense) {
                 const int nq = g_end - g_begin;
-                int count[kcSuper] = {0, 0, 0, 0};
+                int count[kcSuper] = {};
                 for (int b0 = 0; b0 < n_super; b0 += kcThreads) {
                     const int i = b0 + tid;
-                    bool hit[kcSuper] = {false, false, false, false};
+                    bool hit[kcSuper] = {};
                     if (i < n_super) {
                         const double2 p = S.hit_uv[i];
 #pragma unroll
