@@ -40,7 +40,9 @@ enum {
     MWA_GRID_DESIGN_SMEM = 2,   /* K3a: tile-owned shared-memory accumulation (red.shared.add.f32)          */
     MWA_GRID_DESIGN_ROMEIN = 3, /* K3b: threads own cells modulo W, register-resident, flush on cell change */
     MWA_GRID_DESIGN_GATHER = 4, /* K3c: tile-owned, lane = 4x2 cell block of one channel, registers              */
-    MWA_GRID_DESIGN_CHAN = 5    /* K5: tile-owned, lane = channel (32 adjacent channels per warp), registers     */
+    MWA_GRID_DESIGN_CHAN = 5,   /* K5: tile-owned, lane = channel (32 adjacent channels per warp), registers     */
+    MWA_GRID_DESIGN_CHANWS = 6  /* K6: K5's ownership as a warp-specialised producer / consumer pipeline: exact-index
+                                   pre-pass, TMA bulk loads, mbarrier hand-off, tensor-map TMA stores (k_chanws.cu) */
 };
 
 /* Create a plan (R5-R8 for the table).
@@ -100,6 +102,12 @@ int mwa_grid_plan_stage_ms(mwa_grid_plan* plan, float* out_ms, int n);
  * BASELINE.json north_star needs a measured denominator): out_tflops[0] = fma.rn.f32, out_tflops[1] = fma.rn.f32x2,
  * both in TFLOP/s (2 flop per FMA).  HOST pointer to 2 doubles.  Synchronous; takes a few milliseconds. */
 int mwa_grid_probe_fp32(mwa_grid_plan* plan, double* out_tflops, void* stream);
+
+/* Test / diagnostics query (synchronises with the device): counters the last K6 gridding call left behind, written
+ * into HOST array `out` (up to 8 values): [0] pipeline error code (0 = none; non-zero means a bounded wait inside the
+ * kernel expired and the grid is incomplete), [1] work items, [2] items at least one sample reaches, [3] staged batches
+ * of up to 32 hits, [4] largest number of hits of one item.  Returns the number of values written. */
+int mwa_grid_plan_last_stats(mwa_grid_plan* plan, long long* out, int n);
 
 /* Number of kernel launches (memsets included) enqueued by the last gridding call on this plan. */
 int mwa_grid_plan_last_launches(const mwa_grid_plan* plan);

@@ -11,9 +11,9 @@ import torch
 
 from . import _build
 
-DESIGN_AUTO, DESIGN_ATOMIC, DESIGN_SMEM, DESIGN_ROMEIN, DESIGN_GATHER, DESIGN_CHAN = 0, 1, 2, 3, 4, 5
+DESIGN_AUTO, DESIGN_ATOMIC, DESIGN_SMEM, DESIGN_ROMEIN, DESIGN_GATHER, DESIGN_CHAN, DESIGN_CHANWS = 0, 1, 2, 3, 4, 5, 6
 DESIGNS = {"auto": DESIGN_AUTO, "atomic": DESIGN_ATOMIC, "smem": DESIGN_SMEM, "romein": DESIGN_ROMEIN,
-           "gather": DESIGN_GATHER, "chan": DESIGN_CHAN}
+           "gather": DESIGN_GATHER, "chan": DESIGN_CHAN, "chanws": DESIGN_CHANWS}
 
 if not os.path.exists(_build.LIB):
     raise ImportError(f"{_build.LIB} is missing: the CUDA library has not been built "
@@ -42,6 +42,8 @@ _lib.mwa_grid_plan_last_launches.argtypes = [_P]
 _lib.mwa_grid_plan_last_launches.restype = _I
 _lib.mwa_grid_plan_last_design.argtypes = [_P]
 _lib.mwa_grid_plan_last_design.restype = _I
+_lib.mwa_grid_plan_last_stats.argtypes = [_P, _P, _I]
+_lib.mwa_grid_plan_last_stats.restype = _I
 _lib.mwa_grid_probe_fp32.argtypes = [_P, _P, _P]
 _lib.mwa_grid_probe_fp32.restype = _I
 _lib.mwa_grid_last_error.argtypes = []
@@ -49,7 +51,7 @@ _lib.mwa_grid_last_error.restype = ctypes.c_char_p
 
 EXPORTS = ["mwa_grid_plan_create", "mwa_grid_plan_destroy", "mwa_grid_visibilities", "mwa_grid_visibilities_host",
            "mwa_grid_compute_indices", "mwa_grid_plan_set_design", "mwa_grid_plan_set_profiling",
-           "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_plan_last_design", "mwa_grid_probe_fp32", "mwa_grid_last_error"]
+           "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_plan_last_design", "mwa_grid_plan_last_stats", "mwa_grid_probe_fp32", "mwa_grid_last_error"]
 
 
 class MwaGridError(RuntimeError):
@@ -155,6 +157,14 @@ def mwa_grid_plan_last_design(plan) -> str:
     """Name of the design the last gridding call ran (resolves AUTO; synchronises)."""
     code = _check(_lib.mwa_grid_plan_last_design(plan))
     return {v: k for k, v in DESIGNS.items()}[code]
+
+
+def mwa_grid_plan_last_stats(plan):
+    """Counters of the last K6 call: dict(error, items, items_with_hits, batches, max_hits).  Synchronises."""
+    buf = (ctypes.c_longlong * 8)()
+    _check(_lib.mwa_grid_plan_last_stats(plan, ctypes.cast(buf, ctypes.c_void_p), 8))
+    return {"error": int(buf[0]), "items": int(buf[1]), "items_with_hits": int(buf[2]), "batches": int(buf[3]),
+            "max_hits": int(buf[4])}
 
 
 def mwa_grid_probe_fp32(plan, stream=None):

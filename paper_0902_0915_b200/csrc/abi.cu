@@ -21,25 +21,31 @@ bool cuda_ok(cudaError_t e, const char* what) {
     return false;
 }
 
+// Grows one workspace array: the new buffer is allocated first and swapped in on success, so a failed call leaves the
+// old (smaller) buffer and its capacity valid.
 template <typename T>
 static bool ensure(T*& ptr, size_t count, const char* what) {
-    if (ptr) cudaFree(ptr);
-    ptr = nullptr;
-    if (count == 0) return true;
-    cudaError_t e = cudaMalloc((void**)&ptr, count * sizeof(T));
-    if (e != cudaSuccess) {
-        cudaGetLastError();
-        set_error(std::string("workspace allocation failed (") + what + "): " + cudaGetErrorString(e));
-        ptr = nullptr;
-        return false;
+    T* fresh = nullptr;
+    if (count > 0) {
+        cudaError_t e = cudaMalloc((void**)&fresh, count * sizeof(T));
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            set_error(std::string("workspace allocation failed (") + what + "): " + cudaGetErrorString(e));
+            return false;
+        }
     }
+    if (ptr) cudaFree(ptr);
+    ptr = fresh;
     return true;
 }
 
 // returns 0 / MWA_GRID_ERR_NOMEM
 static int ensure_workspace(Plan* p, long long n_vis, int n_chan) {
     Workspace& ws = p->ws;
+    // every capacity is dropped before its arrays are regrown and restored only when all of them succeeded, so a
+    // call after a failed one reallocates instead of running on a partly grown workspace
     if (n_chan > ws.cap_chan) {
+        ws.cap_chan = 0;
         if (!ensure(ws.d_scale, (size_t)n_chan, "scale")) return MWA_GRID_ERR_NOMEM;
         if (!ensure(ws.d_group, (size_t)((n_chan + 31) / 32) * 4, "group")) return MWA_GRID_ERR_NOMEM;
         ws.cap_chan = n_chan;
@@ -49,11 +55,13 @@ static int ensure_workspace(Plan* p, long long n_vis, int n_chan) {
     const int nb = (p->geom.N + kBucketCells - 1) / kBucketCells;
     const int n_buckets = nb * nb;
     if (n_buckets > ws.cap_buckets) {
+        ws.cap_buckets = 0;
         if (!ensure(ws.d_bucket_count, (size_t)n_buckets + 1, "bucket_count")) return MWA_GRID_ERR_NOMEM;
         if (!ensure(ws.d_bucket_cursor, (size_t)n_buckets, "bucket_cursor")) return MWA_GRID_ERR_NOMEM;
         ws.cap_buckets = n_buckets;
     }
     if (n_vis > ws.cap_vis) {
+        ws.cap_vis = 0;
         if (!ensure(ws.d_perm, (size_t)n_vis, "perm")) return MWA_GRID_ERR_NOMEM;
         if (!ensure(ws.d_perm_tmp, (size_t)n_vis, "perm_tmp")) return MWA_GRID_ERR_NOMEM;
         if (!ensure(ws.d_uv_sorted, (size_t)n_vis, "uv_sorted")) return MWA_GRID_ERR_NOMEM;
@@ -63,11 +71,22 @@ static int ensure_workspace(Plan* p, long long n_vis, int n_chan) {
     const int nt = (p->geom.N + kTile - 1) / kTile;
     const int n_tiles = nt * nt;
     if (n_tiles > ws.cap_tiles) {
+        ws.cap_tiles = 0;
         if (!ensure(ws.d_tile_order, (size_t)n_tiles, "tile_order")) return MWA_GRID_ERR_NOMEM;
         if (!ensure(ws.d_tile_weight, (size_t)n_tiles, "tile_weight")) return MWA_GRID_ERR_NOMEM;
         ws.cap_tiles = n_tiles;
     }
     if (!ws.d_misc && !ensure(ws.d_misc, 4096 + 16, "misc")) return MWA_GRID_ERR_NOMEM;
+    const bool want_ws = (p->design == MWA_GRID_DESIGN_CHANWS || p->design == MWA_GRID_DESIGN_AUTO) && chanws_supported(p, n_chan);
+    const size_t n_pre = want_ws ? (size_t)n_vis * (size_t)((n_chan + 31) / 32) * 32 : 0;
+    if (n_pre > ws.cap_pre) {
+        ws.cap_pre = 0;
+        if (!ensure(ws.d_pre, n_pre, "packed indices")) return MWA_GRID_ERR_NOMEM;
+        unsigned long long* bb = (unsigned long long*)ws.d_bb;
+        if (!ensure(bb, n_pre / 32, "bounding boxes")) { ws.d_bb = bb; return MWA_GRID_ERR_NOMEM; }
+        ws.d_bb = bb;
+        ws.cap_pre = n_pre;
+    }
     return MWA_GRID_OK;
 }
 
@@ -89,6 +108,13 @@ static int grid_device(Plan* p, const double* uv, const double* freqs, const flo
                        long long n_vis, int n_chan, float* grid, cudaStream_t st) {
     p->last_launches = 0;
     if (n_chan == 0) return MWA_GRID_OK;
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev), "cudaGetDevice")) return MWA_GRID_ERR_CUDA;
+    if (dev != p->device) {                       // the workspace and the kernel attributes live on the plan's device
+        set_error("the current CUDA device (" + std::to_string(dev) + ") is not the device the plan was created on (" +
+                  std::to_string(p->device) + ")");
+        return MWA_GRID_ERR_INVALID;
+    }
     int rc = ensure_workspace(p, n_vis, n_chan);
     if (rc != MWA_GRID_OK) return rc;
     const bool prof = p->profiling;
@@ -113,11 +139,14 @@ static int grid_device(Plan* p, const double* uv, const double* freqs, const flo
             case MWA_GRID_DESIGN_ROMEIN: ok = launch_romein(p, uv, vis, weights, n_vis, n_chan, grid, st); break;
             case MWA_GRID_DESIGN_GATHER: ok = launch_gather(p, vis, weights, n_vis, n_chan, grid, nullptr, st); break;
             case MWA_GRID_DESIGN_CHAN: ok = launch_chan(p, vis, weights, n_vis, n_chan, grid, nullptr, st); break;
+            case MWA_GRID_DESIGN_CHANWS: ok = launch_chanws(p, vis, weights, n_vis, n_chan, grid, nullptr, st); break;
             case MWA_GRID_DESIGN_AUTO:
                 // the choice is made on the device by scale_kernel (the host never reads freqs): both kernels
                 // are enqueued and the one that was not picked returns at once
                 ok = true;
-                if (chan_supported(p, n_chan)) ok = launch_chan(p, vis, weights, n_vis, n_chan, grid, p->ws.d_dispatch, st);
+                p->last_chanws = chanws_supported(p, n_chan);
+                if (p->last_chanws) ok = launch_chanws(p, vis, weights, n_vis, n_chan, grid, p->ws.d_dispatch, st);
+                else if (chan_supported(p, n_chan)) ok = launch_chan(p, vis, weights, n_vis, n_chan, grid, p->ws.d_dispatch, st);
                 ok = ok && launch_gather(p, vis, weights, n_vis, n_chan, grid, p->ws.d_dispatch, st);
                 break;
             default: set_error("unknown design"); return MWA_GRID_ERR_INVALID;
@@ -178,7 +207,8 @@ void mwa_grid_plan_destroy(mwa_grid_plan* plan) {
     Plan* p = reinterpret_cast<Plan*>(plan);
     Workspace& ws = p->ws;
     void* ptrs[] = {p->d_table, ws.d_scale, ws.d_group, ws.d_scale_ref, ws.d_bucket_count, ws.d_bucket_cursor, ws.d_perm, ws.d_perm_tmp,
-                    ws.d_uv_sorted, ws.d_row_sorted, ws.d_tile_order, ws.d_tile_weight, ws.d_misc, ws.d_dispatch, ws.d_stage};
+                    ws.d_uv_sorted, ws.d_row_sorted, ws.d_tile_order, ws.d_tile_weight, ws.d_misc, ws.d_dispatch, ws.d_stage,
+                    ws.d_pre, ws.d_bb};
     for (void* q : ptrs)
         if (q) cudaFree(q);
     for (auto& e : p->ev)
@@ -189,7 +219,7 @@ void mwa_grid_plan_destroy(mwa_grid_plan* plan) {
 
 int mwa_grid_plan_set_design(mwa_grid_plan* plan, int design) {
     if (!plan) { set_error("plan is NULL"); return MWA_GRID_ERR_INVALID; }
-    if (design < MWA_GRID_DESIGN_AUTO || design > MWA_GRID_DESIGN_CHAN) { set_error("unknown design"); return MWA_GRID_ERR_INVALID; }
+    if (design < MWA_GRID_DESIGN_AUTO || design > MWA_GRID_DESIGN_CHANWS) { set_error("unknown design"); return MWA_GRID_ERR_INVALID; }
     reinterpret_cast<Plan*>(plan)->design = design;
     return MWA_GRID_OK;
 }
@@ -233,7 +263,19 @@ int mwa_grid_plan_last_design(mwa_grid_plan* plan) {
     if (!p->ws.d_dispatch) { set_error("no gridding call recorded"); return MWA_GRID_ERR_INVALID; }
     int v = 0;
     if (!cuda_ok(cudaMemcpy(&v, p->ws.d_dispatch, sizeof(int), cudaMemcpyDeviceToHost), "read dispatch")) return MWA_GRID_ERR_CUDA;
-    return v == 1 ? MWA_GRID_DESIGN_CHAN : MWA_GRID_DESIGN_GATHER;
+    if (v != 1) return MWA_GRID_DESIGN_GATHER;
+    return p->last_chanws ? MWA_GRID_DESIGN_CHANWS : MWA_GRID_DESIGN_CHAN;
+}
+
+int mwa_grid_plan_last_stats(mwa_grid_plan* plan, long long* out, int n) {
+    if (!plan || !out || n < 0) { set_error("bad argument"); return MWA_GRID_ERR_INVALID; }
+    Plan* p = reinterpret_cast<Plan*>(plan);
+    if (!p->ws.d_misc) { set_error("no gridding call recorded"); return MWA_GRID_ERR_INVALID; }
+    int v[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    if (!cuda_ok(cudaMemcpy(v, p->ws.d_misc + 4, sizeof(v), cudaMemcpyDeviceToHost), "read stats")) return MWA_GRID_ERR_CUDA;
+    const int k = n < 8 ? n : 8;
+    for (int i = 0; i < k; ++i) out[i] = v[i];
+    return k;
 }
 
 int mwa_grid_compute_indices(mwa_grid_plan* plan, const double* uv_f64, const double* freqs, long long n_vis,

@@ -68,7 +68,7 @@ __global__ void scale_kernel(const double* __restrict__ freqs, int n_chan, int h
 }
 
 bool launch_scale(Plan* p, const double* freqs, int n_chan, cudaStream_t st) {
-    scale_kernel<<<1, 256, 0, st>>>(freqs, n_chan, p->geom.N / 2, chan_supported(p, n_chan) ? 1 : 0, p->ws.d_scale,
+    scale_kernel<<<1, 256, 0, st>>>(freqs, n_chan, p->geom.N / 2, (chan_supported(p, n_chan) || chanws_supported(p, n_chan)) ? 1 : 0, p->ws.d_scale,
                                     p->ws.d_scale_ref, p->ws.d_dispatch, (double4*)p->ws.d_group);
     p->last_launches += 1;
     return cuda_ok(cudaGetLastError(), "scale_kernel");

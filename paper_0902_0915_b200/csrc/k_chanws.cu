@@ -1,0 +1,759 @@
+// k_chanws.cu - K6, the warp-specialised channel-SIMD gridder (a2 + a4 + a5) for finely channelised data (C4).
+//
+// Same ownership idea as K5 (k_chan.cu): the 32 lanes of a warp are 32 ADJACENT CHANNELS (768 channels
+// of 40 kHz see a baseline at almost the same cell, and every channel owns its grid), a warp owns a 4x2-cell block and
+// keeps its 8 cells x 4 pol x (re, im) = 64 fp32 accumulators in registers from the first tap to the single store.
+// What changed is everything around the FMA loop.  K5 ran its phases (bucket sweep, fp64 index, staging, FMA,
+// write-out) one after the other on all warps of a CTA, separated by CTA-wide barriers, and repeated the sweep and
+// index work for each 16x4 strip: 5.8 G warp instructions for C4, 80 % of them overhead, issue slot use 42 %
+// (profiles/r01_chan_v8_c4x128.md).  K6 is a producer / consumer pipeline with no CTA-wide barrier in steady state:
+//
+//   chan_index_kernel (pre-pass, once per call): the exact fp64 index (index.cuh) of every (row, channel), packed in
+//       32 bits (stamp origin + table row per axis), and per (row, 32-channel group) the bounding box of the stamp
+//       origins over the group's channels.  After it nothing on the path touches fp64 per sample.
+//
+//   chanws_kernel, persistent, one CTA of 20 warps per SM; item = (16 x 8 cell tile, 32-channel group):
+//     warp 16  "sweeper"  walks the uv buckets (k_bin.cu) under the item's tile, tests the bounding boxes (integer
+//                         compares), and appends the hits (row, 16-bit block mask) to a queue in batches of 32;
+//     warp 17, 18 "stagers"  one batch each in turn: one bulk-async copy (TMA engine, mbarrier complete_tx) of the
+//                         32 channels x 32 B of visibilities per hit, the packed indices -> per-lane table offsets,
+//                         the weights;
+//     warp 0..15 "consumers" (4 x 4 blocks of 4 x 2 cells): wait on the batch's mbarrier, run the FFMA2 loop of K5
+//                         over the hits that touch their block, release the batch; at the end of an item put the
+//                         accumulators into a 128 B-swizzled stage and signal the store warp;
+//     warp 19  "store"    one cp.async.bulk.tensor store per (2 tile rows x 32 channels x 4 pol) box through a 4-D
+//                         tensor map of grid_out with dimension order (u, channel, v, pol); items nothing reaches
+//                         are zero-filled from a small zero buffer without involving any other warp.
+//
+// No atomics on grid data, every cell of grid_out is written exactly once (R10), the hit order is a pure function
+// of the sorted rows, so the grid is bit-identical from run to run.  Registers: the kernel is compiled for 96 per
+// thread (640 threads); with setmaxnreg the consumers raise themselves to 104 (64 accumulators + two operand sets, no
+// spills) and the four service warps drop to 64: 16 x 104 + 4 x 64 = 20 x 96, exactly the CTA's register pool (an
+// increase that the pool cannot serve blocks for ever).
+#include <cuda.h>
+
+#include "plan.h"
+
+namespace mwa {
+
+constexpr int k6Consumers = 16;                       // consumer warps
+constexpr int k6Threads = (k6Consumers + 4) * 32;     // + sweeper, two stagers, store warp
+constexpr int k6TileX = 16, k6TileY = 8;
+constexpr int k6Batch = 32;                           // hits per batch (one per lane of a stager)
+constexpr int k6Stages = 2;                           // batches in flight (one per stager)
+constexpr int k6BatchRing = 8;                        // batch descriptors / queue segments between sweeper and stagers
+constexpr int k6ItemRing = 16;                        // item descriptors between sweeper and store warp
+constexpr int k6PadU = 16, k6PadV = 8;                // zero padding in front of a table row (floats)
+constexpr int k6ZeroFloats = 32;                      // all-zero block behind each table (target of a missing lane)
+constexpr int k6WoBytes = 4 * 32768;                  // write-out stage: 4 block rows x [pol 4][v 2][chan 32][128 B]
+constexpr int k6StageV = k6Batch * 1024, k6StageGeo = k6Batch * 128, k6StageW = k6Batch * 128;
+constexpr int k6StageBytes = k6StageV + k6StageGeo + k6StageW;
+constexpr int k6ZeroBytes = 4096;                     // zero buffer: [chan 32][128 B]
+constexpr unsigned k6FlagEnd = 1u, k6FlagExit = 2u;
+constexpr unsigned k6Invalid = 0xffffffffu;           // packed index of a dropped sample
+constexpr long long k6SpinLimit = 6000000000LL;       // ~3 s of SM clocks: a wait this long is a bug -> abort, never hang
+
+enum { K6_ERR_NONE = 0, K6_ERR_FULL = 1, K6_ERR_EMPTY = 2, K6_ERR_WOFULL = 3, K6_ERR_WOEMPTY = 4, K6_ERR_BATCH = 5,
+       K6_ERR_ITEM = 6, K6_ERR_RING = 7 };
+
+struct K6Params {
+    GridGeom g;
+    const double4* group;        // [n_groups] s_lo, s_hi, s_ref / s_lo, s_ref / s_hi (scale_kernel)
+    const int* bucket_start;     // [nb*nb + 1]
+    const int* perm;             // [n_vis] sorted position -> row
+    const unsigned* pre;         // [n_vis][n_groups * 32] packed indices, by ROW
+    const ushort4* bb;           // [n_groups][n_vis] bounding boxes, by SORTED POSITION
+    int* counter;                // work counter
+    int* stats;                  // [8] error, items, items with hits, batches, max hits of an item
+    const int* dispatch;         // device-side design choice (AUTO); null = always run
+    int dispatch_want;
+    const float* vis;            // [n_vis][n_chan][8]
+    const float* weights;        // [n_vis][n_chan] or null
+    const float* table;          // [(O+1)][W]
+    int n_vis, n_chan, n_groups, nb;
+    int ntx, nty;                // tiles per row / column
+    int rlu, rlv, n_tu, n_tv;    // padded row lengths and sizes (floats) of the shifted table copies
+    long long n_items;
+};
+
+struct K6Ctrl {
+    unsigned long long full[k6Stages], empty[k6Stages];     // mbarriers: batch staged / batch consumed
+    unsigned long long wo_full[4], wo_empty[4];             // mbarriers: block row staged for the store / stage free
+    int st_n[k6Stages];
+    unsigned st_flags[k6Stages];
+    unsigned st_mask[k6Stages][k6Batch];
+    int q_row[k6BatchRing * k6Batch];
+    unsigned q_mask[k6BatchRing * k6Batch];                 // bits 0..15 block mask, bit 16: slow staging path
+    int b_n[k6BatchRing];
+    unsigned b_flags[k6BatchRing];
+    int b_x0[k6BatchRing], b_y0[k6BatchRing], b_g[k6BatchRing];
+    int it_x0[k6ItemRing], it_y0[k6ItemRing], it_g[k6ItemRing], it_kind[k6ItemRing];   // kind 0 zero-fill, 1 consumers, 2 exit
+    volatile int pub_batches, pub_items, done_items;
+    volatile int done_batches[k6Stages];
+    volatile int abort;
+};
+
+struct K6Layout { size_t wo, ring, zero, tu, tv, ctrl, total; };
+
+__host__ __device__ inline K6Layout k6_layout(int n_tu, int n_tv) {
+    K6Layout L;
+    L.wo = 0;
+    L.ring = L.wo + k6WoBytes;
+    L.zero = L.ring + (size_t)k6Stages * k6StageBytes;
+    L.tu = L.zero + k6ZeroBytes;
+    L.tv = L.tu + (size_t)(n_tu + k6ZeroFloats) * 4;
+    L.ctrl = (L.tv + (size_t)(n_tv + k6ZeroFloats) * 4 + 15) & ~size_t(15);
+    L.total = L.ctrl + sizeof(K6Ctrl) + 1024;               // + slack for the 1024 B alignment of the base
+    return L;
+}
+
+// ------------------------------------------------------------------------------------------------ PTX helpers
+typedef unsigned long long u64;
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try(unsigned bar, unsigned parity) {
+    unsigned ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
+// Bounded wait: returns false when the kernel is being aborted (a wait that exceeded k6SpinLimit raises the abort).
+__device__ __forceinline__ bool mbar_wait(unsigned bar, unsigned parity, volatile int* abort_flag, int code) {
+    if (mbar_try(bar, parity)) return true;
+    const long long t0 = clock64();
+    while (!mbar_try(bar, parity)) {
+        if (*abort_flag) return false;
+        if (clock64() - t0 > k6SpinLimit) { *abort_flag = code; return false; }
+    }
+    return true;
+}
+__device__ __forceinline__ bool spin_until_gt(volatile int* var, int value, volatile int* abort_flag, int code) {
+    if (*var > value) return true;
+    const long long t0 = clock64();
+    while (!(*var > value)) {
+        if (*abort_flag) return false;
+        if (clock64() - t0 > k6SpinLimit) { *abort_flag = code; return false; }
+        __nanosleep(64);
+    }
+    return true;
+}
+__device__ __forceinline__ void bulk_load(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_store4(const CUtensorMap* m, unsigned src, int d0, int d1, int d2, int d3) {
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%1, %2, %3, %4}], [%5];"
+                 ::"l"(m), "r"(d0), "r"(d1), "r"(d2), "r"(d3), "r"(src) : "memory");
+}
+__device__ __forceinline__ void k6_unpack2(u64 v, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ u64 k6_pack2(float a, float b) {
+    u64 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
+    return r;
+}
+__device__ __forceinline__ void k6_ffma2(u64& d, u64 a, u64 b) { asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(a), "l"(b)); }
+
+// ------------------------------------------------------------------------------------------------ pre-pass
+// One warp per (sorted row r, channel group g), lane = channel.  pre[row][c] = origin_u | ru << 11 | origin_v << 16
+// | rv << 27 (origin = i - h, the first cell of the stamp), k6Invalid for a dropped sample (R11) or a channel
+// beyond n_chan.  bb[g][r] = (min origin_u, max origin_u | any-dropped << 15, min origin_v, max origin_v) over the
+// valid lanes; a group with no valid lane gets min = 0x7fff, which no tile reaches.
+__global__ void __launch_bounds__(256)
+chan_index_kernel(GridGeom g, const double4* __restrict__ row_sorted, const double* __restrict__ scale, int n_vis,
+                  int n_chan, int n_groups, unsigned* __restrict__ pre, ushort4* __restrict__ bb,
+                  const int* __restrict__ dispatch, int dispatch_want) {
+    if (dispatch != nullptr && *dispatch != dispatch_want) return;
+    const int lane = threadIdx.x & 31;
+    const long long warps = ((long long)gridDim.x * blockDim.x) >> 5;
+    const long long tasks = (long long)n_vis * n_groups;
+    const int ncp = n_groups * 32;
+    for (long long t = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; t < tasks; t += warps) {
+        const int grp = (int)(t / n_vis), r = (int)(t - (long long)grp * n_vis);
+        const double4 rec = row_sorted[r];
+        const int c = grp * 32 + lane;
+        const bool cvalid = c < n_chan;
+        const double sc = scale[cvalid ? c : n_chan - 1];
+        SampleIndex s;
+        const bool ok = sample_index(rec.x, rec.y, sc, g, s) && cvalid;
+        const int ou = s.iu - g.h, ov = s.iv - g.h;
+        const unsigned word = ok ? ((unsigned)ou | ((unsigned)s.ru << 11) | ((unsigned)ov << 16) | ((unsigned)s.rv << 27)) : k6Invalid;
+        pre[(size_t)(int)rec.z * ncp + c] = word;
+        const unsigned full = 0xffffffffu;
+        const unsigned u_min = __reduce_min_sync(full, ok ? (unsigned)ou : 0x7fffu);
+        const unsigned u_max = __reduce_max_sync(full, ok ? (unsigned)ou : 0u);
+        const unsigned v_min = __reduce_min_sync(full, ok ? (unsigned)ov : 0x7fffu);
+        const unsigned v_max = __reduce_max_sync(full, ok ? (unsigned)ov : 0u);
+        const unsigned bad = __ballot_sync(full, cvalid && !ok) != 0u ? 0x8000u : 0u;
+        if (lane == 0)
+            bb[(size_t)grp * n_vis + r] = make_ushort4((unsigned short)u_min, (unsigned short)(u_max | bad),
+                                                        (unsigned short)v_min, (unsigned short)v_max);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ main kernel
+template <bool HAS_W>
+__global__ void __launch_bounds__(k6Threads, 1)
+chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtensorMap map_out,
+              const __grid_constant__ CUtensorMap map_zero) {
+    if (P.dispatch != nullptr && *P.dispatch != P.dispatch_want) return;
+    extern __shared__ unsigned char smem_dyn[];
+    unsigned char* base = reinterpret_cast<unsigned char*>((reinterpret_cast<size_t>(smem_dyn) + 1023) & ~size_t(1023));
+    const K6Layout L = k6_layout(P.n_tu, P.n_tv);
+    float* tu = reinterpret_cast<float*>(base + L.tu);
+    float* tv = reinterpret_cast<float*>(base + L.tv);
+    K6Ctrl& S = *reinterpret_cast<K6Ctrl*>(base + L.ctrl);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int W = P.g.W, O1 = P.g.O + 1, N = P.g.N;
+    const unsigned full = 0xffffffffu;
+
+    // ---- set-up by all 20 warps: shifted zero-padded table copies (as K5), zero buffer, control block, mbarriers
+    //   tu[s][r][q] = Tp_u[r][q + s], Tp_u[r][k6PadU + t] = T[r][t]   s = 0..3 (LDS.128 alignment)
+    //   tv[s][r][q] = Tp_v[r][q + s], Tp_v[r][k6PadV + t] = T[r][t]   s = 0..1 (LDS.64 alignment)
+    for (int k = tid; k < P.n_tu + k6ZeroFloats; k += k6Threads) {
+        float v = 0.0f;
+        if (k < P.n_tu) {
+            const int q = k % P.rlu, r = (k / P.rlu) % O1, s = k / (P.rlu * O1);
+            const int t = q + s - k6PadU;
+            if (t >= 0 && t < W) v = P.table[r * W + t];
+        }
+        tu[k] = v;
+    }
+    for (int k = tid; k < P.n_tv + k6ZeroFloats; k += k6Threads) {
+        float v = 0.0f;
+        if (k < P.n_tv) {
+            const int q = k % P.rlv, r = (k / P.rlv) % O1, s = k / (P.rlv * O1);
+            const int t = q + s - k6PadV;
+            if (t >= 0 && t < W) v = P.table[r * W + t];
+        }
+        tv[k] = v;
+    }
+    for (int k = tid; k < k6ZeroBytes / 4; k += k6Threads) reinterpret_cast<float*>(base + L.zero)[k] = 0.0f;
+    for (int k = tid; k < (int)(sizeof(K6Ctrl) / 4); k += k6Threads) reinterpret_cast<int*>(&S)[k] = 0;
+    __syncthreads();
+    if (tid == 0) {
+        for (int s = 0; s < k6Stages; ++s) { mbar_init(smem_u32(&S.full[s]), 1); mbar_init(smem_u32(&S.empty[s]), k6Consumers); }
+        for (int r = 0; r < 4; ++r) { mbar_init(smem_u32(&S.wo_full[r]), 4); mbar_init(smem_u32(&S.wo_empty[r]), 1); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // zero buffer and barriers visible to the async proxy
+    __syncthreads();
+
+    volatile int* abort_flag = &S.abort;
+    const unsigned ring_s = smem_u32(base + L.ring);
+
+    if (warp < k6Consumers) {
+        // =========================================================================================== consumers
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 104;");
+        const int bx = warp & 3, by = warp >> 2;
+        const unsigned wbit = (unsigned)warp;                           // bit by * 4 + bx of a hit mask
+        const unsigned tu_s = smem_u32(tu) + 16u * bx, tv_s = smem_u32(tv) + 8u * by;
+        // the lane's two 16 B chunks of a 128 B stage row: chunk (2 bx + k) ^ (row & 7), row & 7 = lane & 7
+        const unsigned wo_s = smem_u32(base + L.wo) + 32768u * by + 128u * lane;
+        const unsigned wo_c0 = wo_s + 16u * ((2u * bx) ^ (lane & 7u)), wo_c1 = wo_s + 16u * ((2u * bx + 1u) ^ (lane & 7u));
+        u64 acc[2][4][4];                                               // [row i][col j][pol] = (re, im) of the lane's channel
+#pragma unroll
+        for (int i = 0; i < 2; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+#pragma unroll
+                for (int p = 0; p < 4; ++p) acc[i][j][p] = 0ull;
+        int n_written = 0;
+        for (int k = 0;; ++k) {
+            const int s = k & 1;
+            if (!mbar_wait(smem_u32(&S.full[s]), (unsigned)((k >> 1) & 1), abort_flag, K6_ERR_FULL)) break;
+            const unsigned flags = S.st_flags[s];
+            if (flags & k6FlagExit) break;
+            unsigned m = __ballot_sync(full, (S.st_mask[s][lane] >> wbit) & 1u);
+            const unsigned zs_s = ring_s + (unsigned)s * k6StageBytes + 32u * lane;
+            const unsigned geo_s = ring_s + (unsigned)s * k6StageBytes + k6StageV + 4u * lane;
+            const unsigned wt_s = geo_s + k6StageGeo;
+            if (m != 0u) {
+                // software pipeline over the set bits of m, two visits per trip with two register sets (as K5 phase B)
+#define K6_NEXT(mm, prev) ((mm) ? (int)(__ffs(mm) - 1) : (prev)); (mm) &= (mm) - 1u
+#define K6_LOAD(h, g, Z0, Z1, Z2, Z3, U0, U1, U2, U3, V0, V1, WT)                                                         \
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(Z0), "=l"(Z1) : "r"(zs_s + 1024u * (h)));                       \
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(Z2), "=l"(Z3) : "r"(zs_s + 1024u * (h) + 16u));                 \
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(U0), "=f"(U1), "=f"(U2), "=f"(U3) : "r"(tu_s + ((g) & 0xffffu))); \
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(V0), "=f"(V1) : "r"(tv_s + ((g) >> 16)));                       \
+    if (HAS_W) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(WT) : "r"(wt_s + 128u * (h)));
+#define K6_FMA(Z0, Z1, Z2, Z3, U0, U1, U2, U3, V0, V1, WT)                                                                \
+    {                                                                                                                     \
+        const float kvw[2] = {HAS_W ? V0 * WT : V0, HAS_W ? V1 * WT : V1};                                                \
+        const float kuu[4] = {U0, U1, U2, U3};                                                                            \
+        _Pragma("unroll") for (int i = 0; i < 2; ++i) _Pragma("unroll") for (int j = 0; j < 4; ++j) {                      \
+            const float kq = kvw[i] * kuu[j];                                                                             \
+            const u64 kk = k6_pack2(kq, kq);                                                                              \
+            k6_ffma2(acc[i][j][0], kk, Z0);                                                                               \
+            k6_ffma2(acc[i][j][1], kk, Z1);                                                                               \
+            k6_ffma2(acc[i][j][2], kk, Z2);                                                                               \
+            k6_ffma2(acc[i][j][3], kk, Z3);                                                                               \
+        }                                                                                                                 \
+    }
+                const int cnt = __popc(m);
+                u64 az0, az1, az2, az3, bz0, bz1, bz2, bz3;
+                float au0, au1, au2, au3, av0, av1, aw = 1.0f, bu0, bu1, bu2, bu3, bv0, bv1, bw = 1.0f;
+                const int h0 = K6_NEXT(m, 0);
+                int h1 = K6_NEXT(m, h0);
+                int h2 = K6_NEXT(m, h1);
+                unsigned g1, g2;
+                {
+                    unsigned g0;
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g0) : "r"(geo_s + 128u * h0));
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g1) : "r"(geo_s + 128u * h1));
+                    K6_LOAD(h0, g0, az0, az1, az2, az3, au0, au1, au2, au3, av0, av1, aw)
+                }
+#pragma unroll 1
+                for (int v = 0; v < cnt; v += 2) {
+                    K6_LOAD(h1, g1, bz0, bz1, bz2, bz3, bu0, bu1, bu2, bu3, bv0, bv1, bw)
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g2) : "r"(geo_s + 128u * h2));
+                    const int h3 = K6_NEXT(m, h2);
+                    K6_FMA(az0, az1, az2, az3, au0, au1, au2, au3, av0, av1, aw)
+                    if (v + 1 >= cnt) break;
+                    K6_LOAD(h2, g2, az0, az1, az2, az3, au0, au1, au2, au3, av0, av1, aw)
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g1) : "r"(geo_s + 128u * h3));
+                    const int h4 = K6_NEXT(m, h3);
+                    K6_FMA(bz0, bz1, bz2, bz3, bu0, bu1, bu2, bu3, bv0, bv1, bw)
+                    h1 = h3;
+                    h2 = h4;
+                }
+#undef K6_NEXT
+#undef K6_LOAD
+#undef K6_FMA
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&S.empty[s]));          // this warp has read everything it needs of the batch
+            if (flags & k6FlagEnd) {
+                // ---- a5: accumulators -> swizzled stage of this block row; the store warp issues the TMA store
+                if (!mbar_wait(smem_u32(&S.wo_empty[by]), (unsigned)((n_written & 1) ^ 1), abort_flag, K6_ERR_WOEMPTY)) break;
+#pragma unroll
+                for (int pol = 0; pol < 4; ++pol)
+#pragma unroll
+                    for (int i = 0; i < 2; ++i) {
+                        float a0, a1, a2, a3, b0, b1, b2, b3;
+                        k6_unpack2(acc[i][0][pol], a0, a1); k6_unpack2(acc[i][1][pol], a2, a3);
+                        k6_unpack2(acc[i][2][pol], b0, b1); k6_unpack2(acc[i][3][pol], b2, b3);
+                        const unsigned ro = (unsigned)(pol * 2 + i) * 4096u;
+                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wo_c0 + ro), "f"(a0), "f"(a1), "f"(a2), "f"(a3) : "memory");
+                        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wo_c1 + ro), "f"(b0), "f"(b1), "f"(b2), "f"(b3) : "memory");
+                        acc[i][0][pol] = 0ull; acc[i][1][pol] = 0ull; acc[i][2][pol] = 0ull; acc[i][3][pol] = 0ull;
+                    }
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&S.wo_full[by]));
+                ++n_written;
+            }
+        }
+    } else {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
+        const int role = warp - k6Consumers;
+        if (role == 0) {
+            // =========================================================================================== sweeper
+            const unsigned lt_mask = (1u << lane) - 1u;
+            int b_next = 0;              // global index of the first batch of the current item
+            int n_pub = 0;               // batches published so far (= b_next + complete batches of the current item)
+            int i_pub = 0;               // items published so far
+            int st_items = 0, st_hit_items = 0, st_max = 0;
+            bool alive = true;
+            // wait until batch b's queue segment and descriptor may be reused (batch b - ring has been staged)
+            auto batch_slot_free = [&](int b) -> bool {
+                const int old = b - k6BatchRing;
+                if (old < 0) return true;
+                return spin_until_gt(&S.done_batches[old & 1], old >> 1, abort_flag, K6_ERR_RING);
+            };
+            auto publish_batches = [&](int upto, int n_last, unsigned flags_last, int x0, int y0, int grp) {
+                // publishes batches [n_pub, upto]; all but the last are full and carry no flag
+                if (lane == 0) {
+                    for (int b = n_pub; b <= upto; ++b) {
+                        const int q = b % k6BatchRing;
+                        S.b_n[q] = b == upto ? n_last : k6Batch;
+                        S.b_flags[q] = b == upto ? flags_last : 0u;
+                        S.b_x0[q] = x0; S.b_y0[q] = y0; S.b_g[q] = grp;
+                    }
+                }
+                __syncwarp();
+                __threadfence_block();
+                if (lane == 0) S.pub_batches = upto + 1;
+                n_pub = upto + 1;
+            };
+            auto publish_item = [&](int x0, int y0, int grp, int kind) -> bool {
+                if (!spin_until_gt(&S.done_items, i_pub - k6ItemRing, abort_flag, K6_ERR_ITEM)) return false;
+                if (lane == 0) {
+                    const int q = i_pub % k6ItemRing;
+                    S.it_x0[q] = x0; S.it_y0[q] = y0; S.it_g[q] = grp; S.it_kind[q] = kind;
+                    __threadfence_block();
+                    S.pub_items = i_pub + 1;
+                }
+                __syncwarp();
+                ++i_pub;
+                return true;
+            };
+            while (alive) {
+                long long item = 0;
+                if (lane == 0) item = (long long)atomicAdd(P.counter, 1);
+                item = __shfl_sync(full, item, 0);
+                if (item >= P.n_items) break;
+                // item order: x fastest, then y, then channel group (neighbouring tiles of one group share visibility rows in L2)
+                const int tx = (int)(item % P.ntx);
+                const int ty = (int)((item / P.ntx) % P.nty);
+                const int grp = (int)(item / ((long long)P.ntx * P.nty));
+                const int X0 = tx * k6TileX, Y0 = ty * k6TileY;
+                // bucket window at the reference scale (conservative, K5's back-projection)
+                const double4 gi = P.group[grp];
+                int wx0 = 0, wx1 = P.nb - 1, wy0 = 0, wy1 = P.nb - 1;
+                if (gi.z == gi.z && gi.w == gi.w) {
+                    const double halfN = (double)(N / 2);
+                    const double pad = (double)P.g.h + 1.25;
+                    const double ax = (double)X0 - halfN - pad, bxx = (double)(X0 + k6TileX - 1) - halfN + pad;
+                    const double ay = (double)Y0 - halfN - pad, byy = (double)(Y0 + k6TileY - 1) - halfN + pad;
+                    const double ib = 1.0 / kBucketCells, top = (double)(P.nb - 1);
+                    wx0 = (int)fmin(fmax(floor((fmin(ax * gi.z, ax * gi.w) + halfN) * ib), 0.0), top);
+                    wx1 = (int)fmin(fmax(floor((fmax(bxx * gi.z, bxx * gi.w) + halfN) * ib), 0.0), top);
+                    wy0 = (int)fmin(fmax(floor((fmin(ay * gi.z, ay * gi.w) + halfN) * ib), 0.0), top);
+                    wy1 = (int)fmin(fmax(floor((fmax(byy * gi.z, byy * gi.w) + halfN) * ib), 0.0), top);
+                }
+                int cnt = 0, opened = 0;
+                const ushort4* bbg = P.bb + (size_t)grp * P.n_vis;
+                for (int rg = wy0; rg <= wy1 && alive; rg += 32) {
+                    int k0 = 0, len = 0;
+                    if (rg + lane <= wy1) {
+                        k0 = __ldg(P.bucket_start + (rg + lane) * P.nb + wx0);
+                        len = __ldg(P.bucket_start + (rg + lane) * P.nb + wx1 + 1) - k0;
+                    }
+                    int incl = len;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int t = __shfl_up_sync(full, incl, o);
+                        if (lane >= o) incl += t;
+                    }
+                    const int total = __shfl_sync(full, incl, 31);
+                    const int excl = incl - len;
+                    for (int cb = 0; cb < total && alive; cb += 32) {
+                        const int f = cb + lane;
+                        int lo = 0;                                          // smallest bucket row with incl > f
+#pragma unroll
+                        for (int st = 16; st > 0; st >>= 1) {
+                            const int t = __shfl_sync(full, incl, lo + st - 1);
+                            if (t <= f) lo += st;
+                        }
+                        lo = min(lo, 31);
+                        const int rk0 = __shfl_sync(full, k0, lo), rex = __shfl_sync(full, excl, lo);
+                        bool hit = false;
+                        unsigned mask = 0u;
+                        int row = 0;
+                        if (f < total) {
+                            const int kpos = rk0 + (f - rex);
+                            const ushort4 b = bbg[kpos];
+                            row = __ldg(P.perm + kpos);
+                            const int u_min = b.x, u_max = b.y & 0x7fff, v_min = b.z, v_max = b.w;
+                            hit = u_min <= X0 + k6TileX - 1 && u_max + W - 1 >= X0 && v_min <= Y0 + k6TileY - 1 && v_max + W - 1 >= Y0;
+                            if (hit) {
+                                const int bxl = max(0, (u_min - X0) >> 2), bxh = min(3, (u_max + W - 1 - X0) >> 2);
+                                const int byl = max(0, (v_min - Y0) >> 1), byh = min(3, (v_max + W - 1 - Y0) >> 1);
+                                const unsigned mu = (2u << bxh) - (1u << bxl);
+                                const unsigned mv = 0x1111u & ((1u << (4 * (byh + 1))) - (1u << (4 * byl)));
+                                mask = mu * mv | ((b.y & 0x8000u) ? 0x10000u : 0u);
+                            }
+                        }
+                        const unsigned hm = __ballot_sync(full, hit);
+                        const int n_new = __popc(hm);
+                        if (n_new == 0) continue;
+                        const int need = (cnt + n_new - 1) / k6Batch + 1;    // batches of this item that must be open
+                        while (opened < need) {
+                            if (!batch_slot_free(b_next + opened)) { alive = false; break; }
+                            ++opened;
+                        }
+                        if (!alive) break;
+                        if (hit) {
+                            const int i = cnt + __popc(hm & lt_mask);
+                            const int slot = ((b_next + i / k6Batch) % k6BatchRing) * k6Batch + (i % k6Batch);
+                            S.q_row[slot] = row;
+                            S.q_mask[slot] = mask;
+                        }
+                        cnt += n_new;
+                        const int complete = b_next + (cnt - 1) / k6Batch - 1;    // last batch known to have a successor
+                        if (complete >= n_pub) publish_batches(complete, k6Batch, 0u, X0, Y0, grp);
+                    }
+                }
+                if (!alive) break;
+                if (cnt > 0) {
+                    const int last = b_next + (cnt - 1) / k6Batch;
+                    publish_batches(last, cnt - ((cnt - 1) / k6Batch) * k6Batch, k6FlagEnd, X0, Y0, grp);
+                    b_next = last + 1;
+                    ++st_hit_items;
+                }
+                ++st_items;
+                st_max = max(st_max, cnt);
+                if (!publish_item(X0, Y0, grp, cnt > 0 ? 1 : 0)) break;
+            }
+            // exit: one flagged batch per stager (consumers stop at the first one), one flagged item for the store warp
+            if (!*abort_flag) {
+                bool ok = true;
+                for (int e = 0; e < k6Stages && ok; ++e) ok = batch_slot_free(b_next + e);
+                if (ok) {
+                    if (lane == 0) {
+                        for (int e = 0; e < k6Stages; ++e) {
+                            const int q = (b_next + e) % k6BatchRing;
+                            S.b_n[q] = 0; S.b_flags[q] = k6FlagExit; S.b_x0[q] = 0; S.b_y0[q] = 0; S.b_g[q] = 0;
+                        }
+                        __threadfence_block();
+                        S.pub_batches = b_next + k6Stages;
+                    }
+                    __syncwarp();
+                }
+                publish_item(0, 0, 0, 2);
+            }
+            if (lane == 0 && P.stats) {
+                atomicAdd(P.stats + 1, st_items);
+                atomicAdd(P.stats + 2, st_hit_items);
+                atomicAdd(P.stats + 3, b_next);
+                atomicMax(P.stats + 4, st_max);
+            }
+        } else if (role <= k6Stages) {
+            // =========================================================================================== stagers
+            const int s = role - 1;
+            const unsigned st_base = ring_s + (unsigned)s * k6StageBytes;
+            const unsigned full_bar = smem_u32(&S.full[s]), empty_bar = smem_u32(&S.empty[s]);
+            const unsigned zero_geo = (unsigned)(P.n_tu * 4) | ((unsigned)(P.n_tv * 4) << 16);
+            const int ncp = P.n_groups * 32;
+            for (int b = s;; b += k6Stages) {
+                if (!spin_until_gt(&S.pub_batches, b, abort_flag, K6_ERR_BATCH)) break;
+                __threadfence_block();
+                const int q = b % k6BatchRing;
+                const int n = S.b_n[q];
+                const unsigned flags = S.b_flags[q];
+                const int X0 = S.b_x0[q], Y0 = S.b_y0[q], grp = S.b_g[q];
+                int row = 0;
+                unsigned mask = 0u;
+                if (lane < n) { row = S.q_row[q * k6Batch + lane]; mask = S.q_mask[q * k6Batch + lane]; }
+                __syncwarp();
+                const int use = b >> 1;                                      // this stage's use number
+                if (!mbar_wait(empty_bar, (unsigned)((use & 1) ^ 1), abort_flag, K6_ERR_EMPTY)) break;
+                const int c0 = grp * 32;
+                const int nch = min(32, P.n_chan - c0);                      // channels of the group (last group may be ragged)
+                const bool cvalid = lane < nch;
+                const bool slow = lane < n && (((mask >> 16) & 1u) || nch < 32);   // per hit: dropped lanes / ragged group -> no bulk copy
+                const bool fast = lane < n && !slow;
+                const unsigned n_fast = __popc(__ballot_sync(full, fast));
+                S.st_mask[s][lane] = lane < n ? (mask & 0xffffu) : 0u;
+                if (lane == 0) { S.st_n[s] = n; S.st_flags[s] = flags; }
+                if (fast)                                                    // lane = hit: 32 channels x 32 B in one bulk copy
+                    bulk_load(st_base + 1024u * lane, P.vis + ((size_t)row * P.n_chan + c0) * 8, 1024u, full_bar);
+                // lane = channel: packed index -> table offsets, weight; slow-path visibilities
+                for (int h0 = 0; h0 < n; h0 += 8) {
+                    unsigned pw[8];
+                    float ww[8];
+                    int rr[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        pw[u] = k6Invalid; ww[u] = 0.0f; rr[u] = 0;
+                        if (h0 + u < n) {
+                            rr[u] = __shfl_sync(full, row, h0 + u);
+                            pw[u] = __ldg(P.pre + (size_t)rr[u] * ncp + c0 + lane);
+                            if (HAS_W && cvalid) ww[u] = __ldg(P.weights + (size_t)rr[u] * P.n_chan + c0 + lane);
+                        }
+                    }
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        if (h0 + u < n) {
+                            unsigned geo = zero_geo;
+                            const unsigned w32 = pw[u];
+                            if (w32 != k6Invalid) {
+                                const int ou = (int)(w32 & 0x7ffu), ru = (int)((w32 >> 11) & 31u);
+                                const int ov = (int)((w32 >> 16) & 0x7ffu), rv = (int)(w32 >> 27);
+                                const int tu_ = k6PadU + X0 - ou, tv_ = k6PadV + Y0 - ov;
+                                const unsigned iu_ = (unsigned)(W - 1 + ou - X0), iv_ = (unsigned)(W - 1 + ov - Y0);
+                                if (iu_ < (unsigned)(k6TileX + W - 1) && iv_ < (unsigned)(k6TileY + W - 1)) {
+                                    const int su = tu_ & 3, sv = tv_ & 1;
+                                    const int offu = ru * P.rlu + tu_ + su * (O1 * P.rlu - 1);
+                                    const int offv = rv * P.rlv + tv_ + sv * (O1 * P.rlv - 1);
+                                    geo = (unsigned)(offu * 4) | ((unsigned)(offv * 4) << 16);
+                                }
+                            }
+                            const unsigned hh = (unsigned)(h0 + u);
+                            asm volatile("st.shared.u32 [%0], %1;" ::"r"(st_base + k6StageV + 128u * hh + 4u * lane), "r"(geo) : "memory");
+                            if (HAS_W)
+                                asm volatile("st.shared.f32 [%0], %1;" ::"r"(st_base + k6StageV + k6StageGeo + 128u * hh + 4u * lane), "f"(ww[u]) : "memory");
+                            if (__shfl_sync(full, (int)slow, h0 + u)) {
+                                float4 va = make_float4(0.f, 0.f, 0.f, 0.f), vb = va;      // a dropped sample contributes nothing (R11)
+                                if (cvalid && w32 != k6Invalid) {
+                                    const float4* src = reinterpret_cast<const float4*>(P.vis + ((size_t)rr[u] * P.n_chan + c0 + lane) * 8);
+                                    va = __ldg(src);
+                                    vb = __ldg(src + 1);
+                                }
+                                const unsigned dst = st_base + 1024u * hh + 32u * lane;
+                                asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "f"(va.x), "f"(va.y), "f"(va.z), "f"(va.w) : "memory");
+                                asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(dst + 16u), "f"(vb.x), "f"(vb.y), "f"(vb.z), "f"(vb.w) : "memory");
+                            }
+                        }
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) {
+                    mbar_arrive_tx(full_bar, n_fast * 1024u);
+                    __threadfence_block();
+                    S.done_batches[s] = use + 1;                             // queue segment and descriptor of batch b are free again
+                }
+                if (flags & k6FlagExit) break;
+            }
+        } else {
+            // =========================================================================================== store warp
+            if (lane == 0) {
+                const unsigned wo0 = smem_u32(base + L.wo), zero_s = smem_u32(base + L.zero);
+                int n_written = 0;
+                unsigned pending = 0u;                                       // block rows whose store has been issued but not released
+                auto release_all = [&]() {
+                    if (pending == 0u) return;
+                    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the TMA engine has read the stages
+#pragma unroll
+                    for (int r = 0; r < 4; ++r)
+                        if (pending & (1u << r)) mbar_arrive(smem_u32(&S.wo_empty[r]));
+                    pending = 0u;
+                };
+                for (int i = 0;; ++i) {
+                    if (S.pub_items <= i) {
+                        release_all();                                       // idle: let the consumers have their stage back
+                        if (!spin_until_gt(&S.pub_items, i, abort_flag, K6_ERR_ITEM)) break;
+                    }
+                    __threadfence_block();
+                    const int q = i % k6ItemRing;
+                    const int X0 = S.it_x0[q], Y0 = S.it_y0[q], c0 = S.it_g[q] * 32, kind = S.it_kind[q];
+                    if (kind == 2) break;
+                    if (kind == 0) {
+                        release_all();                                       // a run of empty items must not keep the consumers waiting
+                        for (int pol = 0; pol < 4; ++pol)
+                            for (int v = 0; v < k6TileY; ++v)
+                                if (Y0 + v < N) tma_store4(&map_zero, zero_s, X0, c0, Y0 + v, pol);
+                        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                    } else {
+                        bool ok = true;
+                        for (int r = 0; r < 4 && ok; ++r) {
+                            const unsigned bar = smem_u32(&S.wo_full[r]);
+                            const unsigned par = (unsigned)(n_written & 1);
+                            if (!mbar_try(bar, par)) {
+                                release_all();
+                                ok = mbar_wait(bar, par, abort_flag, K6_ERR_WOFULL);
+                                if (!ok) break;
+                            }
+                            if (Y0 + 2 * r < N) tma_store4(&map_out, wo0 + 32768u * r, X0, c0, Y0 + 2 * r, 0);
+                            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                            pending |= 1u << r;
+                        }
+                        if (!ok) break;
+                        ++n_written;
+                    }
+                    S.done_items = i + 1;
+                }
+                asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // every store has landed before the CTA exits
+            }
+        }
+    }
+    __syncthreads();
+    if (tid == 0 && S.abort && P.stats) atomicMax(P.stats, S.abort);
+}
+
+// ------------------------------------------------------------------------------------------------ host side
+static void chanws_table_geometry(const GridGeom& g, K6Params& P) {
+    P.rlu = (k6PadU + g.W + 15 + 3) & ~3;     // pad + W + (tile - 1) more taps to the right, multiple of 4
+    P.rlv = (k6PadV + g.W + 7 + 1) & ~1;      // pad + W + (tile - 1), multiple of 2
+    P.n_tu = 4 * (g.O + 1) * P.rlu;
+    P.n_tv = 2 * (g.O + 1) * P.rlv;
+}
+
+bool chanws_supported(const Plan* p, int n_chan) {
+    if (n_chan < 1) return false;
+    if (p->geom.N > 2048 || p->geom.O > 30) return false;                    // 11 + 5 bits per axis in the packed index
+    K6Params P;
+    chanws_table_geometry(p->geom, P);
+    if ((P.n_tu + k6ZeroFloats) * 4 > 65535 || (P.n_tv + k6ZeroFloats) * 4 > 65535) return false;   // geo packs 16-bit byte offsets
+    return k6_layout(P.n_tu, P.n_tv).total <= 227 * 1024;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+            return nullptr;
+        fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+// grid_out [n_chan][4][N][N] complex64 seen as a 4-D tensor of 8-byte elements with dimension order (u, channel, v, pol)
+static bool make_grid_map(CUtensorMap* map, float* grid, int N, int n_chan, int box_v, int box_pol, bool swizzle) {
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) { set_error("cuTensorMapEncodeTiled is not available from the driver"); return false; }
+    const cuuint64_t dims[4] = {(cuuint64_t)N, (cuuint64_t)n_chan, (cuuint64_t)N, 4};
+    const cuuint64_t strides[3] = {(cuuint64_t)4 * N * N * 8, (cuuint64_t)N * 8, (cuuint64_t)N * N * 8};
+    const cuuint32_t box[4] = {16, 32, (cuuint32_t)box_v, (cuuint32_t)box_pol};
+    const cuuint32_t es[4] = {1, 1, 1, 1};
+    const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT64, 4, grid, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                           swizzle ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled failed (CUresult " + std::to_string((int)r) + ")"); return false; }
+    return true;
+}
+
+bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
+                   const int* dispatch, cudaStream_t st) {
+    if (!chanws_supported(p, n_chan)) { set_error("design CHANWS does not support this grid / kernel table size"); return false; }
+    Workspace& ws = p->ws;
+    K6Params P;
+    P.g = p->geom;
+    chanws_table_geometry(p->geom, P);
+    P.group = (const double4*)ws.d_group;
+    P.bucket_start = ws.d_bucket_count;
+    P.perm = ws.d_perm;
+    P.pre = ws.d_pre;
+    P.bb = (const ushort4*)ws.d_bb;
+    P.counter = ws.d_misc + 2;
+    P.stats = ws.d_misc + 4;
+    P.dispatch = dispatch;
+    P.dispatch_want = 1;
+    P.vis = vis;
+    P.weights = w;
+    P.table = p->d_table;
+    P.n_vis = (int)n_vis;
+    P.n_chan = n_chan;
+    P.n_groups = (n_chan + 31) / 32;
+    P.nb = (p->geom.N + kBucketCells - 1) / kBucketCells;
+    P.ntx = (p->geom.N + k6TileX - 1) / k6TileX;
+    P.nty = (p->geom.N + k6TileY - 1) / k6TileY;
+    P.n_items = (long long)P.ntx * P.nty * P.n_groups;
+    if (P.n_items >= 0x7fffffffLL) { set_error("design CHANWS: too many work items"); return false; }
+    CUtensorMap map_out, map_zero;
+    if (!make_grid_map(&map_out, grid, p->geom.N, n_chan, 2, 4, true)) return false;
+    if (!make_grid_map(&map_zero, grid, p->geom.N, n_chan, 1, 1, false)) return false;
+
+    long long tasks = n_vis * (long long)P.n_groups;
+    long long iblocks = (tasks + 7) / 8;
+    if (iblocks > (long long)p->sm_count * 16) iblocks = (long long)p->sm_count * 16;
+    if (iblocks < 1) iblocks = 1;
+    chan_index_kernel<<<(unsigned)iblocks, 256, 0, st>>>(p->geom, (const double4*)ws.d_row_sorted, ws.d_scale, (int)n_vis, n_chan,
+                                                         P.n_groups, ws.d_pre, (ushort4*)ws.d_bb, dispatch, 1);
+    const size_t smem = k6_layout(P.n_tu, P.n_tv).total;
+    auto kern = w ? chanws_kernel<true> : chanws_kernel<false>;
+    if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "chanws smem attribute"))
+        return false;
+    long long blocks = p->sm_count;
+    if (blocks > P.n_items) blocks = P.n_items;
+    kern<<<(unsigned)blocks, k6Threads, smem, st>>>(P, map_out, map_zero);
+    p->last_launches += 2;
+    return cuda_ok(cudaGetLastError(), "chanws_kernel");
+}
+
+}  // namespace mwa

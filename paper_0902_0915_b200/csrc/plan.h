@@ -29,8 +29,12 @@ struct Workspace {
     int* d_tile_order = nullptr;     // [n_tiles] tile ids, heaviest first
     int* d_tile_weight = nullptr;    // [n_tiles]
     int* d_misc = nullptr;           // small counters
-    int* d_dispatch = nullptr;       // [1] design picked on the device for AUTO: 0 = gather (K3c), 1 = chan (K5)
+    int* d_dispatch = nullptr;       // [1] design picked on the device for AUTO: 0 = gather (K3c), 1 = chan (K6 / K5)
     int cap_tiles = 0;
+    // K6 (k_chanws.cu) pre-pass outputs
+    unsigned* d_pre = nullptr;       // [n_vis][ceil(n_chan / 32) * 32] packed exact indices, by row
+    void* d_bb = nullptr;            // [ceil(n_chan / 32)][n_vis] ushort4 bounding boxes, by sorted position
+    size_t cap_pre = 0;              // capacity in (row, padded channel) elements
     // host-buffer entry point staging
     void* d_stage = nullptr;
     size_t cap_stage = 0;
@@ -50,6 +54,7 @@ struct Plan {
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     bool ev_valid = false;
     int last_launches = 0;
+    bool last_chanws = false;        // AUTO: the channel-SIMD kernel enqueued by the last call was K6 (else K5)
 };
 
 void set_error(const std::string& msg);
@@ -67,6 +72,9 @@ bool probe_fp32(Plan* p, double* tflops_ffma, double* tflops_ffma2, cudaStream_t
 bool chan_supported(const Plan* p, int n_chan);
 bool launch_chan(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                  const int* dispatch, cudaStream_t st);
+bool chanws_supported(const Plan* p, int n_chan);
+bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
+                   const int* dispatch, cudaStream_t st);
 bool launch_smem(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                  cudaStream_t st);
 bool launch_romein(Plan* p, const double* uv, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
