@@ -272,9 +272,11 @@ int mwa_grid_plan_last_stats(mwa_grid_plan* plan, long long* out, int n) {
     Plan* p = reinterpret_cast<Plan*>(plan);
     if (!p->ws.d_misc) { set_error("no gridding call recorded"); return MWA_GRID_ERR_INVALID; }
     int v[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    long long t[24];
     if (!cuda_ok(cudaMemcpy(v, p->ws.d_misc + 4, sizeof(v), cudaMemcpyDeviceToHost), "read stats")) return MWA_GRID_ERR_CUDA;
-    const int k = n < 8 ? n : 8;
-    for (int i = 0; i < k; ++i) out[i] = v[i];
+    if (!cuda_ok(cudaMemcpy(t, p->ws.d_misc + 2048, sizeof(t), cudaMemcpyDeviceToHost), "read stats")) return MWA_GRID_ERR_CUDA;
+    const int k = n < 32 ? n : 32;
+    for (int i = 0; i < k; ++i) out[i] = i < 8 ? (long long)v[i] : t[i - 8];   // [8..31]: phase clocks of a -DK6_TIMING build, else 0
     return k;
 }
 

@@ -23,7 +23,7 @@
 //                         accumulators into a 128 B-swizzled stage and signal the store warp;
 //     warp 19  "store"    one cp.async.bulk.tensor store per (2 tile rows x 32 channels x 4 pol) box through a 4-D
 //                         tensor map of grid_out with dimension order (u, channel, v, pol); items nothing reaches
-//                         are zero-filled from a small zero buffer without involving any other warp.
+//                         are zero-filled by this warp from a small zero buffer, involving no other warp.
 //
 // No atomics on grid data, every cell of grid_out is written exactly once (R10), the hit order is a pure function
 // of the sorted rows, so the grid is bit-identical from run to run.  Registers: the kernel is compiled for 96 per
@@ -31,6 +31,8 @@
 // spills) and the four service warps drop to 64: 16 x 104 + 4 x 64 = 20 x 96, exactly the CTA's register pool (an
 // increase that the pool cannot serve blocks for ever).
 #include <cuda.h>
+
+#include <cstdint>
 
 #include "plan.h"
 
@@ -43,7 +45,9 @@ constexpr int k6Batch = 32;                           // hits per batch (one per
 constexpr int k6Stages = 2;                           // batches in flight (one per stager)
 constexpr int k6BatchRing = 8;                        // batch descriptors / queue segments between sweeper and stagers
 constexpr int k6ItemRing = 16;                        // item descriptors between sweeper and store warp
-constexpr int k6PadU = 16, k6PadV = 8;                // zero padding in front of a table row (floats)
+constexpr int k6Drift = 8;                            // largest spread (cells) of the stamp origins over the 32 channels of a fast hit
+constexpr int k6PadU = 15 + k6Drift + 1, k6PadV = 7 + k6Drift + 1;   // zero padding in front of a table row (floats)
+constexpr int k6Bias = 2048;                          // > any stamp origin (N <= 2048): keeps both halves of a raw offset word positive
 constexpr int k6ZeroFloats = 32;                      // all-zero block behind each table (target of a missing lane)
 constexpr int k6WoBytes = 4 * 32768;                  // write-out stage: 4 block rows x [pol 4][v 2][chan 32][128 B]
 constexpr int k6StageV = k6Batch * 1024, k6StageGeo = k6Batch * 128, k6StageW = k6Batch * 128;
@@ -70,6 +74,7 @@ struct K6Params {
     const float* vis;            // [n_vis][n_chan][8]
     const float* weights;        // [n_vis][n_chan] or null
     const float* table;          // [(O+1)][W]
+    float* grid;                 // [n_chan][4][N][N][2] (zero-fill of untouched items; everything else goes through the tensor map)
     int n_vis, n_chan, n_groups, nb;
     int ntx, nty;                // tiles per row / column
     int rlu, rlv, n_tu, n_tv;    // padded row lengths and sizes (floats) of the shifted table copies
@@ -81,6 +86,7 @@ struct K6Ctrl {
     unsigned long long wo_full[4], wo_empty[4];             // mbarriers: block row staged for the store / stage free
     int st_n[k6Stages];
     unsigned st_flags[k6Stages];
+    unsigned st_tile[k6Stages];                             // tile term of the batch's raw table-offset words
     unsigned st_mask[k6Stages][k6Batch];
     int q_row[k6BatchRing * k6Batch];
     unsigned q_mask[k6BatchRing * k6Batch];                 // bits 0..15 block mask, bit 16: slow staging path
@@ -91,7 +97,20 @@ struct K6Ctrl {
     volatile int pub_batches, pub_items, done_items;
     volatile int done_batches[k6Stages];
     volatile int abort;
+    int stat_hit_items, stat_max_hits;                      // sweeper's counters for mwa_grid_plan_last_stats
 };
+
+// Optional phase timing (build with MWA_EXTRA_NVCC=-DK6_TIMING): clock64 sums per role in stats64[], read back through
+// mwa_grid_plan_last_stats slots 8.. ; compiled out of the product build.
+#ifdef K6_TIMING
+#define K6_TIC(t) const long long t = clock64()
+#define K6_TOC(acc, t) acc += clock64() - (t)
+#define K6_ADD(slot, v) do { if (lane == 0 && P.stats) atomicAdd(reinterpret_cast<unsigned long long*>(P.stats + 2044) + (slot), (unsigned long long)(v)); } while (0)
+#else
+#define K6_TIC(t)
+#define K6_TOC(acc, t)
+#define K6_ADD(slot, v)
+#endif
 
 struct K6Layout { size_t wo, ring, zero, tu, tv, ctrl, total; };
 
@@ -163,19 +182,26 @@ __device__ __forceinline__ u64 k6_pack2(float a, float b) {
 __device__ __forceinline__ void k6_ffma2(u64& d, u64 a, u64 b) { asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(a), "l"(b)); }
 
 // ------------------------------------------------------------------------------------------------ pre-pass
-// One warp per (sorted row r, channel group g), lane = channel.  pre[row][c] = origin_u | ru << 11 | origin_v << 16
-// | rv << 27 (origin = i - h, the first cell of the stamp), k6Invalid for a dropped sample (R11) or a channel
-// beyond n_chan.  bb[g][r] = (min origin_u, max origin_u | any-dropped << 15, min origin_v, max origin_v) over the
-// valid lanes; a group with no valid lane gets min = 0x7fff, which no tile reaches.
+// One warp per (sorted row r, channel group g), lane = channel.  With origin = i - h (the first cell of the stamp):
+//   bb[g][r]   = (min origin_u, max origin_u | slow << 15, min origin_v, max origin_v) over the valid lanes; a group with
+//                no valid lane gets min = 0x7fff, which no tile reaches.
+//   pre[row][c], fast (row, group): the lane's table offsets with the tile term left out,
+//                lo16 = 4 (ru rlu + su (O1 rlu - 1) + k6PadU + k6Bias - origin_u), su = (k6PadU - origin_u) & 3, hi16 likewise
+//                for v; the consumer adds 4 (X0 - k6Bias) | 4 (Y0 - k6Bias) << 16 of its tile (tiles start at multiples of
+//                16 x 8, so the alignment shifts su, sv do not depend on the tile).
+//   pre[row][c], slow (row, group): origin_u | ru << 11 | origin_v << 16 | rv << 27, or k6Invalid for a dropped sample (R11)
+//                or a channel beyond n_chan; the stager converts these with explicit range checks.
+// slow = some valid channel's sample is dropped, the origins spread over more than k6Drift cells (the zero padding of
+// the table copies covers a tile + stamp + k6Drift, so a fast hit can never index outside it), or the group is ragged.
 __global__ void __launch_bounds__(256)
 chan_index_kernel(GridGeom g, const double4* __restrict__ row_sorted, const double* __restrict__ scale, int n_vis,
-                  int n_chan, int n_groups, unsigned* __restrict__ pre, ushort4* __restrict__ bb,
+                  int n_chan, int n_groups, int rlu, int rlv, unsigned* __restrict__ pre, ushort4* __restrict__ bb,
                   const int* __restrict__ dispatch, int dispatch_want) {
     if (dispatch != nullptr && *dispatch != dispatch_want) return;
     const int lane = threadIdx.x & 31;
     const long long warps = ((long long)gridDim.x * blockDim.x) >> 5;
     const long long tasks = (long long)n_vis * n_groups;
-    const int ncp = n_groups * 32;
+    const int ncp = n_groups * 32, O1 = g.O + 1;
     for (long long t = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; t < tasks; t += warps) {
         const int grp = (int)(t / n_vis), r = (int)(t - (long long)grp * n_vis);
         const double4 rec = row_sorted[r];
@@ -185,16 +211,26 @@ chan_index_kernel(GridGeom g, const double4* __restrict__ row_sorted, const doub
         SampleIndex s;
         const bool ok = sample_index(rec.x, rec.y, sc, g, s) && cvalid;
         const int ou = s.iu - g.h, ov = s.iv - g.h;
-        const unsigned word = ok ? ((unsigned)ou | ((unsigned)s.ru << 11) | ((unsigned)ov << 16) | ((unsigned)s.rv << 27)) : k6Invalid;
-        pre[(size_t)(int)rec.z * ncp + c] = word;
         const unsigned full = 0xffffffffu;
         const unsigned u_min = __reduce_min_sync(full, ok ? (unsigned)ou : 0x7fffu);
         const unsigned u_max = __reduce_max_sync(full, ok ? (unsigned)ou : 0u);
         const unsigned v_min = __reduce_min_sync(full, ok ? (unsigned)ov : 0x7fffu);
         const unsigned v_max = __reduce_max_sync(full, ok ? (unsigned)ov : 0u);
-        const unsigned bad = __ballot_sync(full, cvalid && !ok) != 0u ? 0x8000u : 0u;
+        const bool slow = __ballot_sync(full, cvalid && !ok) != 0u || u_max > u_min + k6Drift || v_max > v_min + k6Drift ||
+                          grp * 32 + 32 > n_chan;                      // a ragged last group is staged lane by lane as well
+        unsigned word = k6Invalid;
+        if (ok) {
+            if (slow) word = (unsigned)ou | ((unsigned)s.ru << 11) | ((unsigned)ov << 16) | ((unsigned)s.rv << 27);
+            else {
+                const int su = (k6PadU - ou) & 3, sv = (k6PadV - ov) & 1;
+                const int lo = s.ru * rlu + su * (O1 * rlu - 1) + k6PadU + k6Bias - ou;
+                const int hi = s.rv * rlv + sv * (O1 * rlv - 1) + k6PadV + k6Bias - ov;
+                word = (unsigned)(lo * 4) | ((unsigned)(hi * 4) << 16);
+            }
+        }
+        pre[(size_t)(int)rec.z * ncp + c] = word;
         if (lane == 0)
-            bb[(size_t)grp * n_vis + r] = make_ushort4((unsigned short)u_min, (unsigned short)(u_max | bad),
+            bb[(size_t)grp * n_vis + r] = make_ushort4((unsigned short)u_min, (unsigned short)(u_max | (slow ? 0x8000u : 0u)),
                                                         (unsigned short)v_min, (unsigned short)v_max);
     }
 }
@@ -240,7 +276,9 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
     for (int k = tid; k < (int)(sizeof(K6Ctrl) / 4); k += k6Threads) reinterpret_cast<int*>(&S)[k] = 0;
     __syncthreads();
     if (tid == 0) {
-        for (int s = 0; s < k6Stages; ++s) { mbar_init(smem_u32(&S.full[s]), 1); mbar_init(smem_u32(&S.empty[s]), k6Consumers); }
+        for (int s = 0; s < k6Stages; ++s) {
+            mbar_init(smem_u32(&S.full[s]), 33); mbar_init(smem_u32(&S.empty[s]), k6Consumers);   // 32 cp.async arrivals + 1
+        }
         for (int r = 0; r < 4; ++r) { mbar_init(smem_u32(&S.wo_full[r]), 4); mbar_init(smem_u32(&S.wo_empty[r]), 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -267,12 +305,18 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
 #pragma unroll
                 for (int p = 0; p < 4; ++p) acc[i][j][p] = 0ull;
         int n_written = 0;
+        long long t_full = 0, t_visit = 0, t_woe = 0, t_wo = 0, n_vis_cnt = 0, n_bat = 0;
+        (void)t_full; (void)t_visit; (void)t_woe; (void)t_wo; (void)n_vis_cnt; (void)n_bat;
         for (int k = 0;; ++k) {
             const int s = k & 1;
+            K6_TIC(c0);
             if (!mbar_wait(smem_u32(&S.full[s]), (unsigned)((k >> 1) & 1), abort_flag, K6_ERR_FULL)) break;
+            K6_TOC(t_full, c0);
+            K6_TIC(c1);
             const unsigned flags = S.st_flags[s];
             if (flags & k6FlagExit) break;
             unsigned m = __ballot_sync(full, (S.st_mask[s][lane] >> wbit) & 1u);
+            const unsigned tc = S.st_tile[s];                           // 4 (X0 - k6Bias) | 4 (Y0 - k6Bias) << 16: completes a raw offset word
             const unsigned zs_s = ring_s + (unsigned)s * k6StageBytes + 32u * lane;
             const unsigned geo_s = ring_s + (unsigned)s * k6StageBytes + k6StageV + 4u * lane;
             const unsigned wt_s = geo_s + k6StageGeo;
@@ -299,6 +343,9 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
         }                                                                                                                 \
     }
                 const int cnt = __popc(m);
+#ifdef K6_TIMING
+                n_vis_cnt += cnt;
+#endif
                 u64 az0, az1, az2, az3, bz0, bz1, bz2, bz3;
                 float au0, au1, au2, au3, av0, av1, aw = 1.0f, bu0, bu1, bu2, bu3, bv0, bv1, bw = 1.0f;
                 const int h0 = K6_NEXT(m, 0);
@@ -309,17 +356,20 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                     unsigned g0;
                     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g0) : "r"(geo_s + 128u * h0));
                     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g1) : "r"(geo_s + 128u * h1));
+                    g0 += tc; g1 += tc;
                     K6_LOAD(h0, g0, az0, az1, az2, az3, au0, au1, au2, au3, av0, av1, aw)
                 }
 #pragma unroll 1
                 for (int v = 0; v < cnt; v += 2) {
                     K6_LOAD(h1, g1, bz0, bz1, bz2, bz3, bu0, bu1, bu2, bu3, bv0, bv1, bw)
                     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g2) : "r"(geo_s + 128u * h2));
+                    g2 += tc;
                     const int h3 = K6_NEXT(m, h2);
                     K6_FMA(az0, az1, az2, az3, au0, au1, au2, au3, av0, av1, aw)
                     if (v + 1 >= cnt) break;
                     K6_LOAD(h2, g2, az0, az1, az2, az3, au0, au1, au2, au3, av0, av1, aw)
                     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g1) : "r"(geo_s + 128u * h3));
+                    g1 += tc;
                     const int h4 = K6_NEXT(m, h3);
                     K6_FMA(bz0, bz1, bz2, bz3, bu0, bu1, bu2, bu3, bv0, bv1, bw)
                     h1 = h3;
@@ -331,9 +381,16 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(&S.empty[s]));          // this warp has read everything it needs of the batch
+            K6_TOC(t_visit, c1);
+#ifdef K6_TIMING
+            ++n_bat;
+#endif
             if (flags & k6FlagEnd) {
                 // ---- a5: accumulators -> swizzled stage of this block row; the store warp issues the TMA store
+                K6_TIC(c2);
                 if (!mbar_wait(smem_u32(&S.wo_empty[by]), (unsigned)((n_written & 1) ^ 1), abort_flag, K6_ERR_WOEMPTY)) break;
+                K6_TOC(t_woe, c2);
+                K6_TIC(c3);
 #pragma unroll
                 for (int pol = 0; pol < 4; ++pol)
 #pragma unroll
@@ -350,24 +407,34 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 __syncwarp();
                 if (lane == 0) mbar_arrive(smem_u32(&S.wo_full[by]));
                 ++n_written;
+                K6_TOC(t_wo, c3);
             }
         }
+        K6_ADD(0, t_full); K6_ADD(1, t_visit); K6_ADD(2, t_woe); K6_ADD(3, t_wo); K6_ADD(4, n_vis_cnt); K6_ADD(5, n_bat);
     } else {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
         const int role = warp - k6Consumers;
         if (role == 0) {
             // =========================================================================================== sweeper
+            // Everything here is latency: the chain item index -> bucket ranges -> bounding boxes goes through L2 three
+            // times.  So: items are claimed four at a time with the next claim in flight, the bucket ranges of item
+            // i + 1 are loaded before item i is processed, and the bounding boxes are loaded 128 candidates at a time.
             const unsigned lt_mask = (1u << lane) - 1u;
             int b_next = 0;              // global index of the first batch of the current item
             int n_pub = 0;               // batches published so far (= b_next + complete batches of the current item)
             int i_pub = 0;               // items published so far
-            int st_items = 0, st_hit_items = 0, st_max = 0;
             bool alive = true;
+            long long t_sw_ring = 0, t_sw_item = 0, t_sw_all = 0, t_sw_atomic = 0, t_sw_desc = 0, t_sw_loop = 0;
+            (void)t_sw_ring; (void)t_sw_item; (void)t_sw_all; (void)t_sw_atomic; (void)t_sw_desc; (void)t_sw_loop;
+            K6_TIC(sw0);
             // wait until batch b's queue segment and descriptor may be reused (batch b - ring has been staged)
             auto batch_slot_free = [&](int b) -> bool {
                 const int old = b - k6BatchRing;
                 if (old < 0) return true;
-                return spin_until_gt(&S.done_batches[old & 1], old >> 1, abort_flag, K6_ERR_RING);
+                K6_TIC(r0);
+                const bool okr = spin_until_gt(&S.done_batches[old & 1], old >> 1, abort_flag, K6_ERR_RING);
+                K6_TOC(t_sw_ring, r0);
+                return okr;
             };
             auto publish_batches = [&](int upto, int n_last, unsigned flags_last, int x0, int y0, int grp) {
                 // publishes batches [n_pub, upto]; all but the last are full and carry no flag
@@ -385,7 +452,9 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 n_pub = upto + 1;
             };
             auto publish_item = [&](int x0, int y0, int grp, int kind) -> bool {
+                K6_TIC(r1);
                 if (!spin_until_gt(&S.done_items, i_pub - k6ItemRing, abort_flag, K6_ERR_ITEM)) return false;
+                K6_TOC(t_sw_item, r1);
                 if (lane == 0) {
                     const int q = i_pub % k6ItemRing;
                     S.it_x0[q] = x0; S.it_y0[q] = y0; S.it_g[q] = grp; S.it_kind[q] = kind;
@@ -396,38 +465,74 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 ++i_pub;
                 return true;
             };
-            while (alive) {
-                long long item = 0;
-                if (lane == 0) item = (long long)atomicAdd(P.counter, 1);
-                item = __shfl_sync(full, item, 0);
-                if (item >= P.n_items) break;
-                // item order: x fastest, then y, then channel group (neighbouring tiles of one group share visibility rows in L2)
-                const int tx = (int)(item % P.ntx);
-                const int ty = (int)((item / P.ntx) % P.nty);
-                const int grp = (int)(item / ((long long)P.ntx * P.nty));
-                const int X0 = tx * k6TileX, Y0 = ty * k6TileY;
-                // bucket window at the reference scale (conservative, K5's back-projection)
-                const double4 gi = P.group[grp];
-                int wx0 = 0, wx1 = P.nb - 1, wy0 = 0, wy1 = P.nb - 1;
-                if (gi.z == gi.z && gi.w == gi.w) {
+            int cur_grp = -1;
+            double g_il = 0.0, g_ih = 0.0;                                   // s_ref / s_lo, s_ref / s_hi of cur_grp
+            // item -> tile, group and bucket window at the reference scale (conservative, K5's back-projection).
+            // Item order: x fastest, then y, then channel group (neighbouring tiles of one group share rows in L2).
+            auto describe = [&](int item, int& X0, int& Y0, int& grp, int& wx0, int& wx1, int& wy0, int& wy1) {
+                const int tx = item % P.ntx;
+                const int ty = (item / P.ntx) % P.nty;
+                grp = item / (P.ntx * P.nty);
+                X0 = tx * k6TileX; Y0 = ty * k6TileY;
+                if (grp != cur_grp) { const double4 gi = P.group[grp]; g_il = gi.z; g_ih = gi.w; cur_grp = grp; }
+                wx0 = 0; wx1 = P.nb - 1; wy0 = 0; wy1 = P.nb - 1;
+                if (g_il == g_il && g_ih == g_ih) {
                     const double halfN = (double)(N / 2);
                     const double pad = (double)P.g.h + 1.25;
                     const double ax = (double)X0 - halfN - pad, bxx = (double)(X0 + k6TileX - 1) - halfN + pad;
                     const double ay = (double)Y0 - halfN - pad, byy = (double)(Y0 + k6TileY - 1) - halfN + pad;
                     const double ib = 1.0 / kBucketCells, top = (double)(P.nb - 1);
-                    wx0 = (int)fmin(fmax(floor((fmin(ax * gi.z, ax * gi.w) + halfN) * ib), 0.0), top);
-                    wx1 = (int)fmin(fmax(floor((fmax(bxx * gi.z, bxx * gi.w) + halfN) * ib), 0.0), top);
-                    wy0 = (int)fmin(fmax(floor((fmin(ay * gi.z, ay * gi.w) + halfN) * ib), 0.0), top);
-                    wy1 = (int)fmin(fmax(floor((fmax(byy * gi.z, byy * gi.w) + halfN) * ib), 0.0), top);
+                    wx0 = (int)fmin(fmax(floor((fmin(ax * g_il, ax * g_ih) + halfN) * ib), 0.0), top);
+                    wx1 = (int)fmin(fmax(floor((fmax(bxx * g_il, bxx * g_ih) + halfN) * ib), 0.0), top);
+                    wy0 = (int)fmin(fmax(floor((fmin(ay * g_il, ay * g_ih) + halfN) * ib), 0.0), top);
+                    wy1 = (int)fmin(fmax(floor((fmax(byy * g_il, byy * g_ih) + halfN) * ib), 0.0), top);
                 }
+            };
+            auto load_rows = [&](int rg, int wy1, int wx0, int wx1, int& k0, int& len) {      // lane = bucket row rg + lane
+                k0 = 0; len = 0;
+                if (rg + lane <= wy1) {
+                    k0 = __ldg(P.bucket_start + (rg + lane) * P.nb + wx0);
+                    len = __ldg(P.bucket_start + (rg + lane) * P.nb + wx1 + 1) - k0;
+                }
+            };
+            auto claim = [&]() -> int {                                                     // raw: valid in lane 0 only
+                return lane == 0 ? atomicAdd(P.counter, 4) : 0;
+            };
+            const int n_items = (int)P.n_items;
+            K6_TIC(r2);
+            int item = __shfl_sync(full, claim(), 0);
+            K6_TOC(t_sw_atomic, r2);
+            int raw_next = claim();
+            int sub = 0, k0 = 0, len = 0;
+            if (item < n_items) {
+                int X0, Y0, grp, wx0, wx1, wy0, wy1;
+                describe(item, X0, Y0, grp, wx0, wx1, wy0, wy1);
+                load_rows(wy0, wy1, wx0, wx1, k0, len);
+            }
+            while (alive && item < n_items && item >= 0) {
+                // ---- the next item and its bucket ranges (in flight while this item is processed)
+                int item_n;
+                if (sub == 3) {
+                    K6_TIC(r3);
+                    item_n = __shfl_sync(full, raw_next, 0);
+                    K6_TOC(t_sw_atomic, r3);
+                } else item_n = item + 1;
+                int k0n = 0, lenn = 0;
+                K6_TIC(d0);
+                if (item_n < n_items && item_n >= 0) {
+                    int X0n, Y0n, grpn, wx0n, wx1n, wy0n, wy1n;
+                    describe(item_n, X0n, Y0n, grpn, wx0n, wx1n, wy0n, wy1n);
+                    load_rows(wy0n, wy1n, wx0n, wx1n, k0n, lenn);
+                }
+                // ---- this item
+                int X0, Y0, grp, wx0, wx1, wy0, wy1;
+                describe(item, X0, Y0, grp, wx0, wx1, wy0, wy1);
+                K6_TOC(t_sw_desc, d0);
+                K6_TIC(d1);
                 int cnt = 0, opened = 0;
                 const ushort4* bbg = P.bb + (size_t)grp * P.n_vis;
                 for (int rg = wy0; rg <= wy1 && alive; rg += 32) {
-                    int k0 = 0, len = 0;
-                    if (rg + lane <= wy1) {
-                        k0 = __ldg(P.bucket_start + (rg + lane) * P.nb + wx0);
-                        len = __ldg(P.bucket_start + (rg + lane) * P.nb + wx1 + 1) - k0;
-                    }
+                    if (rg != wy0) load_rows(rg, wy1, wx0, wx1, k0, len);                   // windows of more than 32 bucket rows
                     int incl = len;
 #pragma unroll
                     for (int o = 1; o < 32; o <<= 1) {
@@ -436,63 +541,76 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                     }
                     const int total = __shfl_sync(full, incl, 31);
                     const int excl = incl - len;
-                    for (int cb = 0; cb < total && alive; cb += 32) {
-                        const int f = cb + lane;
-                        int lo = 0;                                          // smallest bucket row with incl > f
+                    for (int cb = 0; cb < total && alive; cb += 128) {
+                        uint2 bq[4];
+                        int rowq[4];
 #pragma unroll
-                        for (int st = 16; st > 0; st >>= 1) {
-                            const int t = __shfl_sync(full, incl, lo + st - 1);
-                            if (t <= f) lo += st;
+                        for (int u = 0; u < 4; ++u) {
+                            const int f = cb + 32 * u + lane;
+                            int lo = 0;                                      // smallest bucket row with incl > f
+#pragma unroll
+                            for (int st = 16; st > 0; st >>= 1) {
+                                const int t = __shfl_sync(full, incl, lo + st - 1);
+                                if (t <= f) lo += st;
+                            }
+                            lo = min(lo, 31);
+                            const int rk0 = __shfl_sync(full, k0, lo), rex = __shfl_sync(full, excl, lo);
+                            bq[u] = make_uint2(0x00007fffu, 0x00007fffu);    // empty box (min 0x7fff, max 0): reaches no tile
+                            rowq[u] = 0;
+                            if (f < total) {
+                                const int kpos = rk0 + (f - rex);
+                                bq[u] = __ldg(reinterpret_cast<const uint2*>(bbg + kpos));
+                                rowq[u] = __ldg(P.perm + kpos);
+                            }
                         }
-                        lo = min(lo, 31);
-                        const int rk0 = __shfl_sync(full, k0, lo), rex = __shfl_sync(full, excl, lo);
-                        bool hit = false;
-                        unsigned mask = 0u;
-                        int row = 0;
-                        if (f < total) {
-                            const int kpos = rk0 + (f - rex);
-                            const ushort4 b = bbg[kpos];
-                            row = __ldg(P.perm + kpos);
-                            const int u_min = b.x, u_max = b.y & 0x7fff, v_min = b.z, v_max = b.w;
-                            hit = u_min <= X0 + k6TileX - 1 && u_max + W - 1 >= X0 && v_min <= Y0 + k6TileY - 1 && v_max + W - 1 >= Y0;
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            if (cb + 32 * u >= total || !alive) break;
+                            const int u_min = (int)(bq[u].x & 0xffffu), u_max = (int)((bq[u].x >> 16) & 0x7fffu);
+                            const int v_min = (int)(bq[u].y & 0xffffu), v_max = (int)(bq[u].y >> 16);
+                            const bool hit = u_min <= X0 + k6TileX - 1 && u_max + W - 1 >= X0 && v_min <= Y0 + k6TileY - 1 && v_max + W - 1 >= Y0;
+                            unsigned mask = 0u;
                             if (hit) {
                                 const int bxl = max(0, (u_min - X0) >> 2), bxh = min(3, (u_max + W - 1 - X0) >> 2);
                                 const int byl = max(0, (v_min - Y0) >> 1), byh = min(3, (v_max + W - 1 - Y0) >> 1);
                                 const unsigned mu = (2u << bxh) - (1u << bxl);
                                 const unsigned mv = 0x1111u & ((1u << (4 * (byh + 1))) - (1u << (4 * byl)));
-                                mask = mu * mv | ((b.y & 0x8000u) ? 0x10000u : 0u);
+                                mask = mu * mv | ((bq[u].x & 0x80000000u) ? 0x10000u : 0u);
                             }
+                            const unsigned hm = __ballot_sync(full, hit);
+                            const int n_new = __popc(hm);
+                            if (n_new == 0) continue;
+                            const int need = (cnt + n_new - 1) / k6Batch + 1;    // batches of this item that must be open
+                            while (opened < need) {
+                                if (!batch_slot_free(b_next + opened)) { alive = false; break; }
+                                ++opened;
+                            }
+                            if (!alive) break;
+                            if (hit) {
+                                const int i = cnt + __popc(hm & lt_mask);
+                                const int slot = ((b_next + i / k6Batch) % k6BatchRing) * k6Batch + (i % k6Batch);
+                                S.q_row[slot] = rowq[u];
+                                S.q_mask[slot] = mask;
+                            }
+                            cnt += n_new;
+                            const int complete = b_next + (cnt - 1) / k6Batch - 1;    // last batch known to have a successor
+                            if (complete >= n_pub) publish_batches(complete, k6Batch, 0u, X0, Y0, grp);
                         }
-                        const unsigned hm = __ballot_sync(full, hit);
-                        const int n_new = __popc(hm);
-                        if (n_new == 0) continue;
-                        const int need = (cnt + n_new - 1) / k6Batch + 1;    // batches of this item that must be open
-                        while (opened < need) {
-                            if (!batch_slot_free(b_next + opened)) { alive = false; break; }
-                            ++opened;
-                        }
-                        if (!alive) break;
-                        if (hit) {
-                            const int i = cnt + __popc(hm & lt_mask);
-                            const int slot = ((b_next + i / k6Batch) % k6BatchRing) * k6Batch + (i % k6Batch);
-                            S.q_row[slot] = row;
-                            S.q_mask[slot] = mask;
-                        }
-                        cnt += n_new;
-                        const int complete = b_next + (cnt - 1) / k6Batch - 1;    // last batch known to have a successor
-                        if (complete >= n_pub) publish_batches(complete, k6Batch, 0u, X0, Y0, grp);
                     }
                 }
                 if (!alive) break;
+                K6_TOC(t_sw_loop, d1);
                 if (cnt > 0) {
                     const int last = b_next + (cnt - 1) / k6Batch;
                     publish_batches(last, cnt - ((cnt - 1) / k6Batch) * k6Batch, k6FlagEnd, X0, Y0, grp);
                     b_next = last + 1;
-                    ++st_hit_items;
+                    if (lane == 0) { S.stat_hit_items += 1; S.stat_max_hits = max(S.stat_max_hits, cnt); }   // in shared memory: no registers to spare here
                 }
-                ++st_items;
-                st_max = max(st_max, cnt);
-                if (!publish_item(X0, Y0, grp, cnt > 0 ? 1 : 0)) break;
+                if (!publish_item(X0, Y0, grp, cnt > 0 ? 1 : 0)) { alive = false; break; }
+                // ---- advance
+                if (sub == 3) { sub = 0; raw_next = claim(); } else ++sub;
+                item = item_n;
+                k0 = k0n; len = lenn;
             }
             // exit: one flagged batch per stager (consumers stop at the first one), one flagged item for the store warp
             if (!*abort_flag) {
@@ -511,21 +629,36 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 }
                 publish_item(0, 0, 0, 2);
             }
+            K6_TOC(t_sw_all, sw0);
+            K6_ADD(8, t_sw_all); K6_ADD(9, t_sw_ring); K6_ADD(10, t_sw_item); K6_ADD(11, t_sw_atomic); K6_ADD(22, t_sw_desc); K6_ADD(23, t_sw_loop);
             if (lane == 0 && P.stats) {
-                atomicAdd(P.stats + 1, st_items);
-                atomicAdd(P.stats + 2, st_hit_items);
+                atomicAdd(P.stats + 1, i_pub - 1);                           // the exit descriptor is not an item
+                atomicAdd(P.stats + 2, S.stat_hit_items);
                 atomicAdd(P.stats + 3, b_next);
-                atomicMax(P.stats + 4, st_max);
+                atomicMax(P.stats + 4, S.stat_max_hits);
             }
         } else if (role <= k6Stages) {
             // =========================================================================================== stagers
+            // lane = channel.  Every global read of a batch is a cp.async (LDGSTS) straight into the stage: per hit the
+            // raw table-offset words of the pre-pass (the consumer adds the tile term), the weights, and the 32 x 32 B of
+            // visibilities.  Nothing is computed here on the common path and the stager never waits for its copies: each
+            // lane arrives on the batch's mbarrier through cp.async.mbarrier.arrive.noinc, which fires when the lane's
+            // copies have landed.  Slow hits (dropped samples, wide spread, ragged last group; rare) are converted with
+            // explicit range checks and get zero-filled visibilities where a lane has nothing to contribute.
+            // (Per-lane bulk copies, cp.async.bulk = UBLKCP, were measured first: they are issued one lane at a time at
+            // ~60 ns each, 6.4 us per 32-hit batch.)
             const int s = role - 1;
             const unsigned st_base = ring_s + (unsigned)s * k6StageBytes;
+            const unsigned zs_a = st_base + 32u * lane, geo_a = st_base + k6StageV + 4u * lane, wt_a = geo_a + k6StageGeo;
             const unsigned full_bar = smem_u32(&S.full[s]), empty_bar = smem_u32(&S.empty[s]);
             const unsigned zero_geo = (unsigned)(P.n_tu * 4) | ((unsigned)(P.n_tv * 4) << 16);
             const int ncp = P.n_groups * 32;
+            long long t_st_pub = 0, t_st_empty = 0, t_st_work = 0, t_st_pre = 0, n_st = 0;
+            (void)t_st_pub; (void)t_st_empty; (void)t_st_work; (void)t_st_pre; (void)n_st;
             for (int b = s;; b += k6Stages) {
+                K6_TIC(q0);
                 if (!spin_until_gt(&S.pub_batches, b, abort_flag, K6_ERR_BATCH)) break;
+                K6_TOC(t_st_pub, q0);
                 __threadfence_block();
                 const int q = b % k6BatchRing;
                 const int n = S.b_n[q];
@@ -536,124 +669,156 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 if (lane < n) { row = S.q_row[q * k6Batch + lane]; mask = S.q_mask[q * k6Batch + lane]; }
                 __syncwarp();
                 const int use = b >> 1;                                      // this stage's use number
+                K6_TIC(q1);
                 if (!mbar_wait(empty_bar, (unsigned)((use & 1) ^ 1), abort_flag, K6_ERR_EMPTY)) break;
+                K6_TOC(t_st_empty, q1);
+                K6_TIC(q2);
                 const int c0 = grp * 32;
-                const int nch = min(32, P.n_chan - c0);                      // channels of the group (last group may be ragged)
-                const bool cvalid = lane < nch;
-                const bool slow = lane < n && (((mask >> 16) & 1u) || nch < 32);   // per hit: dropped lanes / ragged group -> no bulk copy
-                const bool fast = lane < n && !slow;
-                const unsigned n_fast = __popc(__ballot_sync(full, fast));
+                const bool cvalid = c0 + lane < P.n_chan;                    // the last group may be ragged
+                const int cc = cvalid ? c0 + lane : P.n_chan - 1;            // a valid address for every lane
+                const unsigned slow_m = __ballot_sync(full, lane < n && (((mask >> 16) & 1u) || c0 + 32 > P.n_chan));
+                const unsigned tile_c = (unsigned)(4 * (X0 - k6Bias)) + ((unsigned)(4 * (Y0 - k6Bias)) << 16);
                 S.st_mask[s][lane] = lane < n ? (mask & 0xffffu) : 0u;
-                if (lane == 0) { S.st_n[s] = n; S.st_flags[s] = flags; }
-                if (fast)                                                    // lane = hit: 32 channels x 32 B in one bulk copy
-                    bulk_load(st_base + 1024u * lane, P.vis + ((size_t)row * P.n_chan + c0) * 8, 1024u, full_bar);
-                // lane = channel: packed index -> table offsets, weight; slow-path visibilities
-                for (int h0 = 0; h0 < n; h0 += 8) {
-                    unsigned pw[8];
-                    float ww[8];
-                    int rr[8];
-#pragma unroll
-                    for (int u = 0; u < 8; ++u) {
-                        pw[u] = k6Invalid; ww[u] = 0.0f; rr[u] = 0;
-                        if (h0 + u < n) {
-                            rr[u] = __shfl_sync(full, row, h0 + u);
-                            pw[u] = __ldg(P.pre + (size_t)rr[u] * ncp + c0 + lane);
-                            if (HAS_W && cvalid) ww[u] = __ldg(P.weights + (size_t)rr[u] * P.n_chan + c0 + lane);
-                        }
-                    }
-#pragma unroll
-                    for (int u = 0; u < 8; ++u) {
-                        if (h0 + u < n) {
-                            unsigned geo = zero_geo;
-                            const unsigned w32 = pw[u];
-                            if (w32 != k6Invalid) {
-                                const int ou = (int)(w32 & 0x7ffu), ru = (int)((w32 >> 11) & 31u);
-                                const int ov = (int)((w32 >> 16) & 0x7ffu), rv = (int)(w32 >> 27);
-                                const int tu_ = k6PadU + X0 - ou, tv_ = k6PadV + Y0 - ov;
-                                const unsigned iu_ = (unsigned)(W - 1 + ou - X0), iv_ = (unsigned)(W - 1 + ov - Y0);
-                                if (iu_ < (unsigned)(k6TileX + W - 1) && iv_ < (unsigned)(k6TileY + W - 1)) {
-                                    const int su = tu_ & 3, sv = tv_ & 1;
-                                    const int offu = ru * P.rlu + tu_ + su * (O1 * P.rlu - 1);
-                                    const int offv = rv * P.rlv + tv_ + sv * (O1 * P.rlv - 1);
-                                    geo = (unsigned)(offu * 4) | ((unsigned)(offv * 4) << 16);
-                                }
-                            }
-                            const unsigned hh = (unsigned)(h0 + u);
-                            asm volatile("st.shared.u32 [%0], %1;" ::"r"(st_base + k6StageV + 128u * hh + 4u * lane), "r"(geo) : "memory");
-                            if (HAS_W)
-                                asm volatile("st.shared.f32 [%0], %1;" ::"r"(st_base + k6StageV + k6StageGeo + 128u * hh + 4u * lane), "f"(ww[u]) : "memory");
-                            if (__shfl_sync(full, (int)slow, h0 + u)) {
-                                float4 va = make_float4(0.f, 0.f, 0.f, 0.f), vb = va;      // a dropped sample contributes nothing (R11)
-                                if (cvalid && w32 != k6Invalid) {
-                                    const float4* src = reinterpret_cast<const float4*>(P.vis + ((size_t)rr[u] * P.n_chan + c0 + lane) * 8);
-                                    va = __ldg(src);
-                                    vb = __ldg(src + 1);
-                                }
-                                const unsigned dst = st_base + 1024u * hh + 32u * lane;
-                                asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(dst), "f"(va.x), "f"(va.y), "f"(va.z), "f"(va.w) : "memory");
-                                asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(dst + 16u), "f"(vb.x), "f"(vb.y), "f"(vb.z), "f"(vb.w) : "memory");
-                            }
-                        }
-                    }
+                if (lane == 0) { S.st_n[s] = n; S.st_flags[s] = flags; S.st_tile[s] = tile_c; }
+                for (int hh = 0; hh < n; ++hh) {
+                    const int r = __shfl_sync(full, row, hh);
+                    if (HAS_W)
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(wt_a + 128u * (unsigned)hh), "l"(P.weights + (size_t)r * P.n_chan + cc) : "memory");
+                    if ((slow_m >> hh) & 1u) continue;                       // uniform
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(geo_a + 128u * (unsigned)hh), "l"(P.pre + (size_t)r * ncp + c0 + lane) : "memory");
+                    const float* src = P.vis + ((size_t)r * P.n_chan + cc) * 8;
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(zs_a + 1024u * (unsigned)hh), "l"(src) : "memory");
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(zs_a + 1024u * (unsigned)hh + 16u), "l"(src + 4) : "memory");
                 }
+                for (unsigned sm_ = slow_m; sm_ != 0u; sm_ &= sm_ - 1u) {   // slow hits: packed (origin, table row) words, range-checked here
+                    const int hh = __ffs(sm_) - 1;
+                    const int r = __shfl_sync(full, row, hh);
+                    const unsigned w32 = __ldg(P.pre + (size_t)r * ncp + c0 + lane);
+                    unsigned geo = zero_geo;
+                    if (w32 != k6Invalid) {
+                        const int ou = (int)(w32 & 0x7ffu), ru = (int)((w32 >> 11) & 31u);
+                        const int ov = (int)((w32 >> 16) & 0x7ffu), rv = (int)(w32 >> 27);
+                        const int tu_ = k6PadU + X0 - ou, tv_ = k6PadV + Y0 - ov;
+                        const unsigned iu_ = (unsigned)(W - 1 + ou - X0), iv_ = (unsigned)(W - 1 + ov - Y0);
+                        if (iu_ < (unsigned)(k6TileX + W - 1) && iv_ < (unsigned)(k6TileY + W - 1)) {
+                            const int su = tu_ & 3, sv = tv_ & 1;
+                            const int offu = ru * P.rlu + tu_ + su * (O1 * P.rlu - 1);
+                            const int offv = rv * P.rlv + tv_ + sv * (O1 * P.rlv - 1);
+                            geo = (unsigned)(offu * 4) | ((unsigned)(offv * 4) << 16);
+                        }
+                    }
+                    geo -= tile_c;                                           // the consumer adds the tile term to every word
+                    asm volatile("st.shared.u32 [%0], %1;" ::"r"(geo_a + 128u * (unsigned)hh), "r"(geo) : "memory");
+                    const float* src = P.vis + ((size_t)r * P.n_chan + cc) * 8;
+                    const unsigned sz = (cvalid && w32 != k6Invalid) ? 16u : 0u;   // zero-filled where the lane has no sample (R11)
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(zs_a + 1024u * (unsigned)hh), "l"(src), "r"(sz) : "memory");
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(zs_a + 1024u * (unsigned)hh + 16u), "l"(src + 4), "r"(sz) : "memory");
+                }
+                // the batch is complete when all 32 lanes' copies have landed (noinc arrivals) and the meta data are written
+                asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(full_bar) : "memory");
                 __syncwarp();
                 if (lane == 0) {
-                    mbar_arrive_tx(full_bar, n_fast * 1024u);
+                    mbar_arrive(full_bar);
                     __threadfence_block();
                     S.done_batches[s] = use + 1;                             // queue segment and descriptor of batch b are free again
                 }
+                K6_TOC(t_st_work, q2);
+#ifdef K6_TIMING
+                ++n_st;
+#endif
                 if (flags & k6FlagExit) break;
             }
+            asm volatile("cp.async.wait_all;" ::: "memory");
+            K6_ADD(12, t_st_pub); K6_ADD(13, t_st_empty); K6_ADD(14, t_st_work); K6_ADD(15, n_st); K6_ADD(21, t_st_pre);
         } else {
             // =========================================================================================== store warp
-            if (lane == 0) {
-                const unsigned wo0 = smem_u32(base + L.wo), zero_s = smem_u32(base + L.zero);
-                int n_written = 0;
-                unsigned pending = 0u;                                       // block rows whose store has been issued but not released
-                auto release_all = [&]() {
-                    if (pending == 0u) return;
-                    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the TMA engine has read the stages
+            // lane 0 issues the tensor-map stores of the block rows in whatever order the consumers finish them, and the
+            // zero-fill stores of the items nothing reaches.
+            const unsigned wo0 = smem_u32(base + L.wo), zero_s = smem_u32(base + L.zero);
+            int n_written = 0;
+            unsigned pending = 0u;                                           // block rows whose store has been issued but not released (lane 0)
+            long long t_so_rel = 0, t_so_items = 0, t_so_full = 0, t_so_zero = 0, t_so_all = 0;
+            (void)t_so_rel; (void)t_so_items; (void)t_so_full; (void)t_so_zero; (void)t_so_all;
+            K6_TIC(so0);
+            auto release_all = [&]() {                                       // lane 0 only
+                if (pending == 0u) return;
+                K6_TIC(s0);
+                asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the TMA engine has read the stages
+                K6_TOC(t_so_rel, s0);
 #pragma unroll
-                    for (int r = 0; r < 4; ++r)
-                        if (pending & (1u << r)) mbar_arrive(smem_u32(&S.wo_empty[r]));
-                    pending = 0u;
-                };
-                for (int i = 0;; ++i) {
-                    if (S.pub_items <= i) {
-                        release_all();                                       // idle: let the consumers have their stage back
-                        if (!spin_until_gt(&S.pub_items, i, abort_flag, K6_ERR_ITEM)) break;
-                    }
-                    __threadfence_block();
-                    const int q = i % k6ItemRing;
-                    const int X0 = S.it_x0[q], Y0 = S.it_y0[q], c0 = S.it_g[q] * 32, kind = S.it_kind[q];
-                    if (kind == 2) break;
-                    if (kind == 0) {
-                        release_all();                                       // a run of empty items must not keep the consumers waiting
+                for (int r = 0; r < 4; ++r)
+                    if (pending & (1u << r)) mbar_arrive(smem_u32(&S.wo_empty[r]));
+                pending = 0u;
+            };
+            for (int i = 0;; ++i) {
+                int okw = 1;
+                if (lane == 0 && S.pub_items <= i) {
+                    release_all();                                           // idle: let the consumers have their stage back
+                    K6_TIC(s1);
+                    okw = spin_until_gt(&S.pub_items, i, abort_flag, K6_ERR_ITEM) ? 1 : 0;
+                    K6_TOC(t_so_items, s1);
+                }
+                okw = __shfl_sync(full, okw, 0);
+                if (!okw) break;
+                __threadfence_block();
+                const int q = i % k6ItemRing;
+                const int X0 = S.it_x0[q], Y0 = S.it_y0[q], c0 = S.it_g[q] * 32, kind = S.it_kind[q];
+                if (kind == 2) break;
+                if (kind == 0) {
+                    // one 4 KB box (16 cells x 32 channels) per tile row and pol from the zero buffer.  (Plain st.global
+                    // from this one warp was measured at 4 B / clock - latency-throttled; the TMA queue is deep.)
+                    K6_TIC(s2);
+                    if (lane == 0) {
                         for (int pol = 0; pol < 4; ++pol)
                             for (int v = 0; v < k6TileY; ++v)
                                 if (Y0 + v < N) tma_store4(&map_zero, zero_s, X0, c0, Y0 + v, pol);
                         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-                    } else {
-                        bool ok = true;
-                        for (int r = 0; r < 4 && ok; ++r) {
-                            const unsigned bar = smem_u32(&S.wo_full[r]);
-                            const unsigned par = (unsigned)(n_written & 1);
-                            if (!mbar_try(bar, par)) {
-                                release_all();
-                                ok = mbar_wait(bar, par, abort_flag, K6_ERR_WOFULL);
-                                if (!ok) break;
-                            }
-                            if (Y0 + 2 * r < N) tma_store4(&map_out, wo0 + 32768u * r, X0, c0, Y0 + 2 * r, 0);
-                            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-                            pending |= 1u << r;
-                        }
-                        if (!ok) break;
-                        ++n_written;
                     }
-                    S.done_items = i + 1;
+                    K6_TOC(t_so_zero, s2);
+                } else {
+                    int oks = 1;
+                    if (lane == 0) {
+                        unsigned remaining = 0xfu;
+                        const unsigned par = (unsigned)(n_written & 1);
+                        long long t0 = 0;
+                        bool timing = false;
+                        while (remaining) {
+                            bool progress = false;
+#pragma unroll
+                            for (int r = 0; r < 4; ++r) {
+                                if ((remaining >> r) & 1u) {
+                                    if (mbar_try(smem_u32(&S.wo_full[r]), par)) {
+                                        if (Y0 + 2 * r < N) tma_store4(&map_out, wo0 + 32768u * r, X0, c0, Y0 + 2 * r, 0);
+                                        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                                        pending |= 1u << r;
+                                        remaining &= ~(1u << r);
+                                        progress = true;
+                                    }
+                                }
+                            }
+                            if (!progress) {
+                                release_all();
+                                if (!timing) { t0 = clock64(); timing = true; }
+                                if (*abort_flag) { oks = 0; break; }
+                                if (clock64() - t0 > k6SpinLimit) { *abort_flag = K6_ERR_WOFULL; oks = 0; break; }
+                            }
+                        }
+#ifdef K6_TIMING
+                        if (timing) t_so_full += clock64() - t0;
+#endif
+                    }
+                    oks = __shfl_sync(full, oks, 0);
+                    if (!oks) break;
+                    ++n_written;
                 }
-                asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // every store has landed before the CTA exits
+                __syncwarp();
+                if (lane == 0) S.done_items = i + 1;
             }
+            if (lane == 0) {
+                asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // every store has landed before the CTA exits
+                K6_TOC(t_so_all, so0);
+            }
+            K6_ADD(16, t_so_all); K6_ADD(17, t_so_rel); K6_ADD(18, t_so_items); K6_ADD(19, t_so_full); K6_ADD(20, t_so_zero);
         }
     }
     __syncthreads();
@@ -662,8 +827,8 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
 
 // ------------------------------------------------------------------------------------------------ host side
 static void chanws_table_geometry(const GridGeom& g, K6Params& P) {
-    P.rlu = (k6PadU + g.W + 15 + 3) & ~3;     // pad + W + (tile - 1) more taps to the right, multiple of 4
-    P.rlv = (k6PadV + g.W + 7 + 1) & ~1;      // pad + W + (tile - 1), multiple of 2
+    P.rlu = (k6PadU + g.W + 15 + k6Drift + 3) & ~3;     // pad + W + (tile - 1) + drift more taps to the right, multiple of 4
+    P.rlv = (k6PadV + g.W + 7 + k6Drift + 1) & ~1;      // pad + W + (tile - 1) + drift, multiple of 2
     P.n_tu = 4 * (g.O + 1) * P.rlu;
     P.n_tv = 2 * (g.O + 1) * P.rlv;
 }
@@ -727,6 +892,7 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
     P.vis = vis;
     P.weights = w;
     P.table = p->d_table;
+    P.grid = grid;
     P.n_vis = (int)n_vis;
     P.n_chan = n_chan;
     P.n_groups = (n_chan + 31) / 32;
@@ -744,7 +910,7 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
     if (iblocks > (long long)p->sm_count * 16) iblocks = (long long)p->sm_count * 16;
     if (iblocks < 1) iblocks = 1;
     chan_index_kernel<<<(unsigned)iblocks, 256, 0, st>>>(p->geom, (const double4*)ws.d_row_sorted, ws.d_scale, (int)n_vis, n_chan,
-                                                         P.n_groups, ws.d_pre, (ushort4*)ws.d_bb, dispatch, 1);
+                                                         P.n_groups, P.rlu, P.rlv, ws.d_pre, (ushort4*)ws.d_bb, dispatch, 1);
     const size_t smem = k6_layout(P.n_tu, P.n_tv).total;
     auto kern = w ? chanws_kernel<true> : chanws_kernel<false>;
     if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "chanws smem attribute"))
