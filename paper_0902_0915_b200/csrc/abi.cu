@@ -87,6 +87,23 @@ static int ensure_workspace(Plan* p, long long n_vis, int n_chan) {
         ws.d_bb = bb;
         ws.cap_pre = n_pre;
     }
+    if (want_ws) {
+        // hit lists of K6: 64 entries of 8 B per item while that stays below 2 GiB, else fewer, else none
+        const long long items = chanws_items(p, n_chan);
+        int cap = 64;
+        while (cap >= 16 && items * cap * 8 > (2LL << 30)) cap >>= 1;
+        if (cap < 16) cap = 0;
+        if (items > ws.cap_items || cap > ws.list_cap) {
+            ws.cap_items = 0;
+            ws.list_cap = 0;
+            if (!ensure(ws.d_list_cnt, (size_t)items, "hit counts")) return MWA_GRID_ERR_NOMEM;
+            unsigned long long* l = (unsigned long long*)ws.d_lists;
+            if (!ensure(l, (size_t)items * cap, "hit lists")) { ws.d_lists = l; return MWA_GRID_ERR_NOMEM; }
+            ws.d_lists = l;
+            ws.cap_items = items;
+        }
+        ws.list_cap = cap;
+    }
     return MWA_GRID_OK;
 }
 
@@ -208,7 +225,7 @@ void mwa_grid_plan_destroy(mwa_grid_plan* plan) {
     Workspace& ws = p->ws;
     void* ptrs[] = {p->d_table, ws.d_scale, ws.d_group, ws.d_scale_ref, ws.d_bucket_count, ws.d_bucket_cursor, ws.d_perm, ws.d_perm_tmp,
                     ws.d_uv_sorted, ws.d_row_sorted, ws.d_tile_order, ws.d_tile_weight, ws.d_misc, ws.d_dispatch, ws.d_stage,
-                    ws.d_pre, ws.d_bb};
+                    ws.d_pre, ws.d_bb, ws.d_list_cnt, ws.d_lists};
     for (void* q : ptrs)
         if (q) cudaFree(q);
     for (auto& e : p->ev)

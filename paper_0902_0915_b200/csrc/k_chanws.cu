@@ -41,9 +41,10 @@ namespace mwa {
 constexpr int k6Consumers = 16;                       // consumer warps
 constexpr int k6Threads = (k6Consumers + 4) * 32;     // + sweeper, two stagers, store warp
 constexpr int k6TileX = 16, k6TileY = 8;
-constexpr int k6Batch = 32;                           // hits per batch (one per lane of a stager)
-constexpr int k6Stages = 2;                           // batches in flight (one per stager)
-constexpr int k6BatchRing = 8;                        // batch descriptors / queue segments between sweeper and stagers
+constexpr int k6Batch = 16;                           // hits per batch
+constexpr int k6Stages = 4;                           // batches in flight (two per stager)
+constexpr int k6Stagers = 2;                          // stager warps; batch b is staged by stager b % 2 into stage b % 4
+constexpr int k6BatchRing = 16;                       // batch descriptors / queue segments between sweeper and stagers
 constexpr int k6ItemRing = 16;                        // item descriptors between sweeper and store warp
 constexpr int k6Drift = 8;                            // largest spread (cells) of the stamp origins over the 32 channels of a fast hit
 constexpr int k6PadU = 15 + k6Drift + 1, k6PadV = 7 + k6Drift + 1;   // zero padding in front of a table row (floats)
@@ -67,6 +68,9 @@ struct K6Params {
     const int* perm;             // [n_vis] sorted position -> row
     const unsigned* pre;         // [n_vis][n_groups * 32] packed indices, by ROW
     const ushort4* bb;           // [n_groups][n_vis] bounding boxes, by SORTED POSITION
+    const int* list_cnt;         // [n_items] hits of every item (chan_list_kernel)
+    const uint2* lists;          // [n_items][list_cap] (row, mask) of the first list_cap hits of every item
+    int list_cap;                // 0 = no lists: the in-kernel sweeper sweeps every item
     int* counter;                // work counter
     int* stats;                  // [8] error, items, items with hits, batches, max hits of an item
     const int* dispatch;         // device-side design choice (AUTO); null = always run
@@ -95,7 +99,7 @@ struct K6Ctrl {
     int b_x0[k6BatchRing], b_y0[k6BatchRing], b_g[k6BatchRing];
     int it_x0[k6ItemRing], it_y0[k6ItemRing], it_g[k6ItemRing], it_kind[k6ItemRing];   // kind 0 zero-fill, 1 consumers, 2 exit
     volatile int pub_batches, pub_items, done_items;
-    volatile int done_batches[k6Stages];
+    volatile int done_batches[k6Stagers];
     volatile int abort;
     int stat_hit_items, stat_max_hits;                      // sweeper's counters for mwa_grid_plan_last_stats
 };
@@ -235,6 +239,125 @@ chan_index_kernel(GridGeom g, const double4* __restrict__ row_sorted, const doub
     }
 }
 
+// ------------------------------------------------------------------------------------------------ the sweep
+// Item = (16 x 8 tile at X0, Y0; channel group grp).  Its bucket window at the reference scale is K5's conservative
+// back-projection: il, ih = s_ref / s_lo, s_ref / s_hi of the group (NaN = scan every bucket).
+struct K6Item { int X0, Y0, grp, wx0, wx1, wy0, wy1; };
+
+__device__ __forceinline__ K6Item k6_describe(const K6Params& P, int X0, int Y0, int grp, double il, double ih) {
+    K6Item it;
+    it.X0 = X0; it.Y0 = Y0; it.grp = grp;
+    it.wx0 = 0; it.wx1 = P.nb - 1; it.wy0 = 0; it.wy1 = P.nb - 1;
+    if (il == il && ih == ih) {
+        const double halfN = (double)(P.g.N / 2);
+        const double pad = (double)P.g.h + 1.25;
+        const double ax = (double)X0 - halfN - pad, bxx = (double)(X0 + k6TileX - 1) - halfN + pad;
+        const double ay = (double)Y0 - halfN - pad, byy = (double)(Y0 + k6TileY - 1) - halfN + pad;
+        const double ib = 1.0 / kBucketCells, top = (double)(P.nb - 1);
+        it.wx0 = (int)fmin(fmax(floor((fmin(ax * il, ax * ih) + halfN) * ib), 0.0), top);
+        it.wx1 = (int)fmin(fmax(floor((fmax(bxx * il, bxx * ih) + halfN) * ib), 0.0), top);
+        it.wy0 = (int)fmin(fmax(floor((fmin(ay * il, ay * ih) + halfN) * ib), 0.0), top);
+        it.wy1 = (int)fmin(fmax(floor((fmax(byy * il, byy * ih) + halfN) * ib), 0.0), top);
+    }
+    return it;
+}
+
+// One warp walks the sorted rows of the item's bucket window (lane = candidate, 128 candidates' bounding boxes in
+// flight), tests them against the tile with integer compares and calls emit(hit, row, mask, ballot, popc(ballot)) for
+// every 32 candidates with at least one hit, in sorted-row order.  mask: bits 0..15 = the 4 x 4 blocks (4 x 2 cells)
+// the bounding box of the stamps touches, bit 16 = slow staging path.  Returns false as soon as emit does.
+template <typename Emit>
+__device__ __forceinline__ bool k6_sweep(const K6Params& P, const K6Item& it, int lane, Emit&& emit) {
+    const unsigned full = 0xffffffffu;
+    const int W = P.g.W, X0 = it.X0, Y0 = it.Y0;
+    const ushort4* bbg = P.bb + (size_t)it.grp * P.n_vis;
+    for (int rg = it.wy0; rg <= it.wy1; rg += 32) {
+        int k0 = 0, len = 0;
+        if (rg + lane <= it.wy1) {                                           // lane = bucket row rg + lane
+            k0 = __ldg(P.bucket_start + (rg + lane) * P.nb + it.wx0);
+            len = __ldg(P.bucket_start + (rg + lane) * P.nb + it.wx1 + 1) - k0;
+        }
+        int incl = len;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(full, incl, o);
+            if (lane >= o) incl += t;
+        }
+        const int total = __shfl_sync(full, incl, 31);
+        const int excl = incl - len;
+        for (int cb = 0; cb < total; cb += 128) {
+            uint2 bq[4];
+            int rowq[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int f = cb + 32 * u + lane;
+                int lo = 0;                                                  // smallest bucket row with incl > f
+#pragma unroll
+                for (int st = 16; st > 0; st >>= 1) {
+                    const int t = __shfl_sync(full, incl, lo + st - 1);
+                    if (t <= f) lo += st;
+                }
+                lo = min(lo, 31);
+                const int rk0 = __shfl_sync(full, k0, lo), rex = __shfl_sync(full, excl, lo);
+                bq[u] = make_uint2(0x00007fffu, 0x00007fffu);                // empty box (min 0x7fff, max 0): reaches no tile
+                rowq[u] = 0;
+                if (f < total) {
+                    const int kpos = rk0 + (f - rex);
+                    bq[u] = __ldg(reinterpret_cast<const uint2*>(bbg + kpos));
+                    rowq[u] = __ldg(P.perm + kpos);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (cb + 32 * u >= total) break;
+                const int u_min = (int)(bq[u].x & 0xffffu), u_max = (int)((bq[u].x >> 16) & 0x7fffu);
+                const int v_min = (int)(bq[u].y & 0xffffu), v_max = (int)(bq[u].y >> 16);
+                const bool hit = u_min <= X0 + k6TileX - 1 && u_max + W - 1 >= X0 && v_min <= Y0 + k6TileY - 1 && v_max + W - 1 >= Y0;
+                unsigned mask = 0u;
+                if (hit) {
+                    const int bxl = max(0, (u_min - X0) >> 2), bxh = min(3, (u_max + W - 1 - X0) >> 2);
+                    const int byl = max(0, (v_min - Y0) >> 1), byh = min(3, (v_max + W - 1 - Y0) >> 1);
+                    const unsigned mu = (2u << bxh) - (1u << bxl);
+                    const unsigned mv = 0x1111u & ((1u << (4 * (byh + 1))) - (1u << (4 * byl)));
+                    mask = mu * mv | ((bq[u].x & 0x80000000u) ? 0x10000u : 0u);
+                }
+                const unsigned hm = __ballot_sync(full, hit);
+                const int n_new = __popc(hm);
+                if (n_new == 0) continue;
+                if (!emit(hit, rowq[u], mask, hm, n_new)) return false;
+            }
+        }
+    }
+    return true;
+}
+
+// Second pre-pass: one warp per item sweeps it and writes its hit list (row, mask) into the item's slot of `cap`
+// entries, and the TOTAL number of hits into list_cnt (a count above `cap` tells chanws_kernel's sweeper to sweep the
+// item itself).  Runs with thousands of warps in flight, which hides the L2 round trips a single in-kernel sweeper
+// warp paid one after the other (4.6 us per item measured).
+__global__ void __launch_bounds__(256)
+chan_list_kernel(const __grid_constant__ K6Params P, int* __restrict__ list_cnt, uint2* __restrict__ lists, int cap) {
+    if (P.dispatch != nullptr && *P.dispatch != P.dispatch_want) return;
+    const int lane = threadIdx.x & 31;
+    const int warps = (gridDim.x * blockDim.x) >> 5;
+    const int n_items = (int)P.n_items;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    for (int item = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; item < n_items; item += warps) {
+        const int tx = item % P.ntx, ty = (item / P.ntx) % P.nty, grp = item / (P.ntx * P.nty);
+        const double4 gi = P.group[grp];
+        const K6Item it = k6_describe(P, tx * k6TileX, ty * k6TileY, grp, gi.z, gi.w);
+        uint2* dst = lists + (size_t)item * cap;
+        int cnt = 0;
+        k6_sweep(P, it, lane, [&](bool hit, int row, unsigned mask, unsigned hm, int n_new) -> bool {
+            const int i = cnt + __popc(hm & lt_mask);
+            if (hit && i < cap) dst[i] = make_uint2((unsigned)row, mask);
+            cnt += n_new;
+            return true;
+        });
+        if (lane == 0) list_cnt[item] = cnt;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ main kernel
 template <bool HAS_W>
 __global__ void __launch_bounds__(k6Threads, 1)
@@ -308,14 +431,14 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
         long long t_full = 0, t_visit = 0, t_woe = 0, t_wo = 0, n_vis_cnt = 0, n_bat = 0;
         (void)t_full; (void)t_visit; (void)t_woe; (void)t_wo; (void)n_vis_cnt; (void)n_bat;
         for (int k = 0;; ++k) {
-            const int s = k & 1;
+            const int s = k & (k6Stages - 1);
             K6_TIC(c0);
-            if (!mbar_wait(smem_u32(&S.full[s]), (unsigned)((k >> 1) & 1), abort_flag, K6_ERR_FULL)) break;
+            if (!mbar_wait(smem_u32(&S.full[s]), (unsigned)((k / k6Stages) & 1), abort_flag, K6_ERR_FULL)) break;
             K6_TOC(t_full, c0);
             K6_TIC(c1);
             const unsigned flags = S.st_flags[s];
             if (flags & k6FlagExit) break;
-            unsigned m = __ballot_sync(full, (S.st_mask[s][lane] >> wbit) & 1u);
+            unsigned m = __ballot_sync(full, lane < k6Batch && ((S.st_mask[s][lane] >> wbit) & 1u));
             const unsigned tc = S.st_tile[s];                           // 4 (X0 - k6Bias) | 4 (Y0 - k6Bias) << 16: completes a raw offset word
             const unsigned zs_s = ring_s + (unsigned)s * k6StageBytes + 32u * lane;
             const unsigned geo_s = ring_s + (unsigned)s * k6StageBytes + k6StageV + 4u * lane;
@@ -416,10 +539,9 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
         const int role = warp - k6Consumers;
         if (role == 0) {
             // =========================================================================================== sweeper
-            // Everything here is latency: the chain item index -> bucket ranges -> bounding boxes goes through L2 three
-            // times.  So: items are claimed four at a time with the next claim in flight, the bucket ranges of item
-            // i + 1 are loaded before item i is processed, and the bounding boxes are loaded 128 candidates at a time.
-            const unsigned lt_mask = (1u << lane) - 1u;
+            // Streams the per-item hit lists of chan_list_kernel into the queue: nothing here waits on global memory,
+            // because items are claimed four at a time with the next claim, its hit counts and the next item's list
+            // entries already in flight.  An item whose list overflowed its slot (dense tiles) is swept here instead.
             int b_next = 0;              // global index of the first batch of the current item
             int n_pub = 0;               // batches published so far (= b_next + complete batches of the current item)
             int i_pub = 0;               // items published so far
@@ -432,7 +554,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 const int old = b - k6BatchRing;
                 if (old < 0) return true;
                 K6_TIC(r0);
-                const bool okr = spin_until_gt(&S.done_batches[old & 1], old >> 1, abort_flag, K6_ERR_RING);
+                const bool okr = spin_until_gt(&S.done_batches[old % k6Stagers], old / k6Stagers, abort_flag, K6_ERR_RING);
                 K6_TOC(t_sw_ring, r0);
                 return okr;
             };
@@ -465,141 +587,88 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 ++i_pub;
                 return true;
             };
-            int cur_grp = -1;
-            double g_il = 0.0, g_ih = 0.0;                                   // s_ref / s_lo, s_ref / s_hi of cur_grp
-            // item -> tile, group and bucket window at the reference scale (conservative, K5's back-projection).
-            // Item order: x fastest, then y, then channel group (neighbouring tiles of one group share rows in L2).
-            auto describe = [&](int item, int& X0, int& Y0, int& grp, int& wx0, int& wx1, int& wy0, int& wy1) {
-                const int tx = item % P.ntx;
-                const int ty = (item / P.ntx) % P.nty;
-                grp = item / (P.ntx * P.nty);
-                X0 = tx * k6TileX; Y0 = ty * k6TileY;
-                if (grp != cur_grp) { const double4 gi = P.group[grp]; g_il = gi.z; g_ih = gi.w; cur_grp = grp; }
-                wx0 = 0; wx1 = P.nb - 1; wy0 = 0; wy1 = P.nb - 1;
-                if (g_il == g_il && g_ih == g_ih) {
-                    const double halfN = (double)(N / 2);
-                    const double pad = (double)P.g.h + 1.25;
-                    const double ax = (double)X0 - halfN - pad, bxx = (double)(X0 + k6TileX - 1) - halfN + pad;
-                    const double ay = (double)Y0 - halfN - pad, byy = (double)(Y0 + k6TileY - 1) - halfN + pad;
-                    const double ib = 1.0 / kBucketCells, top = (double)(P.nb - 1);
-                    wx0 = (int)fmin(fmax(floor((fmin(ax * g_il, ax * g_ih) + halfN) * ib), 0.0), top);
-                    wx1 = (int)fmin(fmax(floor((fmax(bxx * g_il, bxx * g_ih) + halfN) * ib), 0.0), top);
-                    wy0 = (int)fmin(fmax(floor((fmin(ay * g_il, ay * g_ih) + halfN) * ib), 0.0), top);
-                    wy1 = (int)fmin(fmax(floor((fmax(byy * g_il, byy * g_ih) + halfN) * ib), 0.0), top);
+            const int n_items = (int)P.n_items, C = P.list_cap;
+            auto claim = [&]() -> int { return lane == 0 ? atomicAdd(P.counter, 4) : 0; };      // raw: valid in lane 0 only
+            auto load_counts = [&](int base) -> int {                                           // lane k < 4: hit count of item base + k
+                int c = 0;
+                if (lane < 4 && base + lane < n_items && base >= 0) c = C > 0 ? __ldg(P.list_cnt + base + lane) : 1 << 30;
+                return c;
+            };
+            auto load_entries = [&](int it, int c, uint2& ea, uint2& eb) {                      // list entries lane and lane + 32
+                ea = make_uint2(0u, 0u); eb = ea;
+                if (c > 0 && c <= C) {
+                    const uint2* src = P.lists + (size_t)it * C;
+                    if (lane < c) ea = __ldg(src + lane);
+                    if (lane + 32 < c) eb = __ldg(src + lane + 32);
                 }
             };
-            auto load_rows = [&](int rg, int wy1, int wx0, int wx1, int& k0, int& len) {      // lane = bucket row rg + lane
-                k0 = 0; len = 0;
-                if (rg + lane <= wy1) {
-                    k0 = __ldg(P.bucket_start + (rg + lane) * P.nb + wx0);
-                    len = __ldg(P.bucket_start + (rg + lane) * P.nb + wx1 + 1) - k0;
-                }
-            };
-            auto claim = [&]() -> int {                                                     // raw: valid in lane 0 only
-                return lane == 0 ? atomicAdd(P.counter, 4) : 0;
-            };
-            const int n_items = (int)P.n_items;
             K6_TIC(r2);
             int item = __shfl_sync(full, claim(), 0);
             K6_TOC(t_sw_atomic, r2);
+            int cnt4 = load_counts(item), cnt4_n = 0, base_n = 0;
             int raw_next = claim();
-            int sub = 0, k0 = 0, len = 0;
-            if (item < n_items) {
-                int X0, Y0, grp, wx0, wx1, wy0, wy1;
-                describe(item, X0, Y0, grp, wx0, wx1, wy0, wy1);
-                load_rows(wy0, wy1, wx0, wx1, k0, len);
-            }
+            int sub = 0;
+            uint2 ea, eb;
+            load_entries(item, __shfl_sync(full, cnt4, 0), ea, eb);
             while (alive && item < n_items && item >= 0) {
-                // ---- the next item and its bucket ranges (in flight while this item is processed)
-                int item_n;
-                if (sub == 3) {
+                // ---- look ahead: the next claim's counts (one item after the claim was issued), the next item's entries
+                if (sub == 1) {
                     K6_TIC(r3);
-                    item_n = __shfl_sync(full, raw_next, 0);
+                    base_n = __shfl_sync(full, raw_next, 0);
                     K6_TOC(t_sw_atomic, r3);
-                } else item_n = item + 1;
-                int k0n = 0, lenn = 0;
-                K6_TIC(d0);
-                if (item_n < n_items && item_n >= 0) {
-                    int X0n, Y0n, grpn, wx0n, wx1n, wy0n, wy1n;
-                    describe(item_n, X0n, Y0n, grpn, wx0n, wx1n, wy0n, wy1n);
-                    load_rows(wy0n, wy1n, wx0n, wx1n, k0n, lenn);
+                    cnt4_n = load_counts(base_n);
                 }
+                const int c = __shfl_sync(full, cnt4, sub);
+                const int item_n = sub == 3 ? base_n : item + 1;
+                const int c_n = (item_n < n_items && item_n >= 0) ? (sub == 3 ? __shfl_sync(full, cnt4_n, 0) : __shfl_sync(full, cnt4, sub + 1)) : 0;
+                uint2 ea_n, eb_n;
+                load_entries(item_n, c_n, ea_n, eb_n);
                 // ---- this item
-                int X0, Y0, grp, wx0, wx1, wy0, wy1;
-                describe(item, X0, Y0, grp, wx0, wx1, wy0, wy1);
-                K6_TOC(t_sw_desc, d0);
-                K6_TIC(d1);
-                int cnt = 0, opened = 0;
-                const ushort4* bbg = P.bb + (size_t)grp * P.n_vis;
-                for (int rg = wy0; rg <= wy1 && alive; rg += 32) {
-                    if (rg != wy0) load_rows(rg, wy1, wx0, wx1, k0, len);                   // windows of more than 32 bucket rows
-                    int incl = len;
-#pragma unroll
-                    for (int o = 1; o < 32; o <<= 1) {
-                        const int t = __shfl_up_sync(full, incl, o);
-                        if (lane >= o) incl += t;
+                const int tx = item % P.ntx, ty = (item / P.ntx) % P.nty, grp = item / (P.ntx * P.nty);
+                const int X0 = tx * k6TileX, Y0 = ty * k6TileY;
+                int cnt = 0;
+                if (c > 0 && c <= C) {
+                    // list path: <= 4 batches; open them all, write the queue, publish
+                    const int nbat = (c + k6Batch - 1) / k6Batch;
+                    for (int j = 0; j < nbat && alive; ++j) alive = batch_slot_free(b_next + j);
+                    if (!alive) break;
+                    if (lane < c) {
+                        const int slot = ((b_next + lane / k6Batch) % k6BatchRing) * k6Batch + (lane % k6Batch);
+                        S.q_row[slot] = (int)ea.x; S.q_mask[slot] = ea.y;
                     }
-                    const int total = __shfl_sync(full, incl, 31);
-                    const int excl = incl - len;
-                    for (int cb = 0; cb < total && alive; cb += 128) {
-                        uint2 bq[4];
-                        int rowq[4];
-#pragma unroll
-                        for (int u = 0; u < 4; ++u) {
-                            const int f = cb + 32 * u + lane;
-                            int lo = 0;                                      // smallest bucket row with incl > f
-#pragma unroll
-                            for (int st = 16; st > 0; st >>= 1) {
-                                const int t = __shfl_sync(full, incl, lo + st - 1);
-                                if (t <= f) lo += st;
-                            }
-                            lo = min(lo, 31);
-                            const int rk0 = __shfl_sync(full, k0, lo), rex = __shfl_sync(full, excl, lo);
-                            bq[u] = make_uint2(0x00007fffu, 0x00007fffu);    // empty box (min 0x7fff, max 0): reaches no tile
-                            rowq[u] = 0;
-                            if (f < total) {
-                                const int kpos = rk0 + (f - rex);
-                                bq[u] = __ldg(reinterpret_cast<const uint2*>(bbg + kpos));
-                                rowq[u] = __ldg(P.perm + kpos);
-                            }
-                        }
-#pragma unroll
-                        for (int u = 0; u < 4; ++u) {
-                            if (cb + 32 * u >= total || !alive) break;
-                            const int u_min = (int)(bq[u].x & 0xffffu), u_max = (int)((bq[u].x >> 16) & 0x7fffu);
-                            const int v_min = (int)(bq[u].y & 0xffffu), v_max = (int)(bq[u].y >> 16);
-                            const bool hit = u_min <= X0 + k6TileX - 1 && u_max + W - 1 >= X0 && v_min <= Y0 + k6TileY - 1 && v_max + W - 1 >= Y0;
-                            unsigned mask = 0u;
-                            if (hit) {
-                                const int bxl = max(0, (u_min - X0) >> 2), bxh = min(3, (u_max + W - 1 - X0) >> 2);
-                                const int byl = max(0, (v_min - Y0) >> 1), byh = min(3, (v_max + W - 1 - Y0) >> 1);
-                                const unsigned mu = (2u << bxh) - (1u << bxl);
-                                const unsigned mv = 0x1111u & ((1u << (4 * (byh + 1))) - (1u << (4 * byl)));
-                                mask = mu * mv | ((bq[u].x & 0x80000000u) ? 0x10000u : 0u);
-                            }
-                            const unsigned hm = __ballot_sync(full, hit);
-                            const int n_new = __popc(hm);
-                            if (n_new == 0) continue;
-                            const int need = (cnt + n_new - 1) / k6Batch + 1;    // batches of this item that must be open
-                            while (opened < need) {
-                                if (!batch_slot_free(b_next + opened)) { alive = false; break; }
-                                ++opened;
-                            }
-                            if (!alive) break;
-                            if (hit) {
-                                const int i = cnt + __popc(hm & lt_mask);
-                                const int slot = ((b_next + i / k6Batch) % k6BatchRing) * k6Batch + (i % k6Batch);
-                                S.q_row[slot] = rowq[u];
-                                S.q_mask[slot] = mask;
-                            }
-                            cnt += n_new;
-                            const int complete = b_next + (cnt - 1) / k6Batch - 1;    // last batch known to have a successor
-                            if (complete >= n_pub) publish_batches(complete, k6Batch, 0u, X0, Y0, grp);
-                        }
+                    if (lane + 32 < c) {
+                        const int i = lane + 32;
+                        const int slot = ((b_next + i / k6Batch) % k6BatchRing) * k6Batch + (i % k6Batch);
+                        S.q_row[slot] = (int)eb.x; S.q_mask[slot] = eb.y;
                     }
+                    cnt = c;
+                } else if (c > C) {
+                    // fallback: the in-kernel sweep (dense tiles; also everything when the lists are disabled)
+                    K6_TIC(d1);
+                    const double4 gi = P.group[grp];
+                    const K6Item it = k6_describe(P, X0, Y0, grp, gi.z, gi.w);
+                    int opened = 0;
+                    const unsigned lt_mask = (1u << lane) - 1u;
+                    alive = k6_sweep(P, it, lane, [&](bool hit, int row, unsigned mask, unsigned hm, int n_new) -> bool {
+                        const int need = (cnt + n_new - 1) / k6Batch + 1;    // batches of this item that must be open
+                        while (opened < need) {
+                            if (!batch_slot_free(b_next + opened)) return false;
+                            ++opened;
+                        }
+                        if (hit) {
+                            const int i = cnt + __popc(hm & lt_mask);
+                            const int slot = ((b_next + i / k6Batch) % k6BatchRing) * k6Batch + (i % k6Batch);
+                            S.q_row[slot] = row;
+                            S.q_mask[slot] = mask;
+                        }
+                        cnt += n_new;
+                        const int complete = b_next + (cnt - 1) / k6Batch - 1;    // last batch known to have a successor
+                        if (complete >= n_pub) publish_batches(complete, k6Batch, 0u, X0, Y0, grp);
+                        return true;
+                    });
+                    K6_TOC(t_sw_loop, d1);
+                    if (!alive) break;
                 }
-                if (!alive) break;
-                K6_TOC(t_sw_loop, d1);
                 if (cnt > 0) {
                     const int last = b_next + (cnt - 1) / k6Batch;
                     publish_batches(last, cnt - ((cnt - 1) / k6Batch) * k6Batch, k6FlagEnd, X0, Y0, grp);
@@ -608,22 +677,22 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 }
                 if (!publish_item(X0, Y0, grp, cnt > 0 ? 1 : 0)) { alive = false; break; }
                 // ---- advance
-                if (sub == 3) { sub = 0; raw_next = claim(); } else ++sub;
+                if (sub == 3) { sub = 0; cnt4 = cnt4_n; raw_next = claim(); } else ++sub;
                 item = item_n;
-                k0 = k0n; len = lenn;
+                ea = ea_n; eb = eb_n;
             }
             // exit: one flagged batch per stager (consumers stop at the first one), one flagged item for the store warp
             if (!*abort_flag) {
                 bool ok = true;
-                for (int e = 0; e < k6Stages && ok; ++e) ok = batch_slot_free(b_next + e);
+                for (int e = 0; e < k6Stagers && ok; ++e) ok = batch_slot_free(b_next + e);
                 if (ok) {
                     if (lane == 0) {
-                        for (int e = 0; e < k6Stages; ++e) {
+                        for (int e = 0; e < k6Stagers; ++e) {
                             const int q = (b_next + e) % k6BatchRing;
                             S.b_n[q] = 0; S.b_flags[q] = k6FlagExit; S.b_x0[q] = 0; S.b_y0[q] = 0; S.b_g[q] = 0;
                         }
                         __threadfence_block();
-                        S.pub_batches = b_next + k6Stages;
+                        S.pub_batches = b_next + k6Stagers;
                     }
                     __syncwarp();
                 }
@@ -637,7 +706,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 atomicAdd(P.stats + 3, b_next);
                 atomicMax(P.stats + 4, S.stat_max_hits);
             }
-        } else if (role <= k6Stages) {
+        } else if (role <= k6Stagers) {
             // =========================================================================================== stagers
             // lane = channel.  Every global read of a batch is a cp.async (LDGSTS) straight into the stage: per hit the
             // raw table-offset words of the pre-pass (the consumer adds the tile term), the weights, and the 32 x 32 B of
@@ -647,15 +716,16 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
             // explicit range checks and get zero-filled visibilities where a lane has nothing to contribute.
             // (Per-lane bulk copies, cp.async.bulk = UBLKCP, were measured first: they are issued one lane at a time at
             // ~60 ns each, 6.4 us per 32-hit batch.)
-            const int s = role - 1;
-            const unsigned st_base = ring_s + (unsigned)s * k6StageBytes;
-            const unsigned zs_a = st_base + 32u * lane, geo_a = st_base + k6StageV + 4u * lane, wt_a = geo_a + k6StageGeo;
-            const unsigned full_bar = smem_u32(&S.full[s]), empty_bar = smem_u32(&S.empty[s]);
+            const int sg = role - 1;                                        // this stager stages batches b = sg, sg + 2, ...
             const unsigned zero_geo = (unsigned)(P.n_tu * 4) | ((unsigned)(P.n_tv * 4) << 16);
             const int ncp = P.n_groups * 32;
             long long t_st_pub = 0, t_st_empty = 0, t_st_work = 0, t_st_pre = 0, n_st = 0;
             (void)t_st_pub; (void)t_st_empty; (void)t_st_work; (void)t_st_pre; (void)n_st;
-            for (int b = s;; b += k6Stages) {
+            for (int b = sg;; b += k6Stagers) {
+                const int s = b & (k6Stages - 1);
+                const unsigned st_base = ring_s + (unsigned)s * k6StageBytes;
+                const unsigned zs_a = st_base + 32u * lane, geo_a = st_base + k6StageV + 4u * lane, wt_a = geo_a + k6StageGeo;
+                const unsigned full_bar = smem_u32(&S.full[s]), empty_bar = smem_u32(&S.empty[s]);
                 K6_TIC(q0);
                 if (!spin_until_gt(&S.pub_batches, b, abort_flag, K6_ERR_BATCH)) break;
                 K6_TOC(t_st_pub, q0);
@@ -668,7 +738,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 unsigned mask = 0u;
                 if (lane < n) { row = S.q_row[q * k6Batch + lane]; mask = S.q_mask[q * k6Batch + lane]; }
                 __syncwarp();
-                const int use = b >> 1;                                      // this stage's use number
+                const int use = b / k6Stages;                                // this stage's use number
                 K6_TIC(q1);
                 if (!mbar_wait(empty_bar, (unsigned)((use & 1) ^ 1), abort_flag, K6_ERR_EMPTY)) break;
                 K6_TOC(t_st_empty, q1);
@@ -678,7 +748,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 const int cc = cvalid ? c0 + lane : P.n_chan - 1;            // a valid address for every lane
                 const unsigned slow_m = __ballot_sync(full, lane < n && (((mask >> 16) & 1u) || c0 + 32 > P.n_chan));
                 const unsigned tile_c = (unsigned)(4 * (X0 - k6Bias)) + ((unsigned)(4 * (Y0 - k6Bias)) << 16);
-                S.st_mask[s][lane] = lane < n ? (mask & 0xffffu) : 0u;
+                if (lane < k6Batch) S.st_mask[s][lane] = lane < n ? (mask & 0xffffu) : 0u;
                 if (lane == 0) { S.st_n[s] = n; S.st_flags[s] = flags; S.st_tile[s] = tile_c; }
                 for (int hh = 0; hh < n; ++hh) {
                     const int r = __shfl_sync(full, row, hh);
@@ -720,7 +790,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 if (lane == 0) {
                     mbar_arrive(full_bar);
                     __threadfence_block();
-                    S.done_batches[s] = use + 1;                             // queue segment and descriptor of batch b are free again
+                    S.done_batches[sg] = b / k6Stagers + 1;                  // queue segment and descriptor of batch b are free again
                 }
                 K6_TOC(t_st_work, q2);
 #ifdef K6_TIMING
@@ -833,6 +903,11 @@ static void chanws_table_geometry(const GridGeom& g, K6Params& P) {
     P.n_tv = 2 * (g.O + 1) * P.rlv;
 }
 
+long long chanws_items(const Plan* p, int n_chan) {
+    const long long ntx = (p->geom.N + k6TileX - 1) / k6TileX, nty = (p->geom.N + k6TileY - 1) / k6TileY;
+    return ntx * nty * ((n_chan + 31) / 32);
+}
+
 bool chanws_supported(const Plan* p, int n_chan) {
     if (n_chan < 1) return false;
     if (p->geom.N > 2048 || p->geom.O > 30) return false;                    // 11 + 5 bits per axis in the packed index
@@ -885,6 +960,9 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
     P.perm = ws.d_perm;
     P.pre = ws.d_pre;
     P.bb = (const ushort4*)ws.d_bb;
+    P.list_cap = ws.list_cap;
+    P.list_cnt = ws.d_list_cnt;
+    P.lists = (const uint2*)ws.d_lists;
     P.counter = ws.d_misc + 2;
     P.stats = ws.d_misc + 4;
     P.dispatch = dispatch;
@@ -911,6 +989,12 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
     if (iblocks < 1) iblocks = 1;
     chan_index_kernel<<<(unsigned)iblocks, 256, 0, st>>>(p->geom, (const double4*)ws.d_row_sorted, ws.d_scale, (int)n_vis, n_chan,
                                                          P.n_groups, P.rlu, P.rlv, ws.d_pre, (ushort4*)ws.d_bb, dispatch, 1);
+    {
+        long long lblocks = (P.n_items + 7) / 8;
+        if (lblocks > (long long)p->sm_count * 32) lblocks = (long long)p->sm_count * 32;
+        if (P.list_cap > 0)
+            chan_list_kernel<<<(unsigned)lblocks, 256, 0, st>>>(P, ws.d_list_cnt, (uint2*)ws.d_lists, P.list_cap);
+    }
     const size_t smem = k6_layout(P.n_tu, P.n_tv).total;
     auto kern = w ? chanws_kernel<true> : chanws_kernel<false>;
     if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "chanws smem attribute"))
@@ -918,7 +1002,7 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
     long long blocks = p->sm_count;
     if (blocks > P.n_items) blocks = P.n_items;
     kern<<<(unsigned)blocks, k6Threads, smem, st>>>(P, map_out, map_zero);
-    p->last_launches += 2;
+    p->last_launches += P.list_cap > 0 ? 3 : 2;
     return cuda_ok(cudaGetLastError(), "chanws_kernel");
 }
 

@@ -35,6 +35,10 @@ struct Workspace {
     unsigned* d_pre = nullptr;       // [n_vis][ceil(n_chan / 32) * 32] packed exact indices, by row
     void* d_bb = nullptr;            // [ceil(n_chan / 32)][n_vis] ushort4 bounding boxes, by sorted position
     size_t cap_pre = 0;              // capacity in (row, padded channel) elements
+    int* d_list_cnt = nullptr;       // [n_items] hits per (16 x 8 tile, channel group) item
+    void* d_lists = nullptr;         // [n_items][list_cap] uint2 (row, mask)
+    long long cap_items = 0;         // items the two arrays above are sized for
+    int list_cap = 0;                // entries per item slot (0 = lists disabled for this problem size)
     // host-buffer entry point staging
     void* d_stage = nullptr;
     size_t cap_stage = 0;
@@ -73,6 +77,7 @@ bool chan_supported(const Plan* p, int n_chan);
 bool launch_chan(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                  const int* dispatch, cudaStream_t st);
 bool chanws_supported(const Plan* p, int n_chan);
+long long chanws_items(const Plan* p, int n_chan);
 bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                    const int* dispatch, cudaStream_t st);
 bool launch_smem(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
