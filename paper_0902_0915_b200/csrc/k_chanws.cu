@@ -41,11 +41,13 @@ namespace mwa {
 constexpr int k6Consumers = 16;                       // consumer warps
 constexpr int k6Threads = (k6Consumers + 4) * 32;     // + sweeper, two stagers, store warp
 constexpr int k6TileX = 16, k6TileY = 8;
-constexpr int k6Batch = 16;                           // hits per batch
-constexpr int k6Stages = 4;                           // batches in flight (two per stager)
+constexpr int k6Batch = 8;                            // hits per batch
+constexpr int k6Stages = 8;                           // batches in flight (two per stager)
 constexpr int k6Stagers = 2;                          // stager warps; batch b is staged by stager b % 2 into stage b % 4
-constexpr int k6BatchRing = 16;                       // batch descriptors / queue segments between sweeper and stagers
-constexpr int k6ItemRing = 16;                        // item descriptors between sweeper and store warp
+constexpr int k6BatchRing = 32;                       // batch descriptors / queue segments between sweeper and stagers
+constexpr int k6ItemRing = 16;                        // consumer-item descriptors between sweeper and store warp
+constexpr int k6ZeroRing = 128;                       // zero-fill item descriptors (the store warp works them off at low priority)
+constexpr unsigned k6ExitItem = 0xffffffffu;
 constexpr int k6Drift = 8;                            // largest spread (cells) of the stamp origins over the 32 channels of a fast hit
 constexpr int k6PadU = 15 + k6Drift + 1, k6PadV = 7 + k6Drift + 1;   // zero padding in front of a table row (floats)
 constexpr int k6Bias = 2048;                          // > any stamp origin (N <= 2048): keeps both halves of a raw offset word positive
@@ -97,8 +99,9 @@ struct K6Ctrl {
     int b_n[k6BatchRing];
     unsigned b_flags[k6BatchRing];
     int b_x0[k6BatchRing], b_y0[k6BatchRing], b_g[k6BatchRing];
-    int it_x0[k6ItemRing], it_y0[k6ItemRing], it_g[k6ItemRing], it_kind[k6ItemRing];   // kind 0 zero-fill, 1 consumers, 2 exit
-    volatile int pub_batches, pub_items, done_items;
+    unsigned c_item[k6ItemRing];                            // consumer items in order: tx | ty << 10 | group << 20, k6ExitItem = exit
+    unsigned z_item[k6ZeroRing];                            // items nothing reaches (zero-fill), any order
+    volatile int pub_batches, pub_c, done_c, pub_z, done_z;
     volatile int done_batches[k6Stagers];
     volatile int abort;
     int stat_hit_items, stat_max_hits;                      // sweeper's counters for mwa_grid_plan_last_stats
@@ -126,7 +129,7 @@ __host__ __device__ inline K6Layout k6_layout(int n_tu, int n_tv) {
     L.tu = L.zero + k6ZeroBytes;
     L.tv = L.tu + (size_t)(n_tu + k6ZeroFloats) * 4;
     L.ctrl = (L.tv + (size_t)(n_tv + k6ZeroFloats) * 4 + 15) & ~size_t(15);
-    L.total = L.ctrl + sizeof(K6Ctrl) + 1024;               // + slack for the 1024 B alignment of the base
+    L.total = L.ctrl + sizeof(K6Ctrl);                      // the base must be 1024 B aligned (checked in the kernel)
     return L;
 }
 
@@ -364,8 +367,12 @@ __global__ void __launch_bounds__(k6Threads, 1)
 chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtensorMap map_out,
               const __grid_constant__ CUtensorMap map_zero) {
     if (P.dispatch != nullptr && *P.dispatch != P.dispatch_want) return;
-    extern __shared__ unsigned char smem_dyn[];
-    unsigned char* base = reinterpret_cast<unsigned char*>((reinterpret_cast<size_t>(smem_dyn) + 1023) & ~size_t(1023));
+    extern __shared__ __align__(1024) unsigned char smem_dyn[];
+    unsigned char* base = smem_dyn;
+    if ((smem_u32(base) & 1023u) != 0u) {                             // the swizzled TMA stage needs it; never seen, never silent
+        if (threadIdx.x == 0 && P.stats) atomicMax(P.stats, 100);
+        return;
+    }
     const K6Layout L = k6_layout(P.n_tu, P.n_tv);
     float* tu = reinterpret_cast<float*>(base + L.tu);
     float* tv = reinterpret_cast<float*>(base + L.tv);
@@ -573,18 +580,31 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 if (lane == 0) S.pub_batches = upto + 1;
                 n_pub = upto + 1;
             };
+            int z_pub = 0;               // zero-fill items published so far
+            // kind 0: zero-fill item (any order), 1: consumer item (in order), 2: exit marker behind the last consumer item
             auto publish_item = [&](int x0, int y0, int grp, int kind) -> bool {
+                const unsigned word = kind == 2 ? k6ExitItem : ((unsigned)(x0 / k6TileX) | ((unsigned)(y0 / k6TileY) << 10) | ((unsigned)grp << 20));
                 K6_TIC(r1);
-                if (!spin_until_gt(&S.done_items, i_pub - k6ItemRing, abort_flag, K6_ERR_ITEM)) return false;
-                K6_TOC(t_sw_item, r1);
-                if (lane == 0) {
-                    const int q = i_pub % k6ItemRing;
-                    S.it_x0[q] = x0; S.it_y0[q] = y0; S.it_g[q] = grp; S.it_kind[q] = kind;
-                    __threadfence_block();
-                    S.pub_items = i_pub + 1;
+                if (kind == 0) {
+                    if (!spin_until_gt(&S.done_z, z_pub - k6ZeroRing, abort_flag, K6_ERR_ITEM)) return false;
+                    K6_TOC(t_sw_item, r1);
+                    if (lane == 0) {
+                        S.z_item[z_pub % k6ZeroRing] = word;
+                        __threadfence_block();
+                        S.pub_z = z_pub + 1;
+                    }
+                    ++z_pub;
+                } else {
+                    if (!spin_until_gt(&S.done_c, i_pub - k6ItemRing, abort_flag, K6_ERR_ITEM)) return false;
+                    K6_TOC(t_sw_item, r1);
+                    if (lane == 0) {
+                        S.c_item[i_pub % k6ItemRing] = word;
+                        __threadfence_block();
+                        S.pub_c = i_pub + 1;
+                    }
+                    ++i_pub;
                 }
                 __syncwarp();
-                ++i_pub;
                 return true;
             };
             const int n_items = (int)P.n_items, C = P.list_cap;
@@ -628,9 +648,10 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 const int X0 = tx * k6TileX, Y0 = ty * k6TileY;
                 int cnt = 0;
                 if (c > 0 && c <= C) {
-                    // list path: <= 4 batches; open them all, write the queue, publish
+                    // list path: open the batches (the two youngest cover both stagers), write the queue and the descriptors
+                    // lane-parallel, publish everything with one fence
                     const int nbat = (c + k6Batch - 1) / k6Batch;
-                    for (int j = 0; j < nbat && alive; ++j) alive = batch_slot_free(b_next + j);
+                    alive = batch_slot_free(b_next + nbat - 1) && (nbat < 2 || batch_slot_free(b_next + nbat - 2));
                     if (!alive) break;
                     if (lane < c) {
                         const int slot = ((b_next + lane / k6Batch) % k6BatchRing) * k6Batch + (lane % k6Batch);
@@ -641,7 +662,41 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                         const int slot = ((b_next + i / k6Batch) % k6BatchRing) * k6Batch + (i % k6Batch);
                         S.q_row[slot] = (int)eb.x; S.q_mask[slot] = eb.y;
                     }
-                    cnt = c;
+                    if (lane < nbat) {
+                        const int q = (b_next + lane) % k6BatchRing;
+                        const bool lastb = lane == nbat - 1;
+                        S.b_n[q] = lastb ? c - (nbat - 1) * k6Batch : k6Batch;
+                        S.b_flags[q] = lastb ? k6FlagEnd : 0u;
+                        S.b_x0[q] = X0; S.b_y0[q] = Y0; S.b_g[q] = grp;
+                    }
+                    __syncwarp();
+                    __threadfence_block();
+                    if (lane == 0) {
+                        S.pub_batches = b_next + nbat;
+                        S.stat_hit_items += 1; S.stat_max_hits = max(S.stat_max_hits, c);
+                    }
+                    b_next += nbat;
+                    n_pub = b_next;
+#ifdef K6_L2_PREFETCH
+                    // warm L2 with what the stagers are about to copy: per hit 8 x 128 B of visibilities and one 128 B line
+                    // of raw table offsets (measured: no gain on C4, left out of the product build)
+                    if (grp * 32 + 32 <= P.n_chan) {
+                        for (int i0 = 0; i0 < c * 9; i0 += 32) {             // uniform trip count: the shuffles below need every lane
+                            const int i = i0 + lane;
+                            const int hit = min(i / 9, c - 1), line = i - (i / 9) * 9;
+                            const int ra = __shfl_sync(full, (int)ea.x, hit & 31), rb = __shfl_sync(full, (int)eb.x, hit & 31);
+                            const int row = hit < 32 ? ra : rb;
+                            const void* a = line < 8 ? (const void*)(P.vis + ((size_t)row * P.n_chan + grp * 32) * 8 + line * 32)
+                                                     : (const void*)(P.pre + (size_t)row * (P.n_groups * 32) + grp * 32);
+                            if (i < c * 9) asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+                        }
+                    }
+#endif
+                    if (!publish_item(X0, Y0, grp, 1)) { alive = false; break; }
+                    if (sub == 3) { sub = 0; cnt4 = cnt4_n; raw_next = claim(); } else ++sub;
+                    item = item_n;
+                    ea = ea_n; eb = eb_n;
+                    continue;
                 } else if (c > C) {
                     // fallback: the in-kernel sweep (dense tiles; also everything when the lists are disabled)
                     K6_TIC(d1);
@@ -701,7 +756,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
             K6_TOC(t_sw_all, sw0);
             K6_ADD(8, t_sw_all); K6_ADD(9, t_sw_ring); K6_ADD(10, t_sw_item); K6_ADD(11, t_sw_atomic); K6_ADD(22, t_sw_desc); K6_ADD(23, t_sw_loop);
             if (lane == 0 && P.stats) {
-                atomicAdd(P.stats + 1, i_pub - 1);                           // the exit descriptor is not an item
+                atomicAdd(P.stats + 1, i_pub - 1 + z_pub);                   // the exit descriptor is not an item
                 atomicAdd(P.stats + 2, S.stat_hit_items);
                 atomicAdd(P.stats + 3, b_next);
                 atomicMax(P.stats + 4, S.stat_max_hits);
@@ -802,93 +857,74 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
             K6_ADD(12, t_st_pub); K6_ADD(13, t_st_empty); K6_ADD(14, t_st_work); K6_ADD(15, n_st); K6_ADD(21, t_st_pre);
         } else {
             // =========================================================================================== store warp
-            // lane 0 issues the tensor-map stores of the block rows in whatever order the consumers finish them, and the
-            // zero-fill stores of the items nothing reaches.
-            const unsigned wo0 = smem_u32(base + L.wo), zero_s = smem_u32(base + L.zero);
-            int n_written = 0;
-            unsigned pending = 0u;                                           // block rows whose store has been issued but not released (lane 0)
-            long long t_so_rel = 0, t_so_items = 0, t_so_full = 0, t_so_zero = 0, t_so_all = 0;
-            (void)t_so_rel; (void)t_so_items; (void)t_so_full; (void)t_so_zero; (void)t_so_all;
-            K6_TIC(so0);
-            auto release_all = [&]() {                                       // lane 0 only
-                if (pending == 0u) return;
-                K6_TIC(s0);
-                asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the TMA engine has read the stages
-                K6_TOC(t_so_rel, s0);
-#pragma unroll
-                for (int r = 0; r < 4; ++r)
-                    if (pending & (1u << r)) mbar_arrive(smem_u32(&S.wo_empty[r]));
-                pending = 0u;
-            };
-            for (int i = 0;; ++i) {
-                int okw = 1;
-                if (lane == 0 && S.pub_items <= i) {
-                    release_all();                                           // idle: let the consumers have their stage back
-                    K6_TIC(s1);
-                    okw = spin_until_gt(&S.pub_items, i, abort_flag, K6_ERR_ITEM) ? 1 : 0;
-                    K6_TOC(t_so_items, s1);
-                }
-                okw = __shfl_sync(full, okw, 0);
-                if (!okw) break;
-                __threadfence_block();
-                const int q = i % k6ItemRing;
-                const int X0 = S.it_x0[q], Y0 = S.it_y0[q], c0 = S.it_g[q] * 32, kind = S.it_kind[q];
-                if (kind == 2) break;
-                if (kind == 0) {
-                    // one 4 KB box (16 cells x 32 channels) per tile row and pol from the zero buffer.  (Plain st.global
-                    // from this one warp was measured at 4 B / clock - latency-throttled; the TMA queue is deep.)
-                    K6_TIC(s2);
-                    if (lane == 0) {
-                        for (int pol = 0; pol < 4; ++pol)
-                            for (int v = 0; v < k6TileY; ++v)
-                                if (Y0 + v < N) tma_store4(&map_zero, zero_s, X0, c0, Y0 + v, pol);
-                        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-                    }
-                    K6_TOC(t_so_zero, s2);
-                } else {
-                    int oks = 1;
-                    if (lane == 0) {
-                        unsigned remaining = 0xfu;
-                        const unsigned par = (unsigned)(n_written & 1);
-                        long long t0 = 0;
-                        bool timing = false;
-                        while (remaining) {
-                            bool progress = false;
+            // One thread.  Consumer items come in order: the tensor-map store of each of their four block rows is issued
+            // as soon as that row's four warps have staged it, and the stage is handed back as soon as the TMA engine has
+            // read it (it is single-buffered: its consumers need it at the end of their next item).  Items nothing reaches
+            // are zero-filled from the zero buffer at low priority, four 4 KB boxes at a time, between looks at the rows.
+            // (Plain st.global zero-fill from this one warp was measured at 4 B / clock - latency-throttled.)
+            if (lane == 0) {
+                const unsigned wo0 = smem_u32(base + L.wo), zero_s = smem_u32(base + L.zero);
+                int ci = 0, zi = 0, zc = 0;                                  // consumer item, zero item, 4-store chunk of the zero item
+                unsigned remaining = 0xfu;                                   // block rows of consumer item ci still to store
+                long long t_so_rel = 0, t_so_idle = 0, t_so_zero = 0, t_so_all = 0;
+                (void)t_so_rel; (void)t_so_idle; (void)t_so_zero; (void)t_so_all;
+                K6_TIC(so0);
+                long long idle_t0 = 0;
+                bool idle = false;
+                for (;;) {
+                    bool progress = false;
+                    if (S.pub_c > ci) {
+                        __threadfence_block();
+                        const unsigned word = S.c_item[ci % k6ItemRing];
+                        if (word == k6ExitItem) {
+                            if (S.pub_z == zi) break;                        // every zero item was published before the exit marker
+                        } else {
+                            const int X0 = (int)(word & 1023u) * k6TileX, Y0 = (int)((word >> 10) & 1023u) * k6TileY, c0 = (int)(word >> 20) * 32;
+                            const unsigned par = (unsigned)(ci & 1);
 #pragma unroll
                             for (int r = 0; r < 4; ++r) {
-                                if ((remaining >> r) & 1u) {
-                                    if (mbar_try(smem_u32(&S.wo_full[r]), par)) {
-                                        if (Y0 + 2 * r < N) tma_store4(&map_out, wo0 + 32768u * r, X0, c0, Y0 + 2 * r, 0);
-                                        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-                                        pending |= 1u << r;
-                                        remaining &= ~(1u << r);
-                                        progress = true;
-                                    }
+                                if (((remaining >> r) & 1u) && mbar_try(smem_u32(&S.wo_full[r]), par)) {
+                                    if (Y0 + 2 * r < N) tma_store4(&map_out, wo0 + 32768u * r, X0, c0, Y0 + 2 * r, 0);
+                                    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                                    K6_TIC(s0);
+                                    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+                                    K6_TOC(t_so_rel, s0);
+                                    mbar_arrive(smem_u32(&S.wo_empty[r]));
+                                    remaining &= ~(1u << r);
+                                    progress = true;
                                 }
                             }
-                            if (!progress) {
-                                release_all();
-                                if (!timing) { t0 = clock64(); timing = true; }
-                                if (*abort_flag) { oks = 0; break; }
-                                if (clock64() - t0 > k6SpinLimit) { *abort_flag = K6_ERR_WOFULL; oks = 0; break; }
-                            }
+                            if (remaining == 0u) { ++ci; S.done_c = ci; remaining = 0xfu; }
                         }
-#ifdef K6_TIMING
-                        if (timing) t_so_full += clock64() - t0;
-#endif
                     }
-                    oks = __shfl_sync(full, oks, 0);
-                    if (!oks) break;
-                    ++n_written;
+                    if (S.pub_z > zi) {
+                        K6_TIC(s2);
+                        __threadfence_block();
+                        const unsigned word = S.z_item[zi % k6ZeroRing];
+                        const int X0 = (int)(word & 1023u) * k6TileX, Y0 = (int)((word >> 10) & 1023u) * k6TileY, c0 = (int)(word >> 20) * 32;
+                        const int pol = zc >> 1, v0 = (zc & 1) * 4;
+                        for (int v = v0; v < v0 + 4; ++v)
+                            if (Y0 + v < N) tma_store4(&map_zero, zero_s, X0, c0, Y0 + v, pol);
+                        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                        if (++zc == 8) { zc = 0; ++zi; S.done_z = zi; }
+                        progress = true;
+                        K6_TOC(t_so_zero, s2);
+                    }
+                    if (progress) {
+#ifdef K6_TIMING
+                        if (idle) t_so_idle += clock64() - idle_t0;
+#endif
+                        idle = false;
+                    } else {
+                        if (!idle) { idle_t0 = clock64(); idle = true; }
+                        if (*abort_flag) break;
+                        if (clock64() - idle_t0 > k6SpinLimit) { *abort_flag = K6_ERR_WOFULL; break; }
+                    }
                 }
-                __syncwarp();
-                if (lane == 0) S.done_items = i + 1;
-            }
-            if (lane == 0) {
                 asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // every store has landed before the CTA exits
                 K6_TOC(t_so_all, so0);
+                K6_ADD(16, t_so_all); K6_ADD(17, t_so_rel); K6_ADD(18, t_so_idle); K6_ADD(20, t_so_zero);
             }
-            K6_ADD(16, t_so_all); K6_ADD(17, t_so_rel); K6_ADD(18, t_so_items); K6_ADD(19, t_so_full); K6_ADD(20, t_so_zero);
         }
     }
     __syncthreads();
