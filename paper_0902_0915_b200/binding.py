@@ -160,11 +160,11 @@ def mwa_grid_plan_last_design(plan) -> str:
 
 
 def mwa_grid_plan_last_stats(plan):
-    """Counters of the last K6 call: dict(error, items, items_with_hits, batches, max_hits).  Synchronises."""
+    """Counters of the last K6 call: dict(error, items, items_with_hits, batches, max_hits, swept_items).  Synchronises."""
     buf = (ctypes.c_longlong * 32)()
     _check(_lib.mwa_grid_plan_last_stats(plan, ctypes.cast(buf, ctypes.c_void_p), 32))
     return {"error": int(buf[0]), "items": int(buf[1]), "items_with_hits": int(buf[2]), "batches": int(buf[3]),
-            "max_hits": int(buf[4]), "timing": [int(x) for x in buf[8:32]]}
+            "max_hits": int(buf[4]), "swept_items": int(buf[5]), "timing": [int(x) for x in buf[8:32]]}
 
 
 def mwa_grid_probe_fp32(plan, stream=None):

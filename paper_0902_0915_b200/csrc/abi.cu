@@ -88,21 +88,31 @@ static int ensure_workspace(Plan* p, long long n_vis, int n_chan) {
         ws.cap_pre = n_pre;
     }
     if (want_ws) {
-        // hit lists of K6: 64 entries of 8 B per item while that stays below 2 GiB, else fewer, else none
+        // hit lists of K6: per item a count and an offset into a pool sized for 12 candidate entries per (row, channel
+        // group) - about 1.5 x what the slot reservation of chan_list_kernel asks for on C4 - capped at 1 GiB; an item
+        // that finds the pool full is swept inside the gridding kernel instead, so the size is never a correctness matter
         const long long items = chanws_items(p, n_chan);
-        int cap = 64;
-        while (cap >= 16 && items * cap * 8 > (2LL << 30)) cap >>= 1;
-        if (cap < 16) cap = 0;
-        if (items > ws.cap_items || cap > ws.list_cap) {
+        if (items > ws.cap_items) {
             ws.cap_items = 0;
-            ws.list_cap = 0;
             if (!ensure(ws.d_list_cnt, (size_t)items, "hit counts")) return MWA_GRID_ERR_NOMEM;
-            unsigned long long* l = (unsigned long long*)ws.d_lists;
-            if (!ensure(l, (size_t)items * cap, "hit lists")) { ws.d_lists = l; return MWA_GRID_ERR_NOMEM; }
-            ws.d_lists = l;
+            if (!ensure(ws.d_list_off, (size_t)items, "hit list offsets")) return MWA_GRID_ERR_NOMEM;
+            if (!ensure(ws.d_z_list, (size_t)items, "zero item list")) return MWA_GRID_ERR_NOMEM;
+            int4* cd = (int4*)ws.d_c_desc;
+            if (!ensure(cd, (size_t)items, "item descriptors")) { ws.d_c_desc = cd; return MWA_GRID_ERR_NOMEM; }
+            ws.d_c_desc = cd;
             ws.cap_items = items;
         }
-        ws.list_cap = cap;
+        long long pool = n_vis * (long long)((n_chan + 31) / 32) * 12;
+        if (pool > (1LL << 27)) pool = 1LL << 27;
+        if (pool < 1024) pool = 1024;
+        if ((size_t)pool > ws.cap_pool) {
+            ws.cap_pool = 0;
+            unsigned long long* l = (unsigned long long*)ws.d_lists;
+            if (!ensure(l, (size_t)pool, "hit lists")) { ws.d_lists = l; return MWA_GRID_ERR_NOMEM; }
+            ws.d_lists = l;
+            ws.cap_pool = (size_t)pool;
+        }
+        ws.pool_cap = (unsigned)pool;
     }
     return MWA_GRID_OK;
 }
@@ -225,7 +235,7 @@ void mwa_grid_plan_destroy(mwa_grid_plan* plan) {
     Workspace& ws = p->ws;
     void* ptrs[] = {p->d_table, ws.d_scale, ws.d_group, ws.d_scale_ref, ws.d_bucket_count, ws.d_bucket_cursor, ws.d_perm, ws.d_perm_tmp,
                     ws.d_uv_sorted, ws.d_row_sorted, ws.d_tile_order, ws.d_tile_weight, ws.d_misc, ws.d_dispatch, ws.d_stage,
-                    ws.d_pre, ws.d_bb, ws.d_list_cnt, ws.d_lists};
+                    ws.d_pre, ws.d_bb, ws.d_list_cnt, ws.d_list_off, ws.d_c_desc, ws.d_z_list, ws.d_lists};
     for (void* q : ptrs)
         if (q) cudaFree(q);
     for (auto& e : p->ev)

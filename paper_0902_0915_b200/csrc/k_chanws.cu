@@ -42,17 +42,17 @@ constexpr int k6Consumers = 16;                       // consumer warps
 constexpr int k6Threads = (k6Consumers + 4) * 32;     // + sweeper, two stagers, store warp
 constexpr int k6TileX = 16, k6TileY = 8;
 constexpr int k6Batch = 8;                            // hits per batch
-constexpr int k6Stages = 8;                           // batches in flight (two per stager)
+constexpr int k6Stages = 14;                          // batches in flight (even: every stager keeps its own stages)
 constexpr int k6Stagers = 2;                          // stager warps; batch b is staged by stager b % 2 into stage b % 4
 constexpr int k6BatchRing = 32;                       // batch descriptors / queue segments between sweeper and stagers
 constexpr int k6ItemRing = 16;                        // consumer-item descriptors between sweeper and store warp
-constexpr int k6ZeroRing = 128;                       // zero-fill item descriptors (the store warp works them off at low priority)
 constexpr unsigned k6ExitItem = 0xffffffffu;
 constexpr int k6Drift = 8;                            // largest spread (cells) of the stamp origins over the 32 channels of a fast hit
 constexpr int k6PadU = 15 + k6Drift + 1, k6PadV = 7 + k6Drift + 1;   // zero padding in front of a table row (floats)
 constexpr int k6Bias = 2048;                          // > any stamp origin (N <= 2048): keeps both halves of a raw offset word positive
 constexpr int k6ZeroFloats = 32;                      // all-zero block behind each table (target of a missing lane)
-constexpr int k6WoBytes = 4 * 32768;                  // write-out stage: 4 block rows x [pol 4][v 2][chan 32][128 B]
+constexpr int k6WoSlots = 2;                          // write-out stage slots; block row r uses slot r & 1, rows r and r + 2 take turns
+constexpr int k6WoBytes = k6WoSlots * 32768;          // write-out stage: slots of [pol 4][v 2][chan 32][128 B]
 constexpr int k6StageV = k6Batch * 1024, k6StageGeo = k6Batch * 128, k6StageW = k6Batch * 128;
 constexpr int k6StageBytes = k6StageV + k6StageGeo + k6StageW;
 constexpr int k6ZeroBytes = 4096;                     // zero buffer: [chan 32][128 B]
@@ -70,9 +70,14 @@ struct K6Params {
     const int* perm;             // [n_vis] sorted position -> row
     const unsigned* pre;         // [n_vis][n_groups * 32] packed indices, by ROW
     const ushort4* bb;           // [n_groups][n_vis] bounding boxes, by SORTED POSITION
-    const int* list_cnt;         // [n_items] hits of every item (chan_list_kernel)
-    const uint2* lists;          // [n_items][list_cap] (row, mask) of the first list_cap hits of every item
-    int list_cap;                // 0 = no lists: the in-kernel sweeper sweeps every item
+    const int* list_cnt;         // [n_items] hits of every item (chan_list_kernel); -1 = no list: the in-kernel sweeper sweeps it
+    const unsigned* list_off;    // [n_items] first entry of the item's hit list in the pool
+    const int4* c_desc;          // [n_c] (item, hits or -1, list offset, 0) of the items with hits, in item order (chan_order_kernel)
+    const unsigned* z_list;      // [n_z] the items nothing reaches, in item order
+    const int* n_cz;             // [2] n_c, n_z
+    int* zcounter;               // work counter of the zero list
+    const uint2* lists;          // [pool_cap] pool of hit lists: (row, mask) entries, an item's hits contiguous and in sweep order
+    unsigned pool_cap;           // entries in the pool; 0 = no lists at all
     int* counter;                // work counter
     int* stats;                  // [8] error, items, items with hits, batches, max hits of an item
     const int* dispatch;         // device-side design choice (AUTO); null = always run
@@ -89,7 +94,7 @@ struct K6Params {
 
 struct K6Ctrl {
     unsigned long long full[k6Stages], empty[k6Stages];     // mbarriers: batch staged / batch consumed
-    unsigned long long wo_full[4], wo_empty[4];             // mbarriers: block row staged for the store / stage free
+    unsigned long long wo_full[k6WoSlots], wo_empty[4];     // mbarriers: slot staged for the store (by the 4 warps of a block row) / block row r's store has been read
     int st_n[k6Stages];
     unsigned st_flags[k6Stages];
     unsigned st_tile[k6Stages];                             // tile term of the batch's raw table-offset words
@@ -100,11 +105,10 @@ struct K6Ctrl {
     unsigned b_flags[k6BatchRing];
     int b_x0[k6BatchRing], b_y0[k6BatchRing], b_g[k6BatchRing];
     unsigned c_item[k6ItemRing];                            // consumer items in order: tx | ty << 10 | group << 20, k6ExitItem = exit
-    unsigned z_item[k6ZeroRing];                            // items nothing reaches (zero-fill), any order
-    volatile int pub_batches, pub_c, done_c, pub_z, done_z;
+    volatile int pub_batches, pub_c, done_c;
     volatile int done_batches[k6Stagers];
     volatile int abort;
-    int stat_hit_items, stat_max_hits;                      // sweeper's counters for mwa_grid_plan_last_stats
+    int stat_hit_items, stat_max_hits, stat_swept_items;    // sweeper's counters for mwa_grid_plan_last_stats
 };
 
 // Optional phase timing (build with MWA_EXTRA_NVCC=-DK6_TIMING): clock64 sums per role in stats64[], read back through
@@ -153,12 +157,20 @@ __device__ __forceinline__ bool mbar_try(unsigned bar, unsigned parity) {
     return ok != 0;
 }
 // Bounded wait: returns false when the kernel is being aborted (a wait that exceeded k6SpinLimit raises the abort).
+// try_wait with a suspend-time hint: the hardware parks the thread until the phase completes or ~1 us has passed, so a
+// waiting warp does not take issue slots from the working warps of its scheduler
+__device__ __forceinline__ bool mbar_try_park(unsigned bar, unsigned parity) {
+    unsigned ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok) : "r"(bar), "r"(parity), "r"(1000u) : "memory");
+    return ok != 0;
+}
 __device__ __forceinline__ bool mbar_wait(unsigned bar, unsigned parity, volatile int* abort_flag, int code) {
     if (mbar_try(bar, parity)) return true;
     const long long t0 = clock64();
-    while (!mbar_try(bar, parity)) {
+    for (int spins = 1; !mbar_try_park(bar, parity); ++spins) {
         if (*abort_flag) return false;
-        if (clock64() - t0 > k6SpinLimit) { *abort_flag = code; return false; }
+        if ((spins & 255) == 0 && clock64() - t0 > k6SpinLimit) { *abort_flag = code; return false; }
     }
     return true;
 }
@@ -334,13 +346,17 @@ __device__ __forceinline__ bool k6_sweep(const K6Params& P, const K6Item& it, in
     return true;
 }
 
-// Second pre-pass: one warp per item sweeps it and writes its hit list (row, mask) into the item's slot of `cap`
-// entries, and the TOTAL number of hits into list_cnt (a count above `cap` tells chanws_kernel's sweeper to sweep the
-// item itself).  Runs with thousands of warps in flight, which hides the L2 round trips a single in-kernel sweeper
-// warp paid one after the other (4.6 us per item measured).
+// Second pre-pass: one warp per item sweeps it and writes its hit list (row, mask) into a pool.  The slot of an item is
+// reserved with one atomicAdd of an upper bound that costs nothing to compute - the number of sorted rows in the item's
+// bucket window (every hit is one of them) - so lists of any length are contiguous and written in one sweep; where a
+// list lands in the pool may differ from run to run, what it holds does not.  An item the pool has no room for gets the
+// count -1 and is swept by chanws_kernel's own sweeper instead.  Runs with thousands of warps in flight, which hides the
+// L2 round trips a single in-kernel sweeper warp pays one after the other (4.6 us per item measured).
 __global__ void __launch_bounds__(256)
-chan_list_kernel(const __grid_constant__ K6Params P, int* __restrict__ list_cnt, uint2* __restrict__ lists, int cap) {
+chan_list_kernel(const __grid_constant__ K6Params P, int* __restrict__ list_cnt, unsigned* __restrict__ list_off,
+                 uint2* __restrict__ pool, unsigned long long* __restrict__ cursor) {
     if (P.dispatch != nullptr && *P.dispatch != P.dispatch_want) return;
+    const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const int warps = (gridDim.x * blockDim.x) >> 5;
     const int n_items = (int)P.n_items;
@@ -349,15 +365,74 @@ chan_list_kernel(const __grid_constant__ K6Params P, int* __restrict__ list_cnt,
         const int tx = item % P.ntx, ty = (item / P.ntx) % P.nty, grp = item / (P.ntx * P.nty);
         const double4 gi = P.group[grp];
         const K6Item it = k6_describe(P, tx * k6TileX, ty * k6TileY, grp, gi.z, gi.w);
-        uint2* dst = lists + (size_t)item * cap;
+        int cand = 0;
+        for (int rg = it.wy0 + lane; rg <= it.wy1; rg += 32)
+            cand += __ldg(P.bucket_start + rg * P.nb + it.wx1 + 1) - __ldg(P.bucket_start + rg * P.nb + it.wx0);
+        cand = __reduce_add_sync(full, cand);
+        if (cand == 0) {
+            if (lane == 0) { list_cnt[item] = 0; list_off[item] = 0u; }
+            continue;
+        }
+        unsigned long long base = 0ull;
+        if (lane == 0) base = atomicAdd(cursor, (unsigned long long)cand);
+        base = __shfl_sync(full, base, 0);
+        if (base + (unsigned long long)cand > (unsigned long long)P.pool_cap) {
+            if (lane == 0) { list_cnt[item] = -1; list_off[item] = 0u; }
+            continue;
+        }
+        uint2* dst = pool + base;
         int cnt = 0;
         k6_sweep(P, it, lane, [&](bool hit, int row, unsigned mask, unsigned hm, int n_new) -> bool {
-            const int i = cnt + __popc(hm & lt_mask);
-            if (hit && i < cap) dst[i] = make_uint2((unsigned)row, mask);
+            if (hit) dst[cnt + __popc(hm & lt_mask)] = make_uint2((unsigned)row, mask);
             cnt += n_new;
             return true;
         });
-        if (lane == 0) list_cnt[item] = cnt;
+        if (lane == 0) { list_cnt[item] = cnt; list_off[item] = (unsigned)base; }
+    }
+}
+
+// Third pre-pass, one block: splits the items into those with hits (c_desc: item, hit count, list offset - what the
+// sweeper of chanws_kernel claims, four at a time) and those nothing reaches (z_list - what its zero feeder claims), both
+// in item order, so neighbouring tiles are still worked on at about the same time and share their halo rows in L2.
+__global__ void __launch_bounds__(1024)
+chan_order_kernel(const int* __restrict__ list_cnt, const unsigned* __restrict__ list_off, int n_items, int4* __restrict__ c_desc,
+                  unsigned* __restrict__ z_list, int* __restrict__ n_cz, const int* __restrict__ dispatch, int dispatch_want) {
+    if (dispatch != nullptr && *dispatch != dispatch_want) return;
+    __shared__ int s_tot[32], s_base[32];
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int chunk = (((n_items + 31) / 32 + 31) / 32) * 32;             // items per warp, a multiple of 32
+    const int i0 = warp * chunk, i1 = min(n_items, i0 + chunk);
+    int nz = 0;
+    for (int i = i0 + lane; i < i1; i += 32) nz += list_cnt[i] != 0 ? 1 : 0;
+    nz = __reduce_add_sync(full, nz);
+    if (lane == 0) s_tot[warp] = nz;
+    __syncthreads();
+    if (warp == 0) {
+        const int t = s_tot[lane];
+        int incl = t;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int u = __shfl_up_sync(full, incl, o);
+            if (lane >= o) incl += u;
+        }
+        s_base[lane] = incl - t;
+        if (lane == 31) { n_cz[0] = incl; n_cz[1] = n_items - incl; }
+    }
+    __syncthreads();
+    int cb = s_base[warp], zb = min(i0, n_items) - cb;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    for (int s0 = i0; s0 < i1; s0 += 32) {
+        const int i = s0 + lane;
+        const bool valid = i < i1;
+        const int cnt = valid ? list_cnt[i] : 0;
+        const unsigned bm = __ballot_sync(full, valid && cnt != 0), vm = __ballot_sync(full, valid);
+        if (valid) {
+            if (cnt != 0) c_desc[cb + __popc(bm & lt_mask)] = make_int4(i, cnt, (int)list_off[i], 0);
+            else z_list[zb + __popc(vm & ~bm & lt_mask)] = (unsigned)i;
+        }
+        cb += __popc(bm);
+        zb += __popc(vm & ~bm);
     }
 }
 
@@ -409,7 +484,8 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
         for (int s = 0; s < k6Stages; ++s) {
             mbar_init(smem_u32(&S.full[s]), 33); mbar_init(smem_u32(&S.empty[s]), k6Consumers);   // 32 cp.async arrivals + 1
         }
-        for (int r = 0; r < 4; ++r) { mbar_init(smem_u32(&S.wo_full[r]), 4); mbar_init(smem_u32(&S.wo_empty[r]), 1); }
+        for (int r = 0; r < k6WoSlots; ++r) mbar_init(smem_u32(&S.wo_full[r]), 4);
+        for (int r = 0; r < 4; ++r) mbar_init(smem_u32(&S.wo_empty[r]), 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // zero buffer and barriers visible to the async proxy
@@ -425,7 +501,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
         const unsigned wbit = (unsigned)warp;                           // bit by * 4 + bx of a hit mask
         const unsigned tu_s = smem_u32(tu) + 16u * bx, tv_s = smem_u32(tv) + 8u * by;
         // the lane's two 16 B chunks of a 128 B stage row: chunk (2 bx + k) ^ (row & 7), row & 7 = lane & 7
-        const unsigned wo_s = smem_u32(base + L.wo) + 32768u * by + 128u * lane;
+        const unsigned wo_s = smem_u32(base + L.wo) + 32768u * (by & 1) + 128u * lane;
         const unsigned wo_c0 = wo_s + 16u * ((2u * bx) ^ (lane & 7u)), wo_c1 = wo_s + 16u * ((2u * bx + 1u) ^ (lane & 7u));
         u64 acc[2][4][4];                                               // [row i][col j][pol] = (re, im) of the lane's channel
 #pragma unroll
@@ -438,7 +514,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
         long long t_full = 0, t_visit = 0, t_woe = 0, t_wo = 0, n_vis_cnt = 0, n_bat = 0;
         (void)t_full; (void)t_visit; (void)t_woe; (void)t_wo; (void)n_vis_cnt; (void)n_bat;
         for (int k = 0;; ++k) {
-            const int s = k & (k6Stages - 1);
+            const int s = k % k6Stages;
             K6_TIC(c0);
             if (!mbar_wait(smem_u32(&S.full[s]), (unsigned)((k / k6Stages) & 1), abort_flag, K6_ERR_FULL)) break;
             K6_TOC(t_full, c0);
@@ -447,15 +523,18 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
             if (flags & k6FlagExit) break;
             unsigned m = __ballot_sync(full, lane < k6Batch && ((S.st_mask[s][lane] >> wbit) & 1u));
             const unsigned tc = S.st_tile[s];                           // 4 (X0 - k6Bias) | 4 (Y0 - k6Bias) << 16: completes a raw offset word
-            const unsigned zs_s = ring_s + (unsigned)s * k6StageBytes + 32u * lane;
+            const unsigned zs_s = ring_s + (unsigned)s * k6StageBytes + 16u * lane;   // [hit][half][lane][16 B]: conflict-free LDS.128
             const unsigned geo_s = ring_s + (unsigned)s * k6StageBytes + k6StageV + 4u * lane;
             const unsigned wt_s = geo_s + k6StageGeo;
+#ifdef K6_ABLATE_FMA
+            m = 0u;
+#endif
             if (m != 0u) {
                 // software pipeline over the set bits of m, two visits per trip with two register sets (as K5 phase B)
 #define K6_NEXT(mm, prev) ((mm) ? (int)(__ffs(mm) - 1) : (prev)); (mm) &= (mm) - 1u
 #define K6_LOAD(h, g, Z0, Z1, Z2, Z3, U0, U1, U2, U3, V0, V1, WT)                                                         \
     asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(Z0), "=l"(Z1) : "r"(zs_s + 1024u * (h)));                       \
-    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(Z2), "=l"(Z3) : "r"(zs_s + 1024u * (h) + 16u));                 \
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(Z2), "=l"(Z3) : "r"(zs_s + 1024u * (h) + 512u));                \
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(U0), "=f"(U1), "=f"(U2), "=f"(U3) : "r"(tu_s + ((g) & 0xffffu))); \
     asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(V0), "=f"(V1) : "r"(tv_s + ((g) >> 16)));                       \
     if (HAS_W) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(WT) : "r"(wt_s + 128u * (h)));
@@ -518,7 +597,10 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
             if (flags & k6FlagEnd) {
                 // ---- a5: accumulators -> swizzled stage of this block row; the store warp issues the TMA store
                 K6_TIC(c2);
-                if (!mbar_wait(smem_u32(&S.wo_empty[by]), (unsigned)((n_written & 1) ^ 1), abort_flag, K6_ERR_WOEMPTY)) break;
+                // block rows by and by ^ 2 take turns on slot by & 1 (0, 2, 0, 2, ... item after item): the slot is free when
+                // the store of the OTHER row's last use has been read - rows 2, 3 wait for rows 0, 1 of this item, rows 0, 1 for
+                // rows 2, 3 of the item before (the store warp keeps that order, so the own last use has been read as well)
+                if (!mbar_wait(smem_u32(&S.wo_empty[by ^ 2]), (unsigned)((n_written & 1) ^ (by < 2 ? 1 : 0)), abort_flag, K6_ERR_WOEMPTY)) break;
                 K6_TOC(t_woe, c2);
                 K6_TIC(c3);
 #pragma unroll
@@ -535,7 +617,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                     }
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                 __syncwarp();
-                if (lane == 0) mbar_arrive(smem_u32(&S.wo_full[by]));
+                if (lane == 0) mbar_arrive(smem_u32(&S.wo_full[by & 1]));
                 ++n_written;
                 K6_TOC(t_wo, c3);
             }
@@ -580,125 +662,109 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 if (lane == 0) S.pub_batches = upto + 1;
                 n_pub = upto + 1;
             };
-            int z_pub = 0;               // zero-fill items published so far
-            // kind 0: zero-fill item (any order), 1: consumer item (in order), 2: exit marker behind the last consumer item
-            auto publish_item = [&](int x0, int y0, int grp, int kind) -> bool {
-                const unsigned word = kind == 2 ? k6ExitItem : ((unsigned)(x0 / k6TileX) | ((unsigned)(y0 / k6TileY) << 10) | ((unsigned)grp << 20));
+            // consumer item (in order), or with exit = true the exit marker behind the last one
+            auto publish_item = [&](int x0, int y0, int grp, bool exit) -> bool {
+                const unsigned word = exit ? k6ExitItem : ((unsigned)(x0 / k6TileX) | ((unsigned)(y0 / k6TileY) << 10) | ((unsigned)grp << 20));
                 K6_TIC(r1);
-                if (kind == 0) {
-                    if (!spin_until_gt(&S.done_z, z_pub - k6ZeroRing, abort_flag, K6_ERR_ITEM)) return false;
-                    K6_TOC(t_sw_item, r1);
-                    if (lane == 0) {
-                        S.z_item[z_pub % k6ZeroRing] = word;
-                        __threadfence_block();
-                        S.pub_z = z_pub + 1;
-                    }
-                    ++z_pub;
-                } else {
-                    if (!spin_until_gt(&S.done_c, i_pub - k6ItemRing, abort_flag, K6_ERR_ITEM)) return false;
-                    K6_TOC(t_sw_item, r1);
-                    if (lane == 0) {
-                        S.c_item[i_pub % k6ItemRing] = word;
-                        __threadfence_block();
-                        S.pub_c = i_pub + 1;
-                    }
-                    ++i_pub;
+                if (!spin_until_gt(&S.done_c, i_pub - k6ItemRing, abort_flag, K6_ERR_ITEM)) return false;
+                K6_TOC(t_sw_item, r1);
+                if (lane == 0) {
+                    S.c_item[i_pub % k6ItemRing] = word;
+                    __threadfence_block();
+                    S.pub_c = i_pub + 1;
                 }
+                ++i_pub;
                 __syncwarp();
                 return true;
             };
-            const int n_items = (int)P.n_items, C = P.list_cap;
+            const int n_c = __ldg(P.n_cz);
             auto claim = [&]() -> int { return lane == 0 ? atomicAdd(P.counter, 4) : 0; };      // raw: valid in lane 0 only
-            auto load_counts = [&](int base) -> int {                                           // lane k < 4: hit count of item base + k
-                int c = 0;
-                if (lane < 4 && base + lane < n_items && base >= 0) c = C > 0 ? __ldg(P.list_cnt + base + lane) : 1 << 30;
-                return c;
+            // lane k < 4: (item, hit count, list offset) of entry base + k of the list of items with hits
+            auto load_desc = [&](int base) -> int4 {
+                int4 d = make_int4(0, 0, 0, 0);
+                if (lane < 4 && base + lane < n_c && base >= 0) d = __ldg(P.c_desc + base + lane);
+                return d;
             };
-            auto load_entries = [&](int it, int c, uint2& ea, uint2& eb) {                      // list entries lane and lane + 32
+            auto load_entries = [&](unsigned off, int c, int first, uint2& ea, uint2& eb) {     // list entries first + lane, first + lane + 32
                 ea = make_uint2(0u, 0u); eb = ea;
-                if (c > 0 && c <= C) {
-                    const uint2* src = P.lists + (size_t)it * C;
-                    if (lane < c) ea = __ldg(src + lane);
-                    if (lane + 32 < c) eb = __ldg(src + lane + 32);
+                if (c > 0) {
+                    const uint2* src = P.lists + off;
+                    if (first + lane < c) ea = __ldg(src + first + lane);
+                    if (first + lane + 32 < c) eb = __ldg(src + first + lane + 32);
                 }
             };
             K6_TIC(r2);
-            int item = __shfl_sync(full, claim(), 0);
+            int ci = __shfl_sync(full, claim(), 0);          // index into c_desc
             K6_TOC(t_sw_atomic, r2);
-            int cnt4 = load_counts(item), cnt4_n = 0, base_n = 0;
+            int4 d4 = load_desc(ci), d4_n = make_int4(0, 0, 0, 0);
+            int base_n = 0;
             int raw_next = claim();
             int sub = 0;
             uint2 ea, eb;
-            load_entries(item, __shfl_sync(full, cnt4, 0), ea, eb);
-            while (alive && item < n_items && item >= 0) {
-                // ---- look ahead: the next claim's counts (one item after the claim was issued), the next item's entries
+            load_entries((unsigned)__shfl_sync(full, d4.z, 0), __shfl_sync(full, d4.y, 0), 0, ea, eb);
+            while (alive && ci < n_c && ci >= 0) {
+                // ---- look ahead: the next claim's descriptors (one item after the claim was issued), the next item's entries
                 if (sub == 1) {
                     K6_TIC(r3);
                     base_n = __shfl_sync(full, raw_next, 0);
                     K6_TOC(t_sw_atomic, r3);
-                    cnt4_n = load_counts(base_n);
+                    d4_n = load_desc(base_n);
                 }
-                const int c = __shfl_sync(full, cnt4, sub);
-                const int item_n = sub == 3 ? base_n : item + 1;
-                const int c_n = (item_n < n_items && item_n >= 0) ? (sub == 3 ? __shfl_sync(full, cnt4_n, 0) : __shfl_sync(full, cnt4, sub + 1)) : 0;
+                const int item = __shfl_sync(full, d4.x, sub), c = __shfl_sync(full, d4.y, sub);
+                const unsigned off = (unsigned)__shfl_sync(full, d4.z, sub);
+                const int ci_n = sub == 3 ? base_n : ci + 1;
+                const bool valid_n = ci_n < n_c && ci_n >= 0;
+                const int c_n = valid_n ? (sub == 3 ? __shfl_sync(full, d4_n.y, 0) : __shfl_sync(full, d4.y, (sub + 1) & 3)) : 0;
+                const unsigned off_n = (unsigned)(sub == 3 ? __shfl_sync(full, d4_n.z, 0) : __shfl_sync(full, d4.z, (sub + 1) & 3));
                 uint2 ea_n, eb_n;
-                load_entries(item_n, c_n, ea_n, eb_n);
+                load_entries(off_n, c_n, 0, ea_n, eb_n);
                 // ---- this item
                 const int tx = item % P.ntx, ty = (item / P.ntx) % P.nty, grp = item / (P.ntx * P.nty);
                 const int X0 = tx * k6TileX, Y0 = ty * k6TileY;
                 int cnt = 0;
-                if (c > 0 && c <= C) {
-                    // list path: open the batches (the two youngest cover both stagers), write the queue and the descriptors
-                    // lane-parallel, publish everything with one fence
-                    const int nbat = (c + k6Batch - 1) / k6Batch;
-                    alive = batch_slot_free(b_next + nbat - 1) && (nbat < 2 || batch_slot_free(b_next + nbat - 2));
-                    if (!alive) break;
-                    if (lane < c) {
-                        const int slot = ((b_next + lane / k6Batch) % k6BatchRing) * k6Batch + (lane % k6Batch);
-                        S.q_row[slot] = (int)ea.x; S.q_mask[slot] = ea.y;
-                    }
-                    if (lane + 32 < c) {
-                        const int i = lane + 32;
-                        const int slot = ((b_next + i / k6Batch) % k6BatchRing) * k6Batch + (i % k6Batch);
-                        S.q_row[slot] = (int)eb.x; S.q_mask[slot] = eb.y;
-                    }
-                    if (lane < nbat) {
-                        const int q = (b_next + lane) % k6BatchRing;
-                        const bool lastb = lane == nbat - 1;
-                        S.b_n[q] = lastb ? c - (nbat - 1) * k6Batch : k6Batch;
-                        S.b_flags[q] = lastb ? k6FlagEnd : 0u;
-                        S.b_x0[q] = X0; S.b_y0[q] = Y0; S.b_g[q] = grp;
-                    }
-                    __syncwarp();
-                    __threadfence_block();
-                    if (lane == 0) {
-                        S.pub_batches = b_next + nbat;
-                        S.stat_hit_items += 1; S.stat_max_hits = max(S.stat_max_hits, c);
-                    }
-                    b_next += nbat;
-                    n_pub = b_next;
-#ifdef K6_L2_PREFETCH
-                    // warm L2 with what the stagers are about to copy: per hit 8 x 128 B of visibilities and one 128 B line
-                    // of raw table offsets (measured: no gain on C4, left out of the product build)
-                    if (grp * 32 + 32 <= P.n_chan) {
-                        for (int i0 = 0; i0 < c * 9; i0 += 32) {             // uniform trip count: the shuffles below need every lane
-                            const int i = i0 + lane;
-                            const int hit = min(i / 9, c - 1), line = i - (i / 9) * 9;
-                            const int ra = __shfl_sync(full, (int)ea.x, hit & 31), rb = __shfl_sync(full, (int)eb.x, hit & 31);
-                            const int row = hit < 32 ? ra : rb;
-                            const void* a = line < 8 ? (const void*)(P.vis + ((size_t)row * P.n_chan + grp * 32) * 8 + line * 32)
-                                                     : (const void*)(P.pre + (size_t)row * (P.n_groups * 32) + grp * 32);
-                            if (i < c * 9) asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+                if (c > 0) {
+                    // list path: the list is streamed in chunks of 64 hits = 8 batches, the next chunk in flight while this
+                    // one goes into the queue.  Per chunk: open the batches (the two youngest cover both stagers), write the
+                    // queue and the descriptors lane-parallel, publish everything with one fence
+                    K6_TIC(d0);
+                    for (int done = 0;;) {
+                        const int n_chunk = min(64, c - done);
+                        const bool more = done + 64 < c;
+                        uint2 fa = make_uint2(0u, 0u), fb = fa;
+                        if (more) load_entries(off, c, done + 64, fa, fb);
+                        const int nbat = (n_chunk + k6Batch - 1) / k6Batch;
+                        alive = batch_slot_free(b_next + nbat - 1) && (nbat < 2 || batch_slot_free(b_next + nbat - 2));
+                        if (!alive) break;
+                        if (lane < n_chunk) {
+                            const int slot = ((b_next + lane / k6Batch) % k6BatchRing) * k6Batch + (lane % k6Batch);
+                            S.q_row[slot] = (int)ea.x; S.q_mask[slot] = ea.y;
                         }
+                        if (lane + 32 < n_chunk) {
+                            const int i = lane + 32;
+                            const int slot = ((b_next + i / k6Batch) % k6BatchRing) * k6Batch + (i % k6Batch);
+                            S.q_row[slot] = (int)eb.x; S.q_mask[slot] = eb.y;
+                        }
+                        if (lane < nbat) {
+                            const int q = (b_next + lane) % k6BatchRing;
+                            const bool lastb = lane == nbat - 1;
+                            S.b_n[q] = lastb ? n_chunk - (nbat - 1) * k6Batch : k6Batch;
+                            S.b_flags[q] = (lastb && !more) ? k6FlagEnd : 0u;
+                            S.b_x0[q] = X0; S.b_y0[q] = Y0; S.b_g[q] = grp;
+                        }
+                        __syncwarp();
+                        __threadfence_block();
+                        if (lane == 0) S.pub_batches = b_next + nbat;
+                        b_next += nbat;
+                        n_pub = b_next;
+                        if (!more) break;
+                        done += 64;
+                        ea = fa; eb = fb;
                     }
-#endif
-                    if (!publish_item(X0, Y0, grp, 1)) { alive = false; break; }
-                    if (sub == 3) { sub = 0; cnt4 = cnt4_n; raw_next = claim(); } else ++sub;
-                    item = item_n;
-                    ea = ea_n; eb = eb_n;
-                    continue;
-                } else if (c > C) {
-                    // fallback: the in-kernel sweep (dense tiles; also everything when the lists are disabled)
+                    K6_TOC(t_sw_desc, d0);
+                    if (!alive) break;
+                    if (lane == 0) { S.stat_hit_items += 1; S.stat_max_hits = max(S.stat_max_hits, c); }
+                } else {
+                    // fallback: the in-kernel sweep (the pool had no room for this item's list)
                     K6_TIC(d1);
                     const double4 gi = P.group[grp];
                     const K6Item it = k6_describe(P, X0, Y0, grp, gi.z, gi.w);
@@ -723,17 +789,21 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                     });
                     K6_TOC(t_sw_loop, d1);
                     if (!alive) break;
-                }
-                if (cnt > 0) {
-                    const int last = b_next + (cnt - 1) / k6Batch;
-                    publish_batches(last, cnt - ((cnt - 1) / k6Batch) * k6Batch, k6FlagEnd, X0, Y0, grp);
+                    // the last batch carries the end flag; an item the sweep found nothing for gets one empty batch, so the
+                    // consumers write its zeros through the ordinary path
+                    if (cnt == 0 && !batch_slot_free(b_next)) { alive = false; break; }
+                    const int last = cnt > 0 ? b_next + (cnt - 1) / k6Batch : b_next;
+                    publish_batches(last, cnt > 0 ? cnt - ((cnt - 1) / k6Batch) * k6Batch : 0, k6FlagEnd, X0, Y0, grp);
                     b_next = last + 1;
-                    if (lane == 0) { S.stat_hit_items += 1; S.stat_max_hits = max(S.stat_max_hits, cnt); }   // in shared memory: no registers to spare here
+                    if (lane == 0) {                                         // in shared memory: no registers to spare here
+                        S.stat_swept_items += 1;
+                        if (cnt > 0) { S.stat_hit_items += 1; S.stat_max_hits = max(S.stat_max_hits, cnt); }
+                    }
                 }
-                if (!publish_item(X0, Y0, grp, cnt > 0 ? 1 : 0)) { alive = false; break; }
+                if (!publish_item(X0, Y0, grp, false)) { alive = false; break; }
                 // ---- advance
-                if (sub == 3) { sub = 0; cnt4 = cnt4_n; raw_next = claim(); } else ++sub;
-                item = item_n;
+                if (sub == 3) { sub = 0; d4 = d4_n; raw_next = claim(); } else ++sub;
+                ci = ci_n;
                 ea = ea_n; eb = eb_n;
             }
             // exit: one flagged batch per stager (consumers stop at the first one), one flagged item for the store warp
@@ -751,15 +821,16 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                     }
                     __syncwarp();
                 }
-                publish_item(0, 0, 0, 2);
+                publish_item(0, 0, 0, true);
             }
             K6_TOC(t_sw_all, sw0);
             K6_ADD(8, t_sw_all); K6_ADD(9, t_sw_ring); K6_ADD(10, t_sw_item); K6_ADD(11, t_sw_atomic); K6_ADD(22, t_sw_desc); K6_ADD(23, t_sw_loop);
             if (lane == 0 && P.stats) {
-                atomicAdd(P.stats + 1, i_pub - 1 + z_pub);                   // the exit descriptor is not an item
+                atomicAdd(P.stats + 1, i_pub - 1);                           // consumer items (the exit descriptor is not one)
                 atomicAdd(P.stats + 2, S.stat_hit_items);
                 atomicAdd(P.stats + 3, b_next);
                 atomicMax(P.stats + 4, S.stat_max_hits);
+                atomicAdd(P.stats + 5, S.stat_swept_items);
             }
         } else if (role <= k6Stagers) {
             // =========================================================================================== stagers
@@ -777,9 +848,9 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
             long long t_st_pub = 0, t_st_empty = 0, t_st_work = 0, t_st_pre = 0, n_st = 0;
             (void)t_st_pub; (void)t_st_empty; (void)t_st_work; (void)t_st_pre; (void)n_st;
             for (int b = sg;; b += k6Stagers) {
-                const int s = b & (k6Stages - 1);
+                const int s = b % k6Stages;
                 const unsigned st_base = ring_s + (unsigned)s * k6StageBytes;
-                const unsigned zs_a = st_base + 32u * lane, geo_a = st_base + k6StageV + 4u * lane, wt_a = geo_a + k6StageGeo;
+                const unsigned zs_a = st_base + 16u * lane, geo_a = st_base + k6StageV + 4u * lane, wt_a = geo_a + k6StageGeo;
                 const unsigned full_bar = smem_u32(&S.full[s]), empty_bar = smem_u32(&S.empty[s]);
                 K6_TIC(q0);
                 if (!spin_until_gt(&S.pub_batches, b, abort_flag, K6_ERR_BATCH)) break;
@@ -811,9 +882,11 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                         asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(wt_a + 128u * (unsigned)hh), "l"(P.weights + (size_t)r * P.n_chan + cc) : "memory");
                     if ((slow_m >> hh) & 1u) continue;                       // uniform
                     asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(geo_a + 128u * (unsigned)hh), "l"(P.pre + (size_t)r * ncp + c0 + lane) : "memory");
+#ifndef K6_ABLATE_LOAD
                     const float* src = P.vis + ((size_t)r * P.n_chan + cc) * 8;
                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(zs_a + 1024u * (unsigned)hh), "l"(src) : "memory");
-                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(zs_a + 1024u * (unsigned)hh + 16u), "l"(src + 4) : "memory");
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(zs_a + 1024u * (unsigned)hh + 512u), "l"(src + 4) : "memory");
+#endif
                 }
                 for (unsigned sm_ = slow_m; sm_ != 0u; sm_ &= sm_ - 1u) {   // slow hits: packed (origin, table row) words, range-checked here
                     const int hh = __ffs(sm_) - 1;
@@ -837,7 +910,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                     const float* src = P.vis + ((size_t)r * P.n_chan + cc) * 8;
                     const unsigned sz = (cvalid && w32 != k6Invalid) ? 16u : 0u;   // zero-filled where the lane has no sample (R11)
                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(zs_a + 1024u * (unsigned)hh), "l"(src), "r"(sz) : "memory");
-                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(zs_a + 1024u * (unsigned)hh + 16u), "l"(src + 4), "r"(sz) : "memory");
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(zs_a + 1024u * (unsigned)hh + 512u), "l"(src + 4), "r"(sz) : "memory");
                 }
                 // the batch is complete when all 32 lanes' copies have landed (noinc arrivals) and the meta data are written
                 asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(full_bar) : "memory");
@@ -864,7 +937,17 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
             // (Plain st.global zero-fill from this one warp was measured at 4 B / clock - latency-throttled.)
             if (lane == 0) {
                 const unsigned wo0 = smem_u32(base + L.wo), zero_s = smem_u32(base + L.zero);
-                int ci = 0, zi = 0, zc = 0;                                  // consumer item, zero item, 4-store chunk of the zero item
+                int ci = 0, zc = 0;                                          // consumer item, 4-store chunk of the current zero item
+                // zero items are claimed one at a time from the list of chan_order_kernel, two claims ahead: z_cur is being
+                // stored, z_nxt is the next one's item id (its load in flight), z_idx the list index claimed for the one after
+                const int n_z = __ldg(P.n_cz + 1);
+                int z_cur, z_nxt, z_idx;
+                {
+                    const int i0 = atomicAdd(P.zcounter, 1), i1 = atomicAdd(P.zcounter, 1);
+                    z_idx = atomicAdd(P.zcounter, 1);
+                    z_cur = i0 < n_z ? (int)__ldg(P.z_list + i0) : -1;
+                    z_nxt = i1 < n_z ? (int)__ldg(P.z_list + i1) : -1;
+                }
                 unsigned remaining = 0xfu;                                   // block rows of consumer item ci still to store
                 long long t_so_rel = 0, t_so_idle = 0, t_so_zero = 0, t_so_all = 0;
                 (void)t_so_rel; (void)t_so_idle; (void)t_so_zero; (void)t_so_all;
@@ -877,14 +960,17 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                         __threadfence_block();
                         const unsigned word = S.c_item[ci % k6ItemRing];
                         if (word == k6ExitItem) {
-                            if (S.pub_z == zi) break;                        // every zero item was published before the exit marker
+                            if (z_cur < 0) break;                            // the zero list is exhausted as well (claims only grow)
                         } else {
                             const int X0 = (int)(word & 1023u) * k6TileX, Y0 = (int)((word >> 10) & 1023u) * k6TileY, c0 = (int)(word >> 20) * 32;
-                            const unsigned par = (unsigned)(ci & 1);
 #pragma unroll
                             for (int r = 0; r < 4; ++r) {
-                                if (((remaining >> r) & 1u) && mbar_try(smem_u32(&S.wo_full[r]), par)) {
-                                    if (Y0 + 2 * r < N) tma_store4(&map_out, wo0 + 32768u * r, X0, c0, Y0 + 2 * r, 0);
+                                // rows r and r + 2 share a slot and take turns: row r + 2 is looked at once row r is stored
+                                const unsigned par = (unsigned)((2 * ci + (r >> 1)) & 1);
+                                if (((remaining >> r) & 1u) && (r < 2 || !((remaining >> (r - 2)) & 1u)) && mbar_try(smem_u32(&S.wo_full[r & 1]), par)) {
+#ifndef K6_ABLATE_STORE
+                                    if (Y0 + 2 * r < N) tma_store4(&map_out, wo0 + 32768u * (r & 1), X0, c0, Y0 + 2 * r, 0);
+#endif
                                     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
                                     K6_TIC(s0);
                                     asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
@@ -897,16 +983,22 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                             if (remaining == 0u) { ++ci; S.done_c = ci; remaining = 0xfu; }
                         }
                     }
-                    if (S.pub_z > zi) {
+                    if (z_cur >= 0) {
                         K6_TIC(s2);
-                        __threadfence_block();
-                        const unsigned word = S.z_item[zi % k6ZeroRing];
-                        const int X0 = (int)(word & 1023u) * k6TileX, Y0 = (int)((word >> 10) & 1023u) * k6TileY, c0 = (int)(word >> 20) * 32;
+                        const int tx = z_cur % P.ntx, ty = (z_cur / P.ntx) % P.nty, grp = z_cur / (P.ntx * P.nty);
+                        const int X0 = tx * k6TileX, Y0 = ty * k6TileY, c0 = grp * 32;
                         const int pol = zc >> 1, v0 = (zc & 1) * 4;
+#ifndef K6_ABLATE_STORE
                         for (int v = v0; v < v0 + 4; ++v)
                             if (Y0 + v < N) tma_store4(&map_zero, zero_s, X0, c0, Y0 + v, pol);
+#endif
                         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-                        if (++zc == 8) { zc = 0; ++zi; S.done_z = zi; }
+                        if (++zc == 8) {
+                            zc = 0;
+                            z_cur = z_nxt;
+                            z_nxt = z_idx < n_z ? (int)__ldg(P.z_list + z_idx) : -1;
+                            z_idx = atomicAdd(P.zcounter, 1);
+                        }
                         progress = true;
                         K6_TOC(t_so_zero, s2);
                     }
@@ -996,8 +1088,13 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
     P.perm = ws.d_perm;
     P.pre = ws.d_pre;
     P.bb = (const ushort4*)ws.d_bb;
-    P.list_cap = ws.list_cap;
+    P.pool_cap = ws.pool_cap;
     P.list_cnt = ws.d_list_cnt;
+    P.list_off = ws.d_list_off;
+    P.c_desc = (const int4*)ws.d_c_desc;
+    P.z_list = ws.d_z_list;
+    P.n_cz = ws.d_misc + 14;
+    P.zcounter = ws.d_misc + 3;
     P.lists = (const uint2*)ws.d_lists;
     P.counter = ws.d_misc + 2;
     P.stats = ws.d_misc + 4;
@@ -1028,8 +1125,10 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
     {
         long long lblocks = (P.n_items + 7) / 8;
         if (lblocks > (long long)p->sm_count * 32) lblocks = (long long)p->sm_count * 32;
-        if (P.list_cap > 0)
-            chan_list_kernel<<<(unsigned)lblocks, 256, 0, st>>>(P, ws.d_list_cnt, (uint2*)ws.d_lists, P.list_cap);
+        chan_list_kernel<<<(unsigned)lblocks, 256, 0, st>>>(P, ws.d_list_cnt, ws.d_list_off, (uint2*)ws.d_lists,
+                                                            reinterpret_cast<unsigned long long*>(ws.d_misc + 12));
+        chan_order_kernel<<<1, 1024, 0, st>>>(ws.d_list_cnt, ws.d_list_off, (int)P.n_items, (int4*)ws.d_c_desc, ws.d_z_list,
+                                              ws.d_misc + 14, dispatch, 1);
     }
     const size_t smem = k6_layout(P.n_tu, P.n_tv).total;
     auto kern = w ? chanws_kernel<true> : chanws_kernel<false>;
@@ -1038,7 +1137,7 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
     long long blocks = p->sm_count;
     if (blocks > P.n_items) blocks = P.n_items;
     kern<<<(unsigned)blocks, k6Threads, smem, st>>>(P, map_out, map_zero);
-    p->last_launches += P.list_cap > 0 ? 3 : 2;
+    p->last_launches += 4;
     return cuda_ok(cudaGetLastError(), "chanws_kernel");
 }
 

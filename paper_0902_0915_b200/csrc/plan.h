@@ -35,10 +35,14 @@ struct Workspace {
     unsigned* d_pre = nullptr;       // [n_vis][ceil(n_chan / 32) * 32] packed exact indices, by row
     void* d_bb = nullptr;            // [ceil(n_chan / 32)][n_vis] ushort4 bounding boxes, by sorted position
     size_t cap_pre = 0;              // capacity in (row, padded channel) elements
-    int* d_list_cnt = nullptr;       // [n_items] hits per (16 x 8 tile, channel group) item
-    void* d_lists = nullptr;         // [n_items][list_cap] uint2 (row, mask)
-    long long cap_items = 0;         // items the two arrays above are sized for
-    int list_cap = 0;                // entries per item slot (0 = lists disabled for this problem size)
+    int* d_list_cnt = nullptr;       // [n_items] hits per (tile, channel group) item; -1 = not listed
+    unsigned* d_list_off = nullptr;  // [n_items] first entry of the item's list in the pool
+    void* d_c_desc = nullptr;        // [n_items] int4 (item, hits, list offset, 0) of the items with hits, in item order
+    unsigned* d_z_list = nullptr;    // [n_items] the items nothing reaches, in item order
+    long long cap_items = 0;         // items the four arrays above are sized for
+    void* d_lists = nullptr;         // [pool_cap] uint2 (row, mask): pool of hit lists
+    unsigned pool_cap = 0;           // entries in the pool (what this call may use)
+    size_t cap_pool = 0;             // entries allocated
     // host-buffer entry point staging
     void* d_stage = nullptr;
     size_t cap_stage = 0;

@@ -14,7 +14,7 @@ from parity import assert_parity
 
 pytestmark = pytest.mark.gpu
 C = 299792458.0
-DESIGNS = ["atomic", "smem", "romein", "gather", "chan"]
+DESIGNS = ["atomic", "smem", "romein", "gather", "chan", "chanws"]
 
 
 @pytest.fixture(scope="module")
@@ -96,6 +96,8 @@ def test_c1_whole_grid(lib, design):
     ("C4", dict(n_ant=64, core_ant=32, n_chan=16, grid_n=250)),    # grid not a multiple of the tile: ragged tail
 ])
 def test_cut_down_configs(lib, design, name, kw):
+    if design == "chanws" and CONFIGS[name].support_W > 7:
+        pytest.skip("K6's shared-memory budget holds the shifted table copies of W <= 7 kernels only (AUTO falls back to K5)")
     g = generate(scaled(CONFIGS[name], **kw))
     G, A, _ = _oracle(g)
     _to_dev(g)
@@ -115,7 +117,7 @@ def test_c3_whole(lib, design):
     assert_parity(out.cpu().numpy(), G, A, f"C3 {design}")
 
 
-@pytest.mark.parametrize("design", ["chan", "auto"])
+@pytest.mark.parametrize("design", ["chan", "chanws", "auto"])
 @pytest.mark.parametrize("kw", [
     dict(n_ant=96, core_ant=48, n_chan=70, grid_n=512),            # 3 channel groups, the last one ragged (6 channels)
     dict(n_ant=200, core_ant=100, n_chan=33, grid_n=250),          # dense core -> multi-batch tiles; ragged grid edge
@@ -130,7 +132,7 @@ def test_fine_channels_c4_shape(lib, design, kw):
     with _plan(lib, g, design) as p:
         out = p.grid(g.uv, g.freqs, g.vis, g.weights)
         torch.cuda.synchronize()
-        assert lib.mwa_grid_plan_last_design(p.handle) == "chan"
+        assert lib.mwa_grid_plan_last_design(p.handle) == ("chanws" if design == "auto" else design)
         assert_parity(out.cpu().numpy(), G, A, f"fine channels {design}")
         out2 = p.grid(g.uv, g.freqs, g.vis, None)
         assert_parity(out2.cpu().numpy(), G, A, f"fine channels {design} null weights")
@@ -144,7 +146,7 @@ def test_auto_picks_gather_for_coarse_channels(lib):
         assert lib.mwa_grid_plan_last_design(p.handle) == "gather"
 
 
-@pytest.mark.parametrize("design", ["chan", "gather"])
+@pytest.mark.parametrize("design", ["chan", "chanws", "gather"])
 def test_run_to_run_bit_identical(lib, design):
     # rows are put in a fixed order inside every uv bucket and neither product design uses atomics on grid data,
     # so two calls (and two plans) must agree bit for bit
