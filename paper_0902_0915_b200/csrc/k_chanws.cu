@@ -685,12 +685,26 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 if (lane < 4 && base + lane < n_c && base >= 0) d = __ldg(P.c_desc + base + lane);
                 return d;
             };
-            auto load_entries = [&](unsigned off, int c, int first, uint2& ea, uint2& eb) {     // list entries first + lane, first + lane + 32
+            // The list is in sorted-row order, i.e. bucket after bucket: consecutive hits fall on the same few 4 x 2 blocks and
+            // would keep a few consumer warps busy while the others wait.  It is therefore read in a fixed scattered order,
+            // position p -> entry (p * S) mod c with S ~ 0.618 c coprime to c (a low-discrepancy stride: any run of positions
+            // is spread over the whole list, hence over the whole tile).  A pure function of the list: still deterministic.
+            auto stride_of = [&](int c) -> int {
+                if (c < 16) return 1;
+                int S = (int)(((long long)c * 618) / 1000) | 1;
+                for (;; S += 2) {
+                    int a = c, b = S;
+                    while (b) { const int t = a % b; a = b; b = t; }
+                    if (a == 1) return S;
+                }
+            };
+            auto load_entries = [&](unsigned off, int c, int S, int first, uint2& ea, uint2& eb) {   // list positions first + lane, first + lane + 32
                 ea = make_uint2(0u, 0u); eb = ea;
                 if (c > 0) {
                     const uint2* src = P.lists + off;
-                    if (first + lane < c) ea = __ldg(src + first + lane);
-                    if (first + lane + 32 < c) eb = __ldg(src + first + lane + 32);
+                    const int pa = first + lane, pb = first + lane + 32;
+                    if (pa < c) ea = __ldg(src + (int)(((long long)pa * S) % c));
+                    if (pb < c) eb = __ldg(src + (int)(((long long)pb * S) % c));
                 }
             };
             K6_TIC(r2);
@@ -701,7 +715,8 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
             int raw_next = claim();
             int sub = 0;
             uint2 ea, eb;
-            load_entries((unsigned)__shfl_sync(full, d4.z, 0), __shfl_sync(full, d4.y, 0), 0, ea, eb);
+            int S_cur = stride_of(__shfl_sync(full, d4.y, 0));
+            load_entries((unsigned)__shfl_sync(full, d4.z, 0), __shfl_sync(full, d4.y, 0), S_cur, 0, ea, eb);
             while (alive && ci < n_c && ci >= 0) {
                 // ---- look ahead: the next claim's descriptors (one item after the claim was issued), the next item's entries
                 if (sub == 1) {
@@ -717,7 +732,8 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 const int c_n = valid_n ? (sub == 3 ? __shfl_sync(full, d4_n.y, 0) : __shfl_sync(full, d4.y, (sub + 1) & 3)) : 0;
                 const unsigned off_n = (unsigned)(sub == 3 ? __shfl_sync(full, d4_n.z, 0) : __shfl_sync(full, d4.z, (sub + 1) & 3));
                 uint2 ea_n, eb_n;
-                load_entries(off_n, c_n, 0, ea_n, eb_n);
+                const int S_n = stride_of(c_n);
+                load_entries(off_n, c_n, S_n, 0, ea_n, eb_n);
                 // ---- this item
                 const int tx = item % P.ntx, ty = (item / P.ntx) % P.nty, grp = item / (P.ntx * P.nty);
                 const int X0 = tx * k6TileX, Y0 = ty * k6TileY;
@@ -731,7 +747,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                         const int n_chunk = min(64, c - done);
                         const bool more = done + 64 < c;
                         uint2 fa = make_uint2(0u, 0u), fb = fa;
-                        if (more) load_entries(off, c, done + 64, fa, fb);
+                        if (more) load_entries(off, c, S_cur, done + 64, fa, fb);
                         const int nbat = (n_chunk + k6Batch - 1) / k6Batch;
                         alive = batch_slot_free(b_next + nbat - 1) && (nbat < 2 || batch_slot_free(b_next + nbat - 2));
                         if (!alive) break;
@@ -804,6 +820,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 // ---- advance
                 if (sub == 3) { sub = 0; d4 = d4_n; raw_next = claim(); } else ++sub;
                 ci = ci_n;
+                S_cur = S_n;
                 ea = ea_n; eb = eb_n;
             }
             // exit: one flagged batch per stager (consumers stop at the first one), one flagged item for the store warp
