@@ -107,8 +107,14 @@ int mwa_grid_probe_fp32(mwa_grid_plan* plan, double* out_tflops, void* stream);
  * into HOST array `out` (up to 8 values): [0] pipeline error code (0 = none; non-zero means a bounded wait inside the
  * kernel expired and the grid is incomplete), [1] work items, [2] items at least one sample reaches, [3] staged batches
  * of up to 8 hits, [4] largest number of hits of one item, [5] items whose hit list did not fit the pre-pass pool and
- * were swept inside the gridding kernel.  Returns the number of values written. */
+ * were swept inside the gridding kernel, [6] work items K5 served through its dense-tile path.  Returns the number of
+ * values written. */
 int mwa_grid_plan_last_stats(mwa_grid_plan* plan, long long* out, int n);
+
+/* Test / diagnostics: caps the pool that holds K6's per-item hit lists at `entries` list entries (0 = default sizing,
+ * 12 per (row, channel group)).  Items whose list finds no room are swept inside the gridding kernel - the same result
+ * by a slower path, which the tests reach this way.  Takes effect at the next call. */
+int mwa_grid_plan_set_list_pool(mwa_grid_plan* plan, long long entries);
 
 /* Number of kernel launches (memsets included) enqueued by the last gridding call on this plan. */
 int mwa_grid_plan_last_launches(const mwa_grid_plan* plan);

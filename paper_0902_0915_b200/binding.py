@@ -42,6 +42,8 @@ _lib.mwa_grid_plan_last_launches.argtypes = [_P]
 _lib.mwa_grid_plan_last_launches.restype = _I
 _lib.mwa_grid_plan_last_design.argtypes = [_P]
 _lib.mwa_grid_plan_last_design.restype = _I
+_lib.mwa_grid_plan_set_list_pool.argtypes = [_P, _LL]
+_lib.mwa_grid_plan_set_list_pool.restype = _I
 _lib.mwa_grid_plan_last_stats.argtypes = [_P, _P, _I]
 _lib.mwa_grid_plan_last_stats.restype = _I
 _lib.mwa_grid_probe_fp32.argtypes = [_P, _P, _P]
@@ -51,7 +53,7 @@ _lib.mwa_grid_last_error.restype = ctypes.c_char_p
 
 EXPORTS = ["mwa_grid_plan_create", "mwa_grid_plan_destroy", "mwa_grid_visibilities", "mwa_grid_visibilities_host",
            "mwa_grid_compute_indices", "mwa_grid_plan_set_design", "mwa_grid_plan_set_profiling",
-           "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_plan_last_design", "mwa_grid_plan_last_stats", "mwa_grid_probe_fp32", "mwa_grid_last_error"]
+           "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_plan_last_design", "mwa_grid_plan_last_stats", "mwa_grid_plan_set_list_pool", "mwa_grid_probe_fp32", "mwa_grid_last_error"]
 
 
 class MwaGridError(RuntimeError):
@@ -164,7 +166,12 @@ def mwa_grid_plan_last_stats(plan):
     buf = (ctypes.c_longlong * 32)()
     _check(_lib.mwa_grid_plan_last_stats(plan, ctypes.cast(buf, ctypes.c_void_p), 32))
     return {"error": int(buf[0]), "items": int(buf[1]), "items_with_hits": int(buf[2]), "batches": int(buf[3]),
-            "max_hits": int(buf[4]), "swept_items": int(buf[5]), "timing": [int(x) for x in buf[8:32]]}
+            "max_hits": int(buf[4]), "swept_items": int(buf[5]), "k5_dense_items": int(buf[6]), "timing": [int(x) for x in buf[8:32]]}
+
+
+def mwa_grid_plan_set_list_pool(plan, entries: int) -> None:
+    """Diagnostics: cap K6's hit-list pool (0 = default); overflowing items take the in-kernel sweep."""
+    _check(_lib.mwa_grid_plan_set_list_pool(plan, int(entries)))
 
 
 def mwa_grid_probe_fp32(plan, stream=None):

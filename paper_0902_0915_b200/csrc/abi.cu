@@ -105,6 +105,7 @@ static int ensure_workspace(Plan* p, long long n_vis, int n_chan) {
         long long pool = n_vis * (long long)((n_chan + 31) / 32) * 12;
         if (pool > (1LL << 27)) pool = 1LL << 27;
         if (pool < 1024) pool = 1024;
+        if (p->pool_limit > 0 && pool > p->pool_limit) pool = p->pool_limit;
         if ((size_t)pool > ws.cap_pool) {
             ws.cap_pool = 0;
             unsigned long long* l = (unsigned long long*)ws.d_lists;
@@ -277,6 +278,12 @@ int mwa_grid_probe_fp32(mwa_grid_plan* plan, double* out_tflops, void* stream) {
     if (!plan || !out_tflops) { set_error("bad argument"); return MWA_GRID_ERR_INVALID; }
     return probe_fp32(reinterpret_cast<Plan*>(plan), &out_tflops[0], &out_tflops[1], reinterpret_cast<cudaStream_t>(stream))
                ? MWA_GRID_OK : MWA_GRID_ERR_CUDA;
+}
+
+int mwa_grid_plan_set_list_pool(mwa_grid_plan* plan, long long entries) {
+    if (!plan || entries < 0) { set_error("bad argument"); return MWA_GRID_ERR_INVALID; }
+    reinterpret_cast<Plan*>(plan)->pool_limit = entries;
+    return MWA_GRID_OK;
 }
 
 int mwa_grid_plan_last_launches(const mwa_grid_plan* plan) {

@@ -94,7 +94,7 @@ bool launch_indices(Plan* p, const double* uv, long long n_vis, int n_chan, int*
     const long long total = n_vis * (long long)n_chan;
     if (total == 0) return true;
     long long blocks = (total + 255) / 256;
-    if (blocks > 148LL * 64) blocks = 148LL * 64;
+    if (blocks > (long long)p->sm_count * 64) blocks = (long long)p->sm_count * 64;
     indices_kernel<<<(unsigned)blocks, 256, 0, st>>>(p->geom, (const double2*)uv, p->ws.d_scale, n_vis, n_chan,
                                                      (int4*)out_idx);
     p->last_launches += 1;
@@ -143,7 +143,7 @@ bool launch_atomic(Plan* p, const double* uv, const float* vis, const float* w, 
     const long long total = n_vis * (long long)n_chan * p->geom.W;
     if (total == 0) return true;
     long long blocks = (total + 255) / 256;
-    if (blocks > 148LL * 32) blocks = 148LL * 32;
+    if (blocks > (long long)p->sm_count * 32) blocks = (long long)p->sm_count * 32;
     atomic_grid_kernel<<<(unsigned)blocks, 256, 0, st>>>(p->geom, (const double2*)uv, p->ws.d_scale,
                                                          (const float4*)vis, w, p->d_table, n_vis, n_chan, grid);
     p->last_launches += 1;

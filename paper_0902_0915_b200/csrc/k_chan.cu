@@ -59,6 +59,7 @@ struct ChanParams {
     const int* bucket_start;    // [nb*nb + 1]
     const double4* row_sorted;  // [n_vis] (u, v, row id, 0) of the bucket-sorted rows
     int* counter;               // work counter
+    int* stats;                 // diagnostics (mwa_grid_plan_last_stats): [6] items served by the dense path
     const int* dispatch;        // device-side design choice (AUTO): run only if *dispatch == dispatch_want; null = always
     int dispatch_want;
     const float4* vis;          // [n_vis][n_chan][2] float4
@@ -475,6 +476,7 @@ chan_kernel(const __grid_constant__ ChanParams P) {
             int n_super = 0;
             if (g_end - g_begin > 1) n_super = sweep(u_lo, u_hi, u_il, u_ih, rg, base, done);
             const bool dense = !done;                                      // list too small for the tile (or a single group)
+            if (dense && tid == 0) atomicAdd(P.stats + 6, 1);
 
             // ... F: one pass over the list selects, for every group of the super-group, the entries that reach the tile
             if (!dense) {
@@ -575,6 +577,7 @@ bool launch_chan(Plan* p, const float* vis, const float* w, long long n_vis, int
     P.bucket_start = p->ws.d_bucket_count;
     P.row_sorted = (const double4*)p->ws.d_row_sorted;
     P.counter = p->ws.d_misc + 1;
+    P.stats = p->ws.d_misc + 4;
     P.dispatch = dispatch;
     P.dispatch_want = 1;
     P.vis = (const float4*)vis;
@@ -592,12 +595,9 @@ bool launch_chan(Plan* p, const float* vis, const float* w, long long n_vis, int
     P.n_items = (int)n_items;
     const size_t smem = chan_smem_bytes(P);
     auto kern = w ? chan_kernel<true> : chan_kernel<false>;
-    static bool attr_set[2] = {false, false};
-    if (!attr_set[w ? 1 : 0]) {
-        if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024), "chan smem attribute"))
-            return false;
-        attr_set[w ? 1 : 0] = true;
-    }
+    // a per-device setting: set on every launch (cheap)
+    if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024), "chan smem attribute"))
+        return false;
     int ctas_per_sm = 0;
     if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, kcThreads, smem), "chan occupancy"))
         return false;

@@ -322,13 +322,10 @@ bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, i
     P.n_items = (long long)P.nt * P.nt * n_chan;
     const size_t tbl = ((size_t)(4 * P.rlu + 2 * P.rlv) * (p->geom.O + 1) * 4 + 15) & ~size_t(15);
     const size_t smem = tbl + sizeof(WarpSmem) * kWarpsPerCta;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (!cuda_ok(cudaFuncSetAttribute(gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024),
-                     "gather smem attribute"))
-            return false;
-        attr_set = true;
-    }
+    // a per-device setting: set on every launch (cheap), so a process that uses several GPUs gets it on each
+    if (!cuda_ok(cudaFuncSetAttribute(gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024),
+                 "gather smem attribute"))
+        return false;
     int ctas_per_sm = 0;
     if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, gather_kernel, kWarpsPerCta * 32, smem),
                  "gather occupancy"))

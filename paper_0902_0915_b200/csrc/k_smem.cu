@@ -173,11 +173,8 @@ bool launch_smem(Plan* p, const float* vis, const float* w, long long n_vis, int
     if (P.n_items >= 0x7fffffffLL) { set_error("design SMEM: too many work items"); return false; }
     const int n_tab = (p->geom.O + 1) * p->geom.W;
     const size_t smem = (size_t)4 * ksTile * ksTile * 2 * 4 + (size_t)((n_tab + 3) & ~3) * 4 + sizeof(SmemHit) * ksCap;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (!cuda_ok(cudaFuncSetAttribute(smem_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024), "smem attribute")) return false;
-        attr_set = true;
-    }
+    // a per-device setting: set on every launch (cheap)
+    if (!cuda_ok(cudaFuncSetAttribute(smem_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024), "smem attribute")) return false;
     int ctas_per_sm = 0;
     if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, smem_kernel, ksThreads, smem), "smem occupancy")) return false;
     if (ctas_per_sm < 1) { set_error("smem kernel does not fit on an SM"); return false; }

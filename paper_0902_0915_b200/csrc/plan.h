@@ -62,6 +62,7 @@ struct Plan {
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     bool ev_valid = false;
     int last_launches = 0;
+    long long pool_limit = 0;        // diagnostics: cap on K6's hit-list pool in entries (0 = default sizing)
     bool last_chanws = false;        // AUTO: the channel-SIMD kernel enqueued by the last call was K6 (else K5)
 };
 

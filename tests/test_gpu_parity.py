@@ -138,6 +138,54 @@ def test_fine_channels_c4_shape(lib, design, kw):
         assert_parity(out2.cpu().numpy(), G, A, f"fine channels {design} null weights")
 
 
+def _fine(kw):
+    cfg = scaled(CONFIGS["C4"], **kw)
+    return scaled(cfg, f_lo_hz=155e6, f_hi_hz=155e6 + 40e3 * (cfg.n_chan - 1))
+
+
+@pytest.mark.parametrize("design", ["chan", "chanws"])
+@pytest.mark.parametrize("kw", [
+    dict(n_ant=40, core_ant=20, n_chan=7 * 32 + 5, grid_n=128),    # K5: two super-groups, the second of 2 groups, last one ragged
+    dict(n_ant=40, core_ant=20, n_chan=6 * 32 + 20, grid_n=128),   # K5: the second super-group is a single ragged group (dense path)
+    dict(n_ant=24, core_ant=12, n_chan=1024 + 40, grid_n=64),      # more than 1024 channels: K5's group table moves to global memory
+])
+def test_many_channel_groups(lib, design, kw):
+    # every group / super-group decode path of the channel-SIMD kernels, compared on ALL channels
+    g = generate(_fine(kw))
+    G, A, _ = _oracle(g)
+    _to_dev(g)
+    with _plan(lib, g, design) as p:
+        out = p.grid(g.uv, g.freqs, g.vis, g.weights)
+        torch.cuda.synchronize()
+        st = lib.mwa_grid_plan_last_stats(p.handle)
+    assert st["error"] == 0
+    assert_parity(out.cpu().numpy(), G, A, f"{design} {kw}")
+    if design == "chan" and kw["n_chan"] == 6 * 32 + 20:
+        assert st["k5_dense_items"] > 0                            # the single-group super-group took the dense path
+
+
+def test_chanws_pool_overflow_takes_the_in_kernel_sweep(lib):
+    # K6 sweeps an item itself when the pre-pass pool has no room for its hit list: same grid by a slower path
+    g = generate(_fine(dict(n_ant=200, core_ant=100, n_chan=33, grid_n=250)))
+    G, A, _ = _oracle(g)
+    _to_dev(g)
+    with _plan(lib, g, "chanws") as p:
+        ref = p.grid(g.uv, g.freqs, g.vis, g.weights).clone()
+        st0 = lib.mwa_grid_plan_last_stats(p.handle)
+        assert st0["swept_items"] == 0 and st0["max_hits"] > 64 and st0["error"] == 0
+        for cap in (3000, 1):                                      # some items listed and some swept; (almost) all swept
+            lib.mwa_grid_plan_set_list_pool(p.handle, cap)
+            out = p.grid(g.uv, g.freqs, g.vis, g.weights)
+            st = lib.mwa_grid_plan_last_stats(p.handle)
+            assert st["swept_items"] > 0 and st["error"] == 0, st
+            assert_parity(out.cpu().numpy(), G, A, f"pool capped at {cap}")
+            assert st["items_with_hits"] == st0["items_with_hits"] and st["max_hits"] == st0["max_hits"]
+        lib.mwa_grid_plan_set_list_pool(p.handle, 0)
+        out = p.grid(g.uv, g.freqs, g.vis, g.weights)
+        assert torch.equal(out.view(torch.float32), ref.view(torch.float32))
+        assert lib.mwa_grid_plan_last_stats(p.handle)["swept_items"] == 0
+
+
 def test_auto_picks_gather_for_coarse_channels(lib):
     g = generate(scaled(CONFIGS["C2"], n_ant=32, n_chan=16, grid_n=256))     # 16 channels over 140-170 MHz
     _to_dev(g)
@@ -171,10 +219,17 @@ def test_dense_tile_many_calls_on_one_plan(lib):
     g = generate(cfg)
     G, A, _ = _oracle(g)
     _to_dev(g)
-    with _plan(lib, g, "auto") as p:
-        for k in range(12):
-            out = p.grid(g.uv, g.freqs, g.vis, g.weights if k % 3 == 0 else None)
-            assert_parity(out.cpu().numpy(), G, A, f"dense tile, call {k}")
+    for design in ("auto", "chan"):
+        with _plan(lib, g, design) as p:
+            for k in range(12):
+                out = p.grid(g.uv, g.freqs, g.vis, g.weights if k % 3 == 0 else None)
+                assert_parity(out.cpu().numpy(), G, A, f"dense tile, {design}, call {k}")
+            st = lib.mwa_grid_plan_last_stats(p.handle)
+            assert st["error"] == 0
+            if design == "chan":
+                assert st["k5_dense_items"] > 0                    # K5 really took its dense-tile path
+            else:
+                assert st["max_hits"] > 14 * 8                     # K6: items longer than the whole staging ring
 
 
 def test_chan_wide_kernel_repeated_calls(lib):
@@ -270,30 +325,58 @@ def test_plan_reuse_changing_sizes(lib):
             assert_parity(out.cpu().numpy(), G, A, "reuse")
 
 
-# ---------------------------------------------------------------------------- full-size configs, sampled channels
-def _full_size_sampled(lib, name, chans):
-    g = generate(CONFIGS[name], device="cuda")
+# ---------------------------------------------------------------------------- full-size configs
+def _indices_sampled(lib, p, g, chans):
     cfg = g.cfg
+    idx = p.indices(g.uv, g.freqs[chans].contiguous()).cpu().numpy()
+    want_idx = oracle.compute_indices(g.uv.cpu(), g.freqs[chans].cpu(), cfg.grid_n, g.cell_du, cfg.support_W,
+                                      cfg.oversample_O)
+    assert np.array_equal(idx, want_idx)
+
+
+def test_c4_full_size_all_channels_and_run_to_run(lib):
+    """The bench configuration, every one of the 768 channel grids compared with the oracle element by element (16
+    channels at a time), every cell written, and the whole 25.8 GB grid bit-identical over repeated calls - with the
+    deterministic hit order that is a whole-grid race detector."""
+    g = generate(CONFIGS["C4"], device="cuda")
+    cfg = g.cfg
+    shape = (cfg.n_chan, 4, cfg.grid_n, cfg.grid_n)
+    with _plan(lib, g) as p:
+        out = torch.empty(shape, dtype=torch.complex64, device="cuda")
+        out.fill_(float("nan"))
+        lib.mwa_grid_visibilities(p.handle, g.uv, g.freqs, g.vis, g.weights, cfg.n_vis, cfg.n_chan, out)
+        torch.cuda.synchronize()
+        assert lib.mwa_grid_plan_last_design(p.handle) == "chanws"
+        st = lib.mwa_grid_plan_last_stats(p.handle)
+        assert st["error"] == 0 and st["swept_items"] == 0, st
+        assert not bool(torch.isnan(out.view(torch.float32)).any())          # every cell of every plane was written
+        _indices_sampled(lib, p, g, [0, 383, 767])
+        again = torch.empty(shape, dtype=torch.complex64, device="cuda")
+        for k in range(5):
+            again.fill_(float("nan"))
+            lib.mwa_grid_visibilities(p.handle, g.uv, g.freqs, g.vis, g.weights, cfg.n_vis, cfg.n_chan, again)
+            assert torch.equal(out.view(torch.float32), again.view(torch.float32)), f"call {k} differs"
+        del again
+    worst = {"max_ratio": 0.0, "frob": 0.0}
+    for c0 in range(0, cfg.n_chan, 16):
+        ch = list(range(c0, min(c0 + 16, cfg.n_chan)))
+        G, A, _ = _oracle(g, ch)
+        r = assert_parity(out[c0:c0 + len(ch)].cpu().numpy(), G, A, f"C4 channels {c0}..{ch[-1]}")
+        worst = {k: max(worst[k], r[k]) for k in worst}
+    print("C4 full size, all channels:", worst)
+
+
+def test_c5_full_size_sampled_channels(lib):
+    g = generate(CONFIGS["C5"], device="cuda")
+    cfg = g.cfg
+    chans = [0, 31, 63]
     with _plan(lib, g) as p:
         out = torch.empty((cfg.n_chan, 4, cfg.grid_n, cfg.grid_n), dtype=torch.complex64, device="cuda")
         out.fill_(float("nan"))
         lib.mwa_grid_visibilities(p.handle, g.uv, g.freqs, g.vis, g.weights, cfg.n_vis, cfg.n_chan, out)
         torch.cuda.synchronize()
-        idx = p.indices(g.uv, g.freqs[chans].contiguous()).cpu().numpy()
-    want_idx = oracle.compute_indices(g.uv.cpu(), g.freqs[chans].cpu(), cfg.grid_n, g.cell_du, cfg.support_W,
-                                      cfg.oversample_O)
-    assert np.array_equal(idx, want_idx)
-    assert not bool(torch.isnan(out.real).any())                   # every cell of every plane was written
+        _indices_sampled(lib, p, g, chans)
+    assert not bool(torch.isnan(out.view(torch.float32)).any())              # every cell of every plane was written
     for c in chans:
         G, A, _ = _oracle(g, [c])
-        assert_parity(out[c:c + 1].cpu().numpy(), G, A, f"{name} channel {c}")
-    # flux conservation per channel at full size: sum over cells = sum_n w V S(ru) S(rv)  (pin P3 restated for the GPU)
-    return g, out
-
-
-def test_c4_full_size_sampled_channels(lib):
-    _full_size_sampled(lib, "C4", [0, 383, 767])
-
-
-def test_c5_full_size_sampled_channels(lib):
-    _full_size_sampled(lib, "C5", [0, 63])
+        assert_parity(out[c:c + 1].cpu().numpy(), G, A, f"C5 channel {c}")
