@@ -76,7 +76,7 @@ static int ensure_workspace(Plan* p, long long n_vis, int n_chan) {
         if (!ensure(ws.d_tile_weight, (size_t)n_tiles, "tile_weight")) return MWA_GRID_ERR_NOMEM;
         ws.cap_tiles = n_tiles;
     }
-    if (!ws.d_misc && !ensure(ws.d_misc, 4096 + 16, "misc")) return MWA_GRID_ERR_NOMEM;
+    if (!ws.d_misc && !ensure(ws.d_misc, (size_t)kMiscInts, "misc")) return MWA_GRID_ERR_NOMEM;
     const bool want_ws = (p->design == MWA_GRID_DESIGN_CHANWS || p->design == MWA_GRID_DESIGN_AUTO) && chanws_supported(p, n_chan);
     const size_t n_pre = want_ws ? (size_t)n_vis * (size_t)((n_chan + 31) / 32) * 32 : 0;
     if (n_pre > ws.cap_pre) {

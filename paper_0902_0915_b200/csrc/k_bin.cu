@@ -156,7 +156,7 @@ bool launch_binning(Plan* p, const double* uv, long long n_vis, int /*n_chan*/, 
     const int nt = (p->geom.N + kTile - 1) / kTile;
     if (!cuda_ok(cudaMemsetAsync(ws.d_bucket_count, 0, ((size_t)n_buckets + 1) * sizeof(int), st), "memset buckets"))
         return false;
-    if (!cuda_ok(cudaMemsetAsync(ws.d_misc, 0, (4096 + 16) * sizeof(int), st), "memset misc")) return false;
+    if (!cuda_ok(cudaMemsetAsync(ws.d_misc, 0, (size_t)kMiscInts * sizeof(int), st), "memset misc")) return false;
     int blocks = (int)((n_vis + 255) / 256);
     if (blocks > p->sm_count * 8) blocks = p->sm_count * 8;
     bin_count_kernel<<<blocks, 256, 0, st>>>(p->geom, (const double2*)uv, ws.d_scale_ref, (int)n_vis, nb,

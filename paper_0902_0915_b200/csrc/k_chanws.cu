@@ -41,8 +41,14 @@ namespace mwa {
 constexpr int k6Consumers = 16;                       // consumer warps
 constexpr int k6Threads = (k6Consumers + 4) * 32;     // + sweeper, two stagers, store warp
 constexpr int k6TileX = 16, k6TileY = 8;
-constexpr int k6Batch = 8;                            // hits per batch
-constexpr int k6Stages = 14;                          // batches in flight (even: every stager keeps its own stages)
+#ifndef K6_BATCH
+#define K6_BATCH 16
+#endif
+#ifndef K6_STAGES
+#define K6_STAGES 6
+#endif
+constexpr int k6Batch = K6_BATCH;                     // hits per batch
+constexpr int k6Stages = K6_STAGES;                   // batches in flight: 6 x 16 hits (measured on C4: 8 x 8 9.43 ms, 14 x 8 8.44, 7 x 16 8.37, 6 x 16 8.34, 28 x 4 9.8)
 constexpr int k6Stagers = 2;                          // stager warps; batch b is staged by stager b % 2 into stage b % 4
 constexpr int k6BatchRing = 32;                       // batch descriptors / queue segments between sweeper and stagers
 constexpr int k6ItemRing = 16;                        // consumer-item descriptors between sweeper and store warp
@@ -188,9 +194,26 @@ __device__ __forceinline__ void bulk_load(unsigned dst, const void* src, unsigne
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
-__device__ __forceinline__ void tma_store4(const CUtensorMap* m, unsigned src, int d0, int d1, int d2, int d3) {
+// The grid is written once and never read again by this kernel: its lines are marked evict-first in L2, so the 25.8 GB
+// write stream does not push the visibilities (re-read by the 2 - 3 tiles a stamp reaches) out of the cache.
+__device__ __forceinline__ u64 l2_policy_evict_first() {
+    u64 p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ u64 l2_policy_evict_last() {
+    u64 p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void tma_store4(const CUtensorMap* m, unsigned src, int d0, int d1, int d2, int d3, u64 policy) {
+#ifdef K6_NO_L2_HINTS
     asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group [%0, {%1, %2, %3, %4}], [%5];"
                  ::"l"(m), "r"(d0), "r"(d1), "r"(d2), "r"(d3), "r"(src) : "memory");
+#else
+    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%1, %2, %3, %4}], [%5], %6;"
+                 ::"l"(m), "r"(d0), "r"(d1), "r"(d2), "r"(d3), "r"(src), "l"(policy) : "memory");
+#endif
 }
 __device__ __forceinline__ void k6_unpack2(u64 v, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
 __device__ __forceinline__ u64 k6_pack2(float a, float b) {
@@ -201,7 +224,7 @@ __device__ __forceinline__ u64 k6_pack2(float a, float b) {
 __device__ __forceinline__ void k6_ffma2(u64& d, u64 a, u64 b) { asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(a), "l"(b)); }
 
 // ------------------------------------------------------------------------------------------------ pre-pass
-// One warp per (sorted row r, channel group g), lane = channel.  With origin = i - h (the first cell of the stamp):
+// One warp per sorted row r, walking the channel groups g, lane = channel.  With origin = i - h (the first cell of the stamp):
 //   bb[g][r]   = (min origin_u, max origin_u | slow << 15, min origin_v, max origin_v) over the valid lanes; a group with
 //                no valid lane gets min = 0x7fff, which no tile reaches.
 //   pre[row][c], fast (row, group): the lane's table offsets with the tile term left out,
@@ -218,39 +241,41 @@ chan_index_kernel(GridGeom g, const double4* __restrict__ row_sorted, const doub
                   const int* __restrict__ dispatch, int dispatch_want) {
     if (dispatch != nullptr && *dispatch != dispatch_want) return;
     const int lane = threadIdx.x & 31;
-    const long long warps = ((long long)gridDim.x * blockDim.x) >> 5;
-    const long long tasks = (long long)n_vis * n_groups;
+    const int warps = (int)(((long long)gridDim.x * blockDim.x) >> 5);
     const int ncp = n_groups * 32, O1 = g.O + 1;
-    for (long long t = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5; t < tasks; t += warps) {
-        const int grp = (int)(t / n_vis), r = (int)(t - (long long)grp * n_vis);
+    const unsigned full = 0xffffffffu;
+    // a warp takes a sorted row and walks its channel groups (the row record is loaded once, no task division)
+    for (int r = (int)(((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5); r < n_vis; r += warps) {
         const double4 rec = row_sorted[r];
-        const int c = grp * 32 + lane;
-        const bool cvalid = c < n_chan;
-        const double sc = scale[cvalid ? c : n_chan - 1];
-        SampleIndex s;
-        const bool ok = sample_index(rec.x, rec.y, sc, g, s) && cvalid;
-        const int ou = s.iu - g.h, ov = s.iv - g.h;
-        const unsigned full = 0xffffffffu;
-        const unsigned u_min = __reduce_min_sync(full, ok ? (unsigned)ou : 0x7fffu);
-        const unsigned u_max = __reduce_max_sync(full, ok ? (unsigned)ou : 0u);
-        const unsigned v_min = __reduce_min_sync(full, ok ? (unsigned)ov : 0x7fffu);
-        const unsigned v_max = __reduce_max_sync(full, ok ? (unsigned)ov : 0u);
-        const bool slow = __ballot_sync(full, cvalid && !ok) != 0u || u_max > u_min + k6Drift || v_max > v_min + k6Drift ||
-                          grp * 32 + 32 > n_chan;                      // a ragged last group is staged lane by lane as well
-        unsigned word = k6Invalid;
-        if (ok) {
-            if (slow) word = (unsigned)ou | ((unsigned)s.ru << 11) | ((unsigned)ov << 16) | ((unsigned)s.rv << 27);
-            else {
-                const int su = (k6PadU - ou) & 3, sv = (k6PadV - ov) & 1;
-                const int lo = s.ru * rlu + su * (O1 * rlu - 1) + k6PadU + k6Bias - ou;
-                const int hi = s.rv * rlv + sv * (O1 * rlv - 1) + k6PadV + k6Bias - ov;
-                word = (unsigned)(lo * 4) | ((unsigned)(hi * 4) << 16);
+        unsigned* pre_row = pre + (size_t)(int)rec.z * ncp;
+        for (int grp = 0; grp < n_groups; ++grp) {
+            const int c = grp * 32 + lane;
+            const bool cvalid = c < n_chan;
+            const double sc = __ldg(scale + (cvalid ? c : n_chan - 1));
+            SampleIndex s;
+            const bool ok = sample_index(rec.x, rec.y, sc, g, s) && cvalid;
+            const int ou = s.iu - g.h, ov = s.iv - g.h;
+            const unsigned u_min = __reduce_min_sync(full, ok ? (unsigned)ou : 0x7fffu);
+            const unsigned u_max = __reduce_max_sync(full, ok ? (unsigned)ou : 0u);
+            const unsigned v_min = __reduce_min_sync(full, ok ? (unsigned)ov : 0x7fffu);
+            const unsigned v_max = __reduce_max_sync(full, ok ? (unsigned)ov : 0u);
+            const bool slow = __ballot_sync(full, cvalid && !ok) != 0u || u_max > u_min + k6Drift || v_max > v_min + k6Drift ||
+                              grp * 32 + 32 > n_chan;                  // a ragged last group is staged lane by lane as well
+            unsigned word = k6Invalid;
+            if (ok) {
+                if (slow) word = (unsigned)ou | ((unsigned)s.ru << 11) | ((unsigned)ov << 16) | ((unsigned)s.rv << 27);
+                else {
+                    const int su = (k6PadU - ou) & 3, sv = (k6PadV - ov) & 1;
+                    const int lo = s.ru * rlu + su * (O1 * rlu - 1) + k6PadU + k6Bias - ou;
+                    const int hi = s.rv * rlv + sv * (O1 * rlv - 1) + k6PadV + k6Bias - ov;
+                    word = (unsigned)(lo * 4) | ((unsigned)(hi * 4) << 16);
+                }
             }
+            pre_row[c] = word;
+            if (lane == 0)
+                bb[(size_t)grp * n_vis + r] = make_ushort4((unsigned short)u_min, (unsigned short)(u_max | (slow ? 0x8000u : 0u)),
+                                                            (unsigned short)v_min, (unsigned short)v_max);
         }
-        pre[(size_t)(int)rec.z * ncp + c] = word;
-        if (lane == 0)
-            bb[(size_t)grp * n_vis + r] = make_ushort4((unsigned short)u_min, (unsigned short)(u_max | (slow ? 0x8000u : 0u)),
-                                                        (unsigned short)v_min, (unsigned short)v_max);
     }
 }
 
@@ -391,48 +416,76 @@ chan_list_kernel(const __grid_constant__ K6Params P, int* __restrict__ list_cnt,
     }
 }
 
-// Third pre-pass, one block: splits the items into those with hits (c_desc: item, hit count, list offset - what the
-// sweeper of chanws_kernel claims, four at a time) and those nothing reaches (z_list - what its zero feeder claims), both
-// in item order, so neighbouring tiles are still worked on at about the same time and share their halo rows in L2.
+// Third pre-pass: splits the items into those with hits (c_desc: item, hit count, list offset - what the sweeper of
+// chanws_kernel claims, four at a time) and those nothing reaches (z_list - what its store warp claims), both in item
+// order, so neighbouring tiles are still worked on at about the same time and share their halo rows in L2.
+// A block takes `per_block` consecutive items, publishes its number of items with hits in blk_state (zeroed by the
+// call's memset; flag bit 30) and sums the counts of the blocks before it (they were scheduled before it, so the wait
+// cannot deadlock) - a one-level decoupled scan, enough for the <= 2048 blocks the launcher uses.
+constexpr int k6OrderBlocksMax = 2048;
+constexpr int k6OrderFlag = 1 << 30;
+
 __global__ void __launch_bounds__(1024)
-chan_order_kernel(const int* __restrict__ list_cnt, const unsigned* __restrict__ list_off, int n_items, int4* __restrict__ c_desc,
-                  unsigned* __restrict__ z_list, int* __restrict__ n_cz, const int* __restrict__ dispatch, int dispatch_want) {
+chan_order_kernel(const int* __restrict__ list_cnt, const unsigned* __restrict__ list_off, int n_items, int per_block,
+                  int4* __restrict__ c_desc, unsigned* __restrict__ z_list, int* __restrict__ n_cz, volatile int* blk_state,
+                  const int* __restrict__ dispatch, int dispatch_want) {
     if (dispatch != nullptr && *dispatch != dispatch_want) return;
-    __shared__ int s_tot[32], s_base[32];
+    __shared__ int s_warp[32];
+    __shared__ int s_prefix;
     const unsigned full = 0xffffffffu;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int chunk = (((n_items + 31) / 32 + 31) / 32) * 32;             // items per warp, a multiple of 32
-    const int i0 = warp * chunk, i1 = min(n_items, i0 + chunk);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int b = blockIdx.x;
+    const int i0 = min(n_items, b * per_block), i1 = min(n_items, i0 + per_block);
     int nz = 0;
-    for (int i = i0 + lane; i < i1; i += 32) nz += list_cnt[i] != 0 ? 1 : 0;
+    for (int i = i0 + tid; i < i1; i += 1024) nz += list_cnt[i] != 0 ? 1 : 0;
     nz = __reduce_add_sync(full, nz);
-    if (lane == 0) s_tot[warp] = nz;
+    if (lane == 0) s_warp[warp] = nz;
     __syncthreads();
     if (warp == 0) {
-        const int t = s_tot[lane];
+        const int total = __reduce_add_sync(full, s_warp[lane]);
+        if (lane == 0) blk_state[b] = total | k6OrderFlag;
+        int sum = 0;
+        for (int j0 = 0; j0 < b; j0 += 32) {
+            const int j = j0 + lane;
+            int v = 0;
+            if (j < b) {
+                do { v = blk_state[j]; } while (!(v & k6OrderFlag));
+                v &= ~k6OrderFlag;
+            }
+            sum += v;
+        }
+        sum = __reduce_add_sync(full, sum);
+        if (lane == 0) {
+            s_prefix = sum;
+            if (b == (int)gridDim.x - 1) { n_cz[0] = sum + total; n_cz[1] = n_items - (sum + total); }
+        }
+    }
+    __syncthreads();
+    int cb = s_prefix;                                               // items with hits before the current chunk
+    const unsigned lt_mask = (1u << lane) - 1u;
+    for (int s0 = i0; s0 < i1; s0 += 1024) {
+        const int i = s0 + tid;
+        const bool valid = i < i1;
+        const int cnt = valid ? list_cnt[i] : 0;
+        const unsigned bm = __ballot_sync(full, valid && cnt != 0);
+        __syncthreads();                                             // s_warp is free again
+        if (lane == 0) s_warp[warp] = __popc(bm);
+        __syncthreads();
+        const int t = s_warp[lane];
         int incl = t;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const int u = __shfl_up_sync(full, incl, o);
             if (lane >= o) incl += u;
         }
-        s_base[lane] = incl - t;
-        if (lane == 31) { n_cz[0] = incl; n_cz[1] = n_items - incl; }
-    }
-    __syncthreads();
-    int cb = s_base[warp], zb = min(i0, n_items) - cb;
-    const unsigned lt_mask = (1u << lane) - 1u;
-    for (int s0 = i0; s0 < i1; s0 += 32) {
-        const int i = s0 + lane;
-        const bool valid = i < i1;
-        const int cnt = valid ? list_cnt[i] : 0;
-        const unsigned bm = __ballot_sync(full, valid && cnt != 0), vm = __ballot_sync(full, valid);
+        const int before = __shfl_sync(full, incl - t, warp);        // items with hits in the warps before this one
+        const int chunk_total = __shfl_sync(full, incl, 31);
         if (valid) {
-            if (cnt != 0) c_desc[cb + __popc(bm & lt_mask)] = make_int4(i, cnt, (int)list_off[i], 0);
-            else z_list[zb + __popc(vm & ~bm & lt_mask)] = (unsigned)i;
+            const int cpos = cb + before + __popc(bm & lt_mask);     // items with hits before item i
+            if (cnt != 0) c_desc[cpos] = make_int4(i, cnt, (int)list_off[i], 0);
+            else z_list[i - cpos] = (unsigned)i;
         }
-        cb += __popc(bm);
-        zb += __popc(vm & ~bm);
+        cb += chunk_total;
     }
 }
 
@@ -860,6 +913,8 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
             // (Per-lane bulk copies, cp.async.bulk = UBLKCP, were measured first: they are issued one lane at a time at
             // ~60 ns each, 6.4 us per 32-hit batch.)
             const int sg = role - 1;                                        // this stager stages batches b = sg, sg + 2, ...
+            const u64 pol_last = l2_policy_evict_last();
+            (void)pol_last;
             const unsigned zero_geo = (unsigned)(P.n_tu * 4) | ((unsigned)(P.n_tv * 4) << 16);
             const int ncp = P.n_groups * 32;
             long long t_st_pub = 0, t_st_empty = 0, t_st_work = 0, t_st_pre = 0, n_st = 0;
@@ -901,8 +956,13 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                     asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(geo_a + 128u * (unsigned)hh), "l"(P.pre + (size_t)r * ncp + c0 + lane) : "memory");
 #ifndef K6_ABLATE_LOAD
                     const float* src = P.vis + ((size_t)r * P.n_chan + cc) * 8;
+#if defined(K6_NO_L2_HINTS) || !defined(K6_VIS_EVICT_LAST)
                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(zs_a + 1024u * (unsigned)hh), "l"(src) : "memory");
                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(zs_a + 1024u * (unsigned)hh + 512u), "l"(src + 4) : "memory");
+#else
+                    asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(zs_a + 1024u * (unsigned)hh), "l"(src), "l"(pol_last) : "memory");
+                    asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(zs_a + 1024u * (unsigned)hh + 512u), "l"(src + 4), "l"(pol_last) : "memory");
+#endif
 #endif
                 }
                 for (unsigned sm_ = slow_m; sm_ != 0u; sm_ &= sm_ - 1u) {   // slow hits: packed (origin, table row) words, range-checked here
@@ -954,6 +1014,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
             // (Plain st.global zero-fill from this one warp was measured at 4 B / clock - latency-throttled.)
             if (lane == 0) {
                 const unsigned wo0 = smem_u32(base + L.wo), zero_s = smem_u32(base + L.zero);
+                const u64 pol_first = l2_policy_evict_first();
                 int ci = 0, zc = 0;                                          // consumer item, 4-store chunk of the current zero item
                 // zero items are claimed one at a time from the list of chan_order_kernel, two claims ahead: z_cur is being
                 // stored, z_nxt is the next one's item id (its load in flight), z_idx the list index claimed for the one after
@@ -986,7 +1047,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                                 const unsigned par = (unsigned)((2 * ci + (r >> 1)) & 1);
                                 if (((remaining >> r) & 1u) && (r < 2 || !((remaining >> (r - 2)) & 1u)) && mbar_try(smem_u32(&S.wo_full[r & 1]), par)) {
 #ifndef K6_ABLATE_STORE
-                                    if (Y0 + 2 * r < N) tma_store4(&map_out, wo0 + 32768u * (r & 1), X0, c0, Y0 + 2 * r, 0);
+                                    if (Y0 + 2 * r < N) tma_store4(&map_out, wo0 + 32768u * (r & 1), X0, c0, Y0 + 2 * r, 0, pol_first);
 #endif
                                     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
                                     K6_TIC(s0);
@@ -1007,7 +1068,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                         const int pol = zc >> 1, v0 = (zc & 1) * 4;
 #ifndef K6_ABLATE_STORE
                         for (int v = v0; v < v0 + 4; ++v)
-                            if (Y0 + v < N) tma_store4(&map_zero, zero_s, X0, c0, Y0 + v, pol);
+                            if (Y0 + v < N) tma_store4(&map_zero, zero_s, X0, c0, Y0 + v, pol, pol_first);
 #endif
                         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
                         if (++zc == 8) {
@@ -1133,9 +1194,8 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
     if (!make_grid_map(&map_out, grid, p->geom.N, n_chan, 2, 4, true)) return false;
     if (!make_grid_map(&map_zero, grid, p->geom.N, n_chan, 1, 1, false)) return false;
 
-    long long tasks = n_vis * (long long)P.n_groups;
-    long long iblocks = (tasks + 7) / 8;
-    if (iblocks > (long long)p->sm_count * 16) iblocks = (long long)p->sm_count * 16;
+    long long iblocks = (n_vis + 7) / 8;                                      // one warp per sorted row at a time
+    if (iblocks > (long long)p->sm_count * 8) iblocks = (long long)p->sm_count * 8;
     if (iblocks < 1) iblocks = 1;
     chan_index_kernel<<<(unsigned)iblocks, 256, 0, st>>>(p->geom, (const double4*)ws.d_row_sorted, ws.d_scale, (int)n_vis, n_chan,
                                                          P.n_groups, P.rlu, P.rlv, ws.d_pre, (ushort4*)ws.d_bb, dispatch, 1);
@@ -1144,8 +1204,10 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
         if (lblocks > (long long)p->sm_count * 32) lblocks = (long long)p->sm_count * 32;
         chan_list_kernel<<<(unsigned)lblocks, 256, 0, st>>>(P, ws.d_list_cnt, ws.d_list_off, (uint2*)ws.d_lists,
                                                             reinterpret_cast<unsigned long long*>(ws.d_misc + 12));
-        chan_order_kernel<<<1, 1024, 0, st>>>(ws.d_list_cnt, ws.d_list_off, (int)P.n_items, (int4*)ws.d_c_desc, ws.d_z_list,
-                                              ws.d_misc + 14, dispatch, 1);
+        int per_block = (int)(((P.n_items + k6OrderBlocksMax - 1) / k6OrderBlocksMax + 1023) / 1024) * 1024;
+        const int oblocks = (int)((P.n_items + per_block - 1) / per_block);
+        chan_order_kernel<<<oblocks, 1024, 0, st>>>(ws.d_list_cnt, ws.d_list_off, (int)P.n_items, per_block, (int4*)ws.d_c_desc,
+                                                    ws.d_z_list, ws.d_misc + 14, ws.d_misc + kMiscOrderState, dispatch, 1);
     }
     const size_t smem = k6_layout(P.n_tu, P.n_tv).total;
     auto kern = w ? chanws_kernel<true> : chanws_kernel<false>;

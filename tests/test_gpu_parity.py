@@ -229,7 +229,7 @@ def test_dense_tile_many_calls_on_one_plan(lib):
             if design == "chan":
                 assert st["k5_dense_items"] > 0                    # K5 really took its dense-tile path
             else:
-                assert st["max_hits"] > 14 * 8                     # K6: items longer than the whole staging ring
+                assert st["max_hits"] > 6 * 16                     # K6: items longer than the whole staging ring
 
 
 def test_chan_wide_kernel_repeated_calls(lib):
