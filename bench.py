@@ -138,15 +138,17 @@ def run_ours(args):
     ws, rank, lr = _dist()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
-    from paper_0902_0915_b200 import _build
-    if rank == 0:
-        _build.build()                            # no-op when the in-tree library is newer than its sources
-    import paper_0902_0915_b200 as lib
     torch.cuda.set_device(lr)
     dist = None
     if ws > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", lr))
+    # importing the package builds the library when it is stale: rank 0 does that alone, the others import afterwards
+    if rank == 0:
+        import paper_0902_0915_b200 as lib
+    if dist is not None:
+        dist.barrier()
+    import paper_0902_0915_b200 as lib
     cfg = CONFIGS[args.config]
     if args.n_chan:                               # profiling subset (ncu captures): same rows, the TOP n channels
         from gen import scaled                    # of the band at the config's own channel spacing (same du)
@@ -252,7 +254,10 @@ def run_ours(args):
         "kernel_tap_updates_per_sec": value * cfg.support_W ** 2,
         "stage_ms": {"scale_and_binning": bin_ms, "gridding": grid_ms},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None, "peak_source": peak_src, "kernel": {"gather": "gather_kernel", "chan": "chan_kernel", "atomic": "atomic_grid_kernel"}.get(ran, ran),
+                     "traffic": None, "peak_source": peak_src, "kernel": {"gather": "gather_kernel", "chan": "chan_kernel", "chanws": "chanws_kernel", "atomic": "atomic_grid_kernel",
+                                "smem": "smem_kernel", "romein": "romein_kernel"}.get(ran, ran),
+                     "frac_is": "algorithmic bytes / time of the gridding stage (index + list pre-passes and the gridding kernel; "
+                                "CUDA events recorded by the library) / peak; whole_call_frac adds scale + binning",
                      "algorithmic_bytes_per_launch": alg_bytes,
                      "whole_call_frac": alg_bytes / (ms_per_step * 1e-3) / 1e9 / peak,
                      "fp32_peak_tflops_measured": {"fma.rn.f32": fp32_ffma, "fma.rn.f32x2": fp32_ffma2},
@@ -316,6 +321,15 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # not under torchrun: launch the ranks the way the driver does and hand over
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
     if args.impl == "reference":
         run_reference(args)
     else:

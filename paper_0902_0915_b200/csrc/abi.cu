@@ -96,7 +96,7 @@ static int ensure_workspace(Plan* p, long long n_vis, int n_chan) {
             ws.cap_items = 0;
             if (!ensure(ws.d_list_cnt, (size_t)items, "hit counts")) return MWA_GRID_ERR_NOMEM;
             if (!ensure(ws.d_list_off, (size_t)items, "hit list offsets")) return MWA_GRID_ERR_NOMEM;
-            if (!ensure(ws.d_z_list, (size_t)items, "zero item list")) return MWA_GRID_ERR_NOMEM;
+            if (!ensure(ws.d_z_list, (size_t)items + 16, "zero item list")) return MWA_GRID_ERR_NOMEM;   // read 16 at a time
             int4* cd = (int4*)ws.d_c_desc;
             if (!ensure(cd, (size_t)items, "item descriptors")) { ws.d_c_desc = cd; return MWA_GRID_ERR_NOMEM; }
             ws.d_c_desc = cd;

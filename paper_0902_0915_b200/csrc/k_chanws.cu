@@ -41,6 +41,9 @@ namespace mwa {
 constexpr int k6Consumers = 16;                       // consumer warps
 constexpr int k6Threads = (k6Consumers + 4) * 32;     // + sweeper, two stagers, store warp
 constexpr int k6TileX = 16, k6TileY = 8;
+#ifndef K6_ZERO_LEAD_PCT
+#define K6_ZERO_LEAD_PCT 5
+#endif
 #ifndef K6_BATCH
 #define K6_BATCH 16
 #endif
@@ -52,6 +55,7 @@ constexpr int k6Stages = K6_STAGES;                   // batches in flight: 6 x 
 constexpr int k6Stagers = 2;                          // stager warps; batch b is staged by stager b % 2 into stage b % 4
 constexpr int k6BatchRing = 32;                       // batch descriptors / queue segments between sweeper and stagers
 constexpr int k6ItemRing = 16;                        // consumer-item descriptors between sweeper and store warp
+constexpr int k6ZeroChunk = 16;                       // zero items per claim of the store warp
 constexpr unsigned k6ExitItem = 0xffffffffu;
 constexpr int k6Drift = 8;                            // largest spread (cells) of the stamp origins over the 32 channels of a fast hit
 constexpr int k6PadU = 15 + k6Drift + 1, k6PadV = 7 + k6Drift + 1;   // zero padding in front of a table row (floats)
@@ -61,7 +65,8 @@ constexpr int k6WoSlots = 2;                          // write-out stage slots; 
 constexpr int k6WoBytes = k6WoSlots * 32768;          // write-out stage: slots of [pol 4][v 2][chan 32][128 B]
 constexpr int k6StageV = k6Batch * 1024, k6StageGeo = k6Batch * 128, k6StageW = k6Batch * 128;
 constexpr int k6StageBytes = k6StageV + k6StageGeo + k6StageW;
-constexpr int k6ZeroBytes = 4096;                     // zero buffer: [chan 32][128 B]
+constexpr int k6ZeroV = 4;                            // rows of a zero-fill box
+constexpr int k6ZeroBytes = k6ZeroV * 4096;           // zero buffer: [v 4][chan 32][128 B]
 constexpr unsigned k6FlagEnd = 1u, k6FlagExit = 2u;
 constexpr unsigned k6Invalid = 0xffffffffu;           // packed index of a dropped sample
 constexpr long long k6SpinLimit = 6000000000LL;       // ~3 s of SM clocks: a wait this long is a bug -> abort, never hang
@@ -112,8 +117,10 @@ struct K6Ctrl {
     int b_x0[k6BatchRing], b_y0[k6BatchRing], b_g[k6BatchRing];
     unsigned c_item[k6ItemRing];                            // consumer items in order: tx | ty << 10 | group << 20, k6ExitItem = exit
     volatile int pub_batches, pub_c, done_c;
+    volatile int c_pos;                                     // sweeper: index (in the global list of items with hits) of the item it is on
     volatile int done_batches[k6Stagers];
     volatile int abort;
+    alignas(16) int z_ids[k6ZeroChunk];                     // store warp: the zero items of its current claim
     int stat_hit_items, stat_max_hits, stat_swept_items;    // sweeper's counters for mwa_grid_plan_last_stats
 };
 
@@ -779,6 +786,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                     d4_n = load_desc(base_n);
                 }
                 const int item = __shfl_sync(full, d4.x, sub), c = __shfl_sync(full, d4.y, sub);
+                if (lane == 0) S.c_pos = ci;
                 const unsigned off = (unsigned)__shfl_sync(full, d4.z, sub);
                 const int ci_n = sub == 3 ? base_n : ci + 1;
                 const bool valid_n = ci_n < n_c && ci_n >= 0;
@@ -876,6 +884,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 S_cur = S_n;
                 ea = ea_n; eb = eb_n;
             }
+            if (lane == 0) S.c_pos = n_c;                    // nothing left to claim: the store warp may zero-fill at full speed
             // exit: one flagged batch per stager (consumers stop at the first one), one flagged item for the store warp
             if (!*abort_flag) {
                 bool ok = true;
@@ -1016,16 +1025,32 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 const unsigned wo0 = smem_u32(base + L.wo), zero_s = smem_u32(base + L.zero);
                 const u64 pol_first = l2_policy_evict_first();
                 int ci = 0, zc = 0;                                          // consumer item, 4-store chunk of the current zero item
-                // zero items are claimed one at a time from the list of chan_order_kernel, two claims ahead: z_cur is being
-                // stored, z_nxt is the next one's item id (its load in flight), z_idx the list index claimed for the one after
+                // zero items are claimed 16 at a time from the list of chan_order_kernel; the claim of the next chunk is in
+                // flight while this one is stored (one exposed L2 round trip per 16 items of ~3 us each)
                 const int n_z = __ldg(P.n_cz + 1);
-                int z_cur, z_nxt, z_idx;
-                {
-                    const int i0 = atomicAdd(P.zcounter, 1), i1 = atomicAdd(P.zcounter, 1);
-                    z_idx = atomicAdd(P.zcounter, 1);
-                    z_cur = i0 < n_z ? (int)__ldg(P.z_list + i0) : -1;
-                    z_nxt = i1 < n_z ? (int)__ldg(P.z_list + i1) : -1;
-                }
+                int z_cur = -1, z_k = 0, z_n = 0, zX0 = 0, zY0 = 0, zc0 = 0, z_pos = 0;
+                const int n_c = __ldg(P.n_cz);
+                const long long z_lead = (long long)n_c * K6_ZERO_LEAD_PCT / 100 + 8;
+                int z_base_next = atomicAdd(P.zcounter, k6ZeroChunk);
+                int zb_cur = 0;
+                auto z_advance = [&]() {
+                    if (z_k >= z_n) {
+                        const int zb = z_base_next;
+                        if (zb >= n_z) { z_cur = -1; return; }           // claims only grow: the list is exhausted for good
+                        z_n = min(k6ZeroChunk, n_z - zb);
+                        zb_cur = zb;
+                        const int4* src = reinterpret_cast<const int4*>(P.z_list + zb);   // 64 B aligned; the list is padded
+#pragma unroll
+                        for (int q = 0; q < k6ZeroChunk / 4; ++q) reinterpret_cast<int4*>(S.z_ids)[q] = __ldg(src + q);
+                        z_base_next = atomicAdd(P.zcounter, k6ZeroChunk);
+                        z_k = 0;
+                    }
+                    z_pos = zb_cur + z_k;
+                    z_cur = S.z_ids[z_k++];
+                    const int tx = z_cur % P.ntx, ty = (z_cur / P.ntx) % P.nty, grp = z_cur / (P.ntx * P.nty);
+                    zX0 = tx * k6TileX; zY0 = ty * k6TileY; zc0 = grp * 32;
+                };
+                z_advance();
                 unsigned remaining = 0xfu;                                   // block rows of consumer item ci still to store
                 long long t_so_rel = 0, t_so_idle = 0, t_so_zero = 0, t_so_all = 0;
                 (void)t_so_rel; (void)t_so_idle; (void)t_so_zero; (void)t_so_all;
@@ -1061,22 +1086,24 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                             if (remaining == 0u) { ++ci; S.done_c = ci; remaining = 0xfu; }
                         }
                     }
-                    if (z_cur >= 0) {
+                    // Zero-fill is paced by the progress of the consumer items (both lists are global and claimed in order): the
+                    // share of the zero list that is done stays within K6_ZERO_LEAD_PCT of the share of the consumer list the
+                    // sweeper has reached.  Unpaced, every SM zero-fills flat out at the start of the kernel and the write
+                    // stream starves the visibility loads of the dense tiles (measured: 8.2 - 8.6 ms against 7.9).
+                    if (z_cur >= 0 && (long long)z_pos * n_c <= ((long long)S.c_pos + z_lead) * n_z) {
                         K6_TIC(s2);
-                        const int tx = z_cur % P.ntx, ty = (z_cur / P.ntx) % P.nty, grp = z_cur / (P.ntx * P.nty);
-                        const int X0 = tx * k6TileX, Y0 = ty * k6TileY, c0 = grp * 32;
-                        const int pol = zc >> 1, v0 = (zc & 1) * 4;
+                        // one box of [v 4][chan 32][16 cells] per look, and never more than K6_ZERO_INFLIGHT + 1 of them queued in
+                        // the TMA engine: a consumer row that becomes ready must not wait behind a long run of zero boxes
+#ifndef K6_ZERO_INFLIGHT
+#define K6_ZERO_INFLIGHT 1
+#endif
+                        asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(K6_ZERO_INFLIGHT) : "memory");
+                        const int zpol = zc / (k6TileY / k6ZeroV), zv = (zc % (k6TileY / k6ZeroV)) * k6ZeroV;
 #ifndef K6_ABLATE_STORE
-                        for (int v = v0; v < v0 + 4; ++v)
-                            if (Y0 + v < N) tma_store4(&map_zero, zero_s, X0, c0, Y0 + v, pol, pol_first);
+                        if (zY0 + zv < N) tma_store4(&map_zero, zero_s, zX0, zc0, zY0 + zv, zpol, pol_first);
 #endif
                         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-                        if (++zc == 8) {
-                            zc = 0;
-                            z_cur = z_nxt;
-                            z_nxt = z_idx < n_z ? (int)__ldg(P.z_list + z_idx) : -1;
-                            z_idx = atomicAdd(P.zcounter, 1);
-                        }
+                        if (++zc == 4 * (k6TileY / k6ZeroV)) { zc = 0; z_advance(); }
                         progress = true;
                         K6_TOC(t_so_zero, s2);
                     }
@@ -1192,7 +1219,7 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
     if (P.n_items >= 0x7fffffffLL) { set_error("design CHANWS: too many work items"); return false; }
     CUtensorMap map_out, map_zero;
     if (!make_grid_map(&map_out, grid, p->geom.N, n_chan, 2, 4, true)) return false;
-    if (!make_grid_map(&map_zero, grid, p->geom.N, n_chan, 1, 1, false)) return false;
+    if (!make_grid_map(&map_zero, grid, p->geom.N, n_chan, k6ZeroV, 1, false)) return false;
 
     long long iblocks = (n_vis + 7) / 8;                                      // one warp per sorted row at a time
     if (iblocks > (long long)p->sm_count * 8) iblocks = (long long)p->sm_count * 8;
