@@ -119,6 +119,24 @@ int mwa_grid_plan_set_list_pool(mwa_grid_plan* plan, long long entries);
 /* Number of kernel launches (memsets included) enqueued by the last gridding call on this plan. */
 int mwa_grid_plan_last_launches(const mwa_grid_plan* plan);
 
+/* f1 - the two steps after gridding (Table 1 rows "FFT" and "Convolution Correction"; the
+ * grid exists "to permit the operation of the Fast Fourier Transform"): for every N x N plane
+ *   image[q'][p'] = sum_{j,i} grid[j][i] exp(+2 pi i ((i - N/2) p + (j - N/2) q) / N) / (c^(p) c^(q)),  p = p' - N/2, q = q' - N/2
+ *   c^(p) = (1/O) sum'_{k=-WO/2..WO/2} C(k/O) cos(2 pi (k/O) p / N)   (end terms halved; C(k/O) read from the plan's table)
+ * i.e. the unnormalised inverse transform of the grid with both centres at [N/2][N/2], divided by the transform of the
+ * gridding kernel ("convolution correction").  The correction falls to ~2e-4 (W = 7) at the image edge, so only the
+ * inner part of the image is meaningful (SURVEY.md pin P5).
+ *   grid   [n_planes][N][N][2] float (re, im), DEVICE, as written by mwa_grid_visibilities (n_planes = n_chan * 4)
+ *   image  [n_planes][N][N][2] float (re, im), DEVICE; may be the same buffer as grid (in place), else must not overlap
+ * The transform is a batched cuFFT call (library), the shifts, the sign and the division are one fused in-place kernel.
+ * Asynchronous on `stream` except for the first call on a plan (it builds c^ and synchronises once).  Returns 0 or a
+ * negative error code (MWA_GRID_ERR_CUDA with "cuFFT ... could not be loaded" if the library is missing). */
+int mwa_image_from_grid(mwa_grid_plan* plan, const float* grid, float* image, long long n_planes, void* stream);
+
+/* The correction function of the plan: out_corr[p'] = c^(p' - N/2) for p' = 0..min(n, N)-1, HOST array of doubles.
+ * Returns the number of values written.  Synchronous. */
+int mwa_image_correction(mwa_grid_plan* plan, double* out_corr, int n);
+
 /* Free the table and the workspace.  NULL is a no-op. */
 void mwa_grid_plan_destroy(mwa_grid_plan* plan);
 

@@ -48,12 +48,17 @@ _lib.mwa_grid_plan_last_stats.argtypes = [_P, _P, _I]
 _lib.mwa_grid_plan_last_stats.restype = _I
 _lib.mwa_grid_probe_fp32.argtypes = [_P, _P, _P]
 _lib.mwa_grid_probe_fp32.restype = _I
+_lib.mwa_image_from_grid.argtypes = [_P, _P, _P, _LL, _P]
+_lib.mwa_image_from_grid.restype = _I
+_lib.mwa_image_correction.argtypes = [_P, _P, _I]
+_lib.mwa_image_correction.restype = _I
 _lib.mwa_grid_last_error.argtypes = []
 _lib.mwa_grid_last_error.restype = ctypes.c_char_p
 
 EXPORTS = ["mwa_grid_plan_create", "mwa_grid_plan_destroy", "mwa_grid_visibilities", "mwa_grid_visibilities_host",
            "mwa_grid_compute_indices", "mwa_grid_plan_set_design", "mwa_grid_plan_set_profiling",
-           "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_plan_last_design", "mwa_grid_plan_last_stats", "mwa_grid_plan_set_list_pool", "mwa_grid_probe_fp32", "mwa_grid_last_error"]
+           "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_plan_last_design", "mwa_grid_plan_last_stats", "mwa_grid_plan_set_list_pool", "mwa_grid_probe_fp32", "mwa_grid_last_error",
+           "mwa_image_from_grid", "mwa_image_correction"]
 
 
 class MwaGridError(RuntimeError):
@@ -174,6 +179,19 @@ def mwa_grid_plan_set_list_pool(plan, entries: int) -> None:
     _check(_lib.mwa_grid_plan_set_list_pool(plan, int(entries)))
 
 
+def mwa_image_from_grid(plan, grid, image, n_planes, stream=None) -> None:
+    """f1: corrected dirty images of `n_planes` N x N uv grids (device complex64); `image` may be `grid` (in place)."""
+    _check(_lib.mwa_image_from_grid(plan, _ptr(grid, torch.complex64, "cuda", "grid"),
+                                    _ptr(image, torch.complex64, "cuda", "image"), int(n_planes), _stream_ptr(stream)))
+
+
+def mwa_image_correction(plan, n: int):
+    """The plan's correction function c^(p' - N/2), p' = 0..n-1, as a float64 CPU tensor."""
+    out = torch.empty(int(n), dtype=torch.float64)
+    k = _check(_lib.mwa_image_correction(plan, out.data_ptr(), int(n)))
+    return out[:k]
+
+
 def mwa_grid_probe_fp32(plan, stream=None):
     """(TFLOP/s of fma.rn.f32, TFLOP/s of fma.rn.f32x2) measured with a register-only loop."""
     buf = (ctypes.c_double * 2)()
@@ -198,6 +216,13 @@ class Plan:
         if out is None:
             out = torch.empty((n_chan, 4, self.grid_n, self.grid_n), dtype=torch.complex64, device=uv.device)
         mwa_grid_visibilities(self.handle, uv, freqs, vis, weights, n_vis, n_chan, out, stream)
+        return out
+
+    def image(self, grid, out=None, stream=None):
+        """Corrected dirty images of the grids of `grid` [..., N, N]; in place when out is grid."""
+        if out is None:
+            out = torch.empty_like(grid)
+        mwa_image_from_grid(self.handle, grid, out, grid.numel() // (self.grid_n * self.grid_n), stream)
         return out
 
     def indices(self, uv, freqs, stream=None):

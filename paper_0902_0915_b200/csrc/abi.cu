@@ -239,10 +239,41 @@ void mwa_grid_plan_destroy(mwa_grid_plan* plan) {
                     ws.d_pre, ws.d_bb, ws.d_list_cnt, ws.d_list_off, ws.d_c_desc, ws.d_z_list, ws.d_lists};
     for (void* q : ptrs)
         if (q) cudaFree(q);
+    image_release(p);
     for (auto& e : p->ev)
         if (e) cudaEventDestroy(e);
     delete[] p->h_table;
     delete p;
+}
+
+int mwa_image_from_grid(mwa_grid_plan* plan, const float* grid, float* image, long long n_planes, void* stream) {
+    g_last_error.clear();
+    Plan* p = reinterpret_cast<Plan*>(plan);
+    if (!p) { set_error("plan is NULL"); return MWA_GRID_ERR_INVALID; }
+    if (n_planes < 0) { set_error("n_planes must be >= 0"); return MWA_GRID_ERR_INVALID; }
+    p->last_launches = 0;
+    if (n_planes == 0) return MWA_GRID_OK;
+    if (!grid || !image || !aligned(grid, 16) || !aligned(image, 16)) { set_error("grid and image must be non-NULL and 16-byte aligned"); return MWA_GRID_ERR_INVALID; }
+    if (grid != image) {
+        const size_t bytes = (size_t)n_planes * p->geom.N * p->geom.N * 8;
+        const char *a = (const char*)grid, *b = (const char*)image;
+        if (a < b + bytes && b < a + bytes) { set_error("grid and image must be the same buffer or not overlap"); return MWA_GRID_ERR_INVALID; }
+    }
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev), "cudaGetDevice")) return MWA_GRID_ERR_CUDA;
+    if (dev != p->device) { set_error("the current CUDA device is not the device the plan was created on"); return MWA_GRID_ERR_INVALID; }
+    return launch_image(p, grid, image, n_planes, reinterpret_cast<cudaStream_t>(stream)) ? MWA_GRID_OK : MWA_GRID_ERR_CUDA;
+}
+
+int mwa_image_correction(mwa_grid_plan* plan, double* out_corr, int n) {
+    g_last_error.clear();
+    Plan* p = reinterpret_cast<Plan*>(plan);
+    if (!p || !out_corr || n < 0) { set_error("bad argument"); return MWA_GRID_ERR_INVALID; }
+    const double* c = image_correction_host(p, nullptr);
+    if (!c) return MWA_GRID_ERR_CUDA;
+    const int k = n < p->geom.N ? n : p->geom.N;
+    std::memcpy(out_corr, c, (size_t)k * sizeof(double));
+    return k;
 }
 
 int mwa_grid_plan_set_design(mwa_grid_plan* plan, int design) {

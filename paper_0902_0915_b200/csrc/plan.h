@@ -1,6 +1,7 @@
 // plan.h - the plan object behind the C ABI and the launchers of the individual kernels.
 #pragma once
 #include <cuda_runtime.h>
+#include <new>
 #include <string>
 #include "index.cuh"
 
@@ -66,6 +67,11 @@ struct Plan {
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     bool ev_valid = false;
     int last_launches = 0;
+    // f1 imaging step (k_image.cu)
+    float* d_inv_corr = nullptr;     // [N] 1 / c^(p' - N/2)
+    double* h_corr = nullptr;        // [N] c^(p' - N/2), host copy (fp64)
+    int fft_handle[2] = {0, 0};      // cached cuFFT plans ...
+    int fft_batch[2] = {0, 0};       // ... and the batch sizes they were made for (0 = none)
     long long pool_limit = 0;        // diagnostics: cap on K6's hit-list pool in entries (0 = default sizing)
     bool last_chanws = false;        // AUTO: the channel-SIMD kernel enqueued by the last call was K6 (else K5)
 };
@@ -91,6 +97,9 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
                    const int* dispatch, cudaStream_t st);
 bool launch_smem(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                  cudaStream_t st);
+bool launch_image(Plan* p, const float* grid, float* image, long long n_planes, cudaStream_t st);
+const double* image_correction_host(Plan* p, cudaStream_t st);
+void image_release(Plan* p);
 bool launch_romein(Plan* p, const double* uv, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                    cudaStream_t st);
 
