@@ -75,15 +75,15 @@ __device__ __forceinline__ unsigned transpose32(unsigned x, int lane) {
 }
 
 struct WarpSmem {
-    float4 z[kCap][2];      // w*V: {XX.re, XX.im, XY.re, XY.im}, {YX.re, YX.im, YY.re, YY.im}
+    float4 z[kCap][2];      // V: {XX.re, XX.im, XY.re, XY.im}, {YX.re, YX.im, YY.re, YY.im} (cp.async from phase A)
     unsigned geo[kCap];     // (byte offset into u copies + bias) | (byte offset into v copies + bias) << 16
     unsigned mask[kCap];    // lanes (blocks) the stamp overlaps
-    int row[kCap];          // original row id (vis / weights index)
+    float w[kCap];          // weight of the sample (cp.async; multiplied into the v taps in phase B)
 };
 
 constexpr int kBiasU = 16, kBiasV = 16;   // floats; keep the stored offsets non-negative
 
-__global__ void __launch_bounds__(kWarpsPerCta * 32)
+__global__ void __launch_bounds__(kWarpsPerCta * 32, 4)
 gather_kernel(const GatherParams P) {
     if (P.dispatch != nullptr && *P.dispatch != 0) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -114,6 +114,8 @@ gather_kernel(const GatherParams P) {
     const unsigned tv_s = (unsigned)__cvta_generic_to_shared(tv);
     const unsigned z_s = (unsigned)__cvta_generic_to_shared(&wsm->z[0][0]);
     const unsigned geo_s = (unsigned)__cvta_generic_to_shared(&wsm->geo[0]);
+    const unsigned w_s = (unsigned)__cvta_generic_to_shared(&wsm->w[0]);
+    const bool has_w = P.weights != nullptr;
     // lane constants of the table addresses: offset (floats) = stored - bias + 4*bx  (u), + 2*by (v)
     const unsigned cu = tu_s + (unsigned)((4 * bx - kBiasU) * 4);
     const unsigned cv = tv_s + (unsigned)((2 * by - kBiasV) * 4);
@@ -163,19 +165,9 @@ gather_kernel(const GatherParams P) {
 
         // consume the buffered hits: loads of w*V, transpose, per-lane walk
         auto consume = [&](int n) {
+            // the visibilities and weights of the buffered hits were requested with cp.async when the hits were found
+            asm volatile("cp.async.wait_all;" ::: "memory");
             __syncwarp();
-            // pass 2: lane = hit; visibility + weight loads, all independent
-#pragma unroll
-            for (int b = 0; b < kCap / 32; ++b) {
-                const int hidx = b * 32 + lane;
-                if (hidx < n) {
-                    const size_t sidx = (size_t)wsm->row[hidx] * P.n_chan + c;
-                    const float4 va = __ldg(P.vis + 2 * sidx), vb = __ldg(P.vis + 2 * sidx + 1);
-                    const float wt = P.weights ? __ldg(P.weights + sidx) : 1.0f;
-                    wsm->z[hidx][0] = make_float4(wt * va.x, wt * va.y, wt * va.z, wt * va.w);
-                    wsm->z[hidx][1] = make_float4(wt * vb.x, wt * vb.y, wt * vb.z, wt * vb.w);
-                }
-            }
             unsigned mw[kCap / 32];
 #pragma unroll
             for (int b = 0; b < kCap / 32; ++b) {
@@ -200,14 +192,15 @@ gather_kernel(const GatherParams P) {
                     const int hidx = w * 32 + bit;
                     unsigned geo;
                     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(geo) : "r"(geo_s + 4u * hidx));
-                    float ku0, ku1, ku2, ku3, kv0, kv1;
+                    float ku0, ku1, ku2, ku3, kv0, kv1, wt = 1.0f;
+                    if (has_w) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(wt) : "r"(w_s + 4u * hidx));
                     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(ku0), "=f"(ku1), "=f"(ku2), "=f"(ku3) : "r"(cu + (geo & 0xffffu)));
                     asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(kv0), "=f"(kv1) : "r"(cv + (geo >> 16)));
                     u64 z0, z1, z2, z3;
                     asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(z0), "=l"(z1) : "r"(z_s + 32u * hidx));
                     asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(z2), "=l"(z3) : "r"(z_s + 32u * hidx + 16u));
                     const float ku[4] = {ku0, ku1, ku2, ku3};
-                    const float kv[2] = {kv0, kv1};
+                    const float kv[2] = {kv0 * wt, kv1 * wt};
 #pragma unroll
                     for (int i = 0; i < 2; ++i)
 #pragma unroll
@@ -224,23 +217,69 @@ gather_kernel(const GatherParams P) {
             __syncwarp();
         };
 
-        // ---- phase A, pass 1: lane = candidate
-        for (int byb = by0; byb <= by1; ++byb) {
-            const int k0 = __ldg(P.bucket_start + byb * P.nb + bx0);
-            const int k1 = __ldg(P.bucket_start + byb * P.nb + bx1 + 1);
-            for (int kb = k0; kb < k1; kb += 32) {
-                const int k = kb + lane;
+        // ---- phase A, pass 1: lane = candidate.  The candidates of the window (the sorted rows of its bucket rows, `total`
+        // of them) are visited in a fixed scattered order, position j -> candidate (j * S) mod total with S ~ 0.618 total
+        // coprime to total, not bucket after bucket: the hits of one bucket have nearly the same stamp origin and fall on the
+        // same few 4 x 2 blocks, so a buffer filled in sorted order keeps a few lanes busy in phase B while the others
+        // idle.  A pure function of the sorted rows: the result stays bit-identical from run to run.
+        for (int rg = by0; rg <= by1; rg += 32) {
+            int k0 = 0, len = 0;
+            if (rg + lane <= by1) {                                          // lane = bucket row rg + lane
+                k0 = __ldg(P.bucket_start + (rg + lane) * P.nb + bx0);
+                len = __ldg(P.bucket_start + (rg + lane) * P.nb + bx1 + 1) - k0;
+            }
+            int incl = len;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += t;
+            }
+            const int total = __shfl_sync(0xffffffffu, incl, 31);
+            const int excl = incl - len;
+            if (total == 0) continue;
+            int S = 1;
+            if (total >= 64) {
+                S = (int)(((long long)total * 618) / 1000) | 1;
+                for (;; S += 2) {
+                    int ga = total, gb = S;
+                    while (gb) { const int t = ga % gb; ga = gb; gb = t; }
+                    if (ga == 1) break;
+                }
+            }
+            const int step32 = (int)(((long long)32 * S) % total);
+            int f = (int)(((long long)lane * S) % total);
+            // candidate position of chunk `cb` for this lane, and its uv record one chunk ahead of its use
+            auto locate = [&](int cb, int& row, double2& p) {
+                int lo = 0;                                                  // smallest bucket row with incl > f
+#pragma unroll
+                for (int st = 16; st > 0; st >>= 1) {
+                    const int t = __shfl_sync(0xffffffffu, incl, lo + st - 1);
+                    if (t <= f) lo += st;
+                }
+                lo = min(lo, 31);
+                const int k = __shfl_sync(0xffffffffu, k0, lo) + (f - __shfl_sync(0xffffffffu, excl, lo));
+                f += step32;
+                if (f >= total) f -= total;
+                p = make_double2(0.0, 0.0);
+                row = 0;
+                if (cb + lane < total) { p = __ldg(P.uv_sorted + k); row = __ldg(P.perm + k); }
+            };
+            int row_nx;
+            double2 p_nx;
+            locate(0, row_nx, p_nx);
+            for (int cb = 0; cb < total; cb += 32) {
+                const bool in_range = cb + lane < total;
+                const int row = row_nx;
+                const double2 p = p_nx;
+                if (cb + 32 < total) locate(cb + 32, row_nx, p_nx);
                 bool hit = false;
                 unsigned geo = 0, mask = 0;
-                int row = 0;
-                if (k < k1) {
-                    const double2 p = __ldg(P.uv_sorted + k);
+                if (in_range) {
                     SampleIndex s;
                     if (sample_index(p.x, p.y, sc, g, s)) {
                         const int ou = s.iu - g.h - X0, ov = s.iv - g.h - Y0;     // stamp origin relative to the tile
                         if (ou > -g.W && ou < kTile && ov > -g.W && ov < kTile) {
                             hit = true;
-                            row = __ldg(P.perm + k);
                             const int su = (3 - ou) & 3, sv = (1 - ov) & 1;
                             const int offu = (su * (g.O + 1) + s.ru) * P.rlu + (3 - ou - su) + kBiasU;
                             const int offv = (sv * (g.O + 1) + s.rv) * P.rlv + (1 - ov - sv) + kBiasV;
@@ -261,7 +300,13 @@ gather_kernel(const GatherParams P) {
                     const int slot = n_buf + __popc(ball & lt_mask);
                     wsm->geo[slot] = geo;
                     wsm->mask[slot] = mask;
-                    wsm->row[slot] = row;
+                    // the sample's 32 B of visibilities and its weight go straight to the buffer, asynchronously: they land
+                    // while the scan goes on
+                    const size_t sidx = (size_t)row * P.n_chan + c;
+                    const float4* src = P.vis + 2 * sidx;
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(z_s + 32u * slot), "l"(src) : "memory");
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(z_s + 32u * slot + 16u), "l"(src + 1) : "memory");
+                    if (has_w) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(w_s + 4u * slot), "l"(P.weights + sidx) : "memory");
                 }
                 n_buf += cnt;
             }
