@@ -43,6 +43,7 @@ struct GatherParams {
     int n_chan, nb, nt;
     int rlu, rlv;               // padded row lengths of the shifted table copies
     long long n_items;
+    int chunk;                  // consecutive work items per claim (1..8; amortises the round trip of the work counter)
 };
 
 typedef unsigned long long u64;
@@ -75,10 +76,10 @@ __device__ __forceinline__ unsigned transpose32(unsigned x, int lane) {
 }
 
 struct WarpSmem {
-    float4 z[kCap][2];      // V: {XX.re, XX.im, XY.re, XY.im}, {YX.re, YX.im, YY.re, YY.im} (cp.async from phase A)
-    unsigned geo[kCap];     // (byte offset into u copies + bias) | (byte offset into v copies + bias) << 16
+    float4 z[kCap + 1][2];    // V: {XX.re, XX.im, XY.re, XY.im}, {YX.re, YX.im, YY.re, YY.im} (cp.async from phase A)
+    unsigned geo[kCap + 1];   // (byte offset into u copies + bias) | (byte offset into v copies + bias) << 16
     unsigned mask[kCap];    // lanes (blocks) the stamp overlaps
-    float w[kCap];          // weight of the sample (cp.async; multiplied into the v taps in phase B)
+    float w[kCap + 1];        // weight of the sample (cp.async; multiplied into the v taps in phase B)
 };
 
 constexpr int kBiasU = 16, kBiasV = 16;   // floats; keep the stored offsets non-negative
@@ -119,17 +120,26 @@ gather_kernel(const GatherParams P) {
     // lane constants of the table addresses: offset (floats) = stored - bias + 4*bx  (u), + 2*by (v)
     const unsigned cu = tu_s + (unsigned)((4 * bx - kBiasU) * 4);
     const unsigned cv = tv_s + (unsigned)((2 * by - kBiasV) * 4);
+    if (lane == 0) {                                     // the null hit of phase B
+        wsm->z[kCap][0] = make_float4(0.f, 0.f, 0.f, 0.f);
+        wsm->z[kCap][1] = make_float4(0.f, 0.f, 0.f, 0.f);
+        wsm->geo[kCap] = (unsigned)(kBiasU * 4) | ((unsigned)(kBiasV * 4) << 16);
+        wsm->w[kCap] = 0.0f;
+    }
+    __syncwarp();
     const double s_ref = *P.scale_ref;
     const size_t plane = (size_t)g.N * g.N;
     const unsigned lt_mask = (1u << lane) - 1u;
 
-    long long item = 0;
-    if (lane == 0) item = (long long)atomicAdd(P.counter, 1);
-    item = __shfl_sync(0xffffffffu, item, 0);
+    long long base = 0;
+    if (lane == 0) base = (long long)atomicAdd(P.counter, P.chunk);
+    base = __shfl_sync(0xffffffffu, base, 0);
+    int sub = 0;
+    long long next_base = 0;
 
-    while (item < P.n_items) {
-        long long next_item = 0;
-        if (lane == 0) next_item = (long long)atomicAdd(P.counter, 1);      // latency hidden behind this item
+    while (base + sub < P.n_items) {
+        const long long item = base + sub;
+        if (sub == 0 && lane == 0) next_base = (long long)atomicAdd(P.counter, P.chunk);   // used P.chunk items from now
         const int trank = (int)(item / P.n_chan);
         const int c = (int)(item - (long long)trank * P.n_chan);
         const int tile = P.tile_order[trank];
@@ -176,44 +186,72 @@ gather_kernel(const GatherParams P) {
                 mw[b] = (b * 32 < n) ? transpose32(m, lane) : 0u;
             }
             __syncwarp();
-            unsigned m = mw[0];
-            int w = 0;
-            while (true) {
-                if (m == 0u) {
-#pragma unroll
-                    for (int b = 1; b < kCap / 32; ++b)
-                        if (m == 0u && w < b) { w = b; m = mw[b]; }
+            // ---- phase B: every lane walks its own hit list, branch-free.  A lane whose list is exhausted (or whose current
+            // mask word is) takes the null hit - slot kCap: zero visibilities, zero weight, an in-range table offset - so the
+            // whole warp runs the same instruction stream for `steps` rounds, the longest list plus its empty words.  The
+            // loads of a visit are issued under the FMAs of the visit before it (two operand sets, as K6's consumers).
+            unsigned m = mw[0], q1 = mw[1], q2 = mw[2], q3 = mw[3];
+            int wb = 0;
+            int mine = __popc(m) + __popc(q1) + __popc(q2) + __popc(q3);
+            mine += (m == 0u ? 1 : 0) + (q1 == 0u ? 1 : 0) + (q2 == 0u ? 1 : 0);      // a step that only moves on to the next word
+            const int steps = __reduce_max_sync(0xffffffffu, mine);
+            auto next_hit = [&]() -> unsigned {
+                const bool refill = m == 0u;
+                m = refill ? q1 : m; q1 = refill ? q2 : q1; q2 = refill ? q3 : q2; q3 = refill ? 0u : q3;
+                wb += refill ? 32 : 0;
+                const unsigned bit = (unsigned)(__ffs(m) - 1);
+                const unsigned hidx = m != 0u ? (unsigned)wb + bit : (unsigned)kCap;
+                m &= m - 1u;
+                return hidx;
+            };
+#define K3_LOAD(h, g, Z0, Z1, Z2, Z3, U0, U1, U2, U3, V0, V1, WT)                                                          \
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(Z0), "=l"(Z1) : "r"(z_s + 32u * (h)));                           \
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(Z2), "=l"(Z3) : "r"(z_s + 32u * (h) + 16u));                     \
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(U0), "=f"(U1), "=f"(U2), "=f"(U3) : "r"(cu + ((g) & 0xffffu))); \
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(V0), "=f"(V1) : "r"(cv + ((g) >> 16)));                          \
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(WT) : "r"(w_s + 4u * (h)));
+#define K3_FMA(Z0, Z1, Z2, Z3, U0, U1, U2, U3, V0, V1, WT)                                                                 \
+    {                                                                                                                      \
+        const float kvw[2] = {V0 * WT, V1 * WT};                                                                           \
+        const float kuu[4] = {U0, U1, U2, U3};                                                                             \
+        _Pragma("unroll") for (int i = 0; i < 2; ++i) _Pragma("unroll") for (int j = 0; j < 4; ++j) {                       \
+            const float kq = kvw[i] * kuu[j];                                                                              \
+            const u64 kk = pack2(kq, kq);                                                                                  \
+            ffma2(acc[i][j][0], kk, Z0);                                                                                   \
+            ffma2(acc[i][j][1], kk, Z1);                                                                                   \
+            ffma2(acc[i][j][2], kk, Z2);                                                                                   \
+            ffma2(acc[i][j][3], kk, Z3);                                                                                   \
+        }                                                                                                                  \
+    }
+            if (steps > 0) {
+                u64 az0, az1, az2, az3, bz0, bz1, bz2, bz3;
+                float au0, au1, au2, au3, av0, av1, aw, bu0, bu1, bu2, bu3, bv0, bv1, bw;
+                const unsigned h0 = next_hit();
+                unsigned h1 = next_hit(), h2 = next_hit();
+                unsigned g1, g2;
+                {
+                    unsigned g0;
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g0) : "r"(geo_s + 4u * h0));
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g1) : "r"(geo_s + 4u * h1));
+                    K3_LOAD(h0, g0, az0, az1, az2, az3, au0, au1, au2, au3, av0, av1, aw)
                 }
-                const bool act = (m != 0u);
-                if (!__any_sync(0xffffffffu, act)) break;
-                if (act) {
-                    const int bit = __ffs(m) - 1;
-                    m &= m - 1u;
-                    const int hidx = w * 32 + bit;
-                    unsigned geo;
-                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(geo) : "r"(geo_s + 4u * hidx));
-                    float ku0, ku1, ku2, ku3, kv0, kv1, wt = 1.0f;
-                    if (has_w) asm volatile("ld.shared.f32 %0, [%1];" : "=f"(wt) : "r"(w_s + 4u * hidx));
-                    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(ku0), "=f"(ku1), "=f"(ku2), "=f"(ku3) : "r"(cu + (geo & 0xffffu)));
-                    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(kv0), "=f"(kv1) : "r"(cv + (geo >> 16)));
-                    u64 z0, z1, z2, z3;
-                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(z0), "=l"(z1) : "r"(z_s + 32u * hidx));
-                    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(z2), "=l"(z3) : "r"(z_s + 32u * hidx + 16u));
-                    const float ku[4] = {ku0, ku1, ku2, ku3};
-                    const float kv[2] = {kv0 * wt, kv1 * wt};
-#pragma unroll
-                    for (int i = 0; i < 2; ++i)
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            const float k = kv[i] * ku[j];
-                            const u64 kk = pack2(k, k);
-                            ffma2(acc[i][j][0], kk, z0);
-                            ffma2(acc[i][j][1], kk, z1);
-                            ffma2(acc[i][j][2], kk, z2);
-                            ffma2(acc[i][j][3], kk, z3);
-                        }
+#pragma unroll 1
+                for (int v = 0; v < steps; v += 2) {
+                    K3_LOAD(h1, g1, bz0, bz1, bz2, bz3, bu0, bu1, bu2, bu3, bv0, bv1, bw)
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g2) : "r"(geo_s + 4u * h2));
+                    const unsigned h3 = next_hit();
+                    K3_FMA(az0, az1, az2, az3, au0, au1, au2, au3, av0, av1, aw)
+                    if (v + 1 >= steps) break;
+                    K3_LOAD(h2, g2, az0, az1, az2, az3, au0, au1, au2, au3, av0, av1, aw)
+                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g1) : "r"(geo_s + 4u * h3));
+                    const unsigned h4 = next_hit();
+                    K3_FMA(bz0, bz1, bz2, bz3, bu0, bu1, bu2, bu3, bv0, bv1, bw)
+                    h1 = h3;
+                    h2 = h4;
                 }
             }
+#undef K3_LOAD
+#undef K3_FMA
             __syncwarp();
         };
 
@@ -307,6 +345,7 @@ gather_kernel(const GatherParams P) {
                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(z_s + 32u * slot), "l"(src) : "memory");
                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(z_s + 32u * slot + 16u), "l"(src + 1) : "memory");
                     if (has_w) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(w_s + 4u * slot), "l"(P.weights + sidx) : "memory");
+                    else wsm->w[slot] = 1.0f;
                 }
                 n_buf += cnt;
             }
@@ -338,7 +377,7 @@ gather_kernel(const GatherParams P) {
                 }
             }
         }
-        item = __shfl_sync(0xffffffffu, next_item, 0);
+        if (++sub == P.chunk) { sub = 0; base = __shfl_sync(0xffffffffu, next_base, 0); }
     }
 }
 
@@ -380,6 +419,9 @@ bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, i
     long long blocks = (long long)p->sm_count * ctas_per_sm;
     if (blocks > want) blocks = want;
     if (blocks < 1) blocks = 1;
+    // items per claim: up to 8 while every warp still gets at least ~16 claims (small problems keep 1)
+    long long chunk = P.n_items / (blocks * kWarpsPerCta * 16);
+    P.chunk = (int)(chunk < 1 ? 1 : chunk > 8 ? 8 : chunk);
     gather_kernel<<<(unsigned)blocks, kWarpsPerCta * 32, smem, st>>>(P);
     p->last_launches += 1;
     return cuda_ok(cudaGetLastError(), "gather_kernel");
