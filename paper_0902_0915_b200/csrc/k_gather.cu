@@ -76,10 +76,11 @@ __device__ __forceinline__ unsigned transpose32(unsigned x, int lane) {
 }
 
 struct WarpSmem {
-    float4 z[kCap + 1][2];    // V: {XX.re, XX.im, XY.re, XY.im}, {YX.re, YX.im, YY.re, YY.im} (cp.async from phase A)
-    unsigned geo[kCap + 1];   // (byte offset into u copies + bias) | (byte offset into v copies + bias) << 16
+    float4 z[2][kCap + 1];  // V by halves: [0] {XX.re, XX.im, XY.re, XY.im}, [1] {YX.re, YX.im, YY.re, YY.im} (cp.async from
+                            // phase A); 16 B per hit and half, so the lane-private LDS.128 of phase B spread over all banks
+    uint2 gw[kCap + 1];     // x: (byte offset into u copies + bias) | (byte offset into v copies + bias) << 16; y: weight
+                            // (cp.async); one LDS.64 per visit
     unsigned mask[kCap];    // lanes (blocks) the stamp overlaps
-    float w[kCap + 1];        // weight of the sample (cp.async; multiplied into the v taps in phase B)
 };
 
 constexpr int kBiasU = 16, kBiasV = 16;   // floats; keep the stored offsets non-negative
@@ -114,17 +115,16 @@ gather_kernel(const GatherParams P) {
     const unsigned tu_s = (unsigned)__cvta_generic_to_shared(tu);
     const unsigned tv_s = (unsigned)__cvta_generic_to_shared(tv);
     const unsigned z_s = (unsigned)__cvta_generic_to_shared(&wsm->z[0][0]);
-    const unsigned geo_s = (unsigned)__cvta_generic_to_shared(&wsm->geo[0]);
-    const unsigned w_s = (unsigned)__cvta_generic_to_shared(&wsm->w[0]);
+    const unsigned gw_s = (unsigned)__cvta_generic_to_shared(&wsm->gw[0]);
+    constexpr unsigned kZHalf = 16u * (kCap + 1);
     const bool has_w = P.weights != nullptr;
     // lane constants of the table addresses: offset (floats) = stored - bias + 4*bx  (u), + 2*by (v)
     const unsigned cu = tu_s + (unsigned)((4 * bx - kBiasU) * 4);
     const unsigned cv = tv_s + (unsigned)((2 * by - kBiasV) * 4);
     if (lane == 0) {                                     // the null hit of phase B
-        wsm->z[kCap][0] = make_float4(0.f, 0.f, 0.f, 0.f);
-        wsm->z[kCap][1] = make_float4(0.f, 0.f, 0.f, 0.f);
-        wsm->geo[kCap] = (unsigned)(kBiasU * 4) | ((unsigned)(kBiasV * 4) << 16);
-        wsm->w[kCap] = 0.0f;
+        wsm->z[0][kCap] = make_float4(0.f, 0.f, 0.f, 0.f);
+        wsm->z[1][kCap] = make_float4(0.f, 0.f, 0.f, 0.f);
+        wsm->gw[kCap] = make_uint2((unsigned)(kBiasU * 4) | ((unsigned)(kBiasV * 4) << 16), 0u);
     }
     __syncwarp();
     const double s_ref = *P.scale_ref;
@@ -204,15 +204,15 @@ gather_kernel(const GatherParams P) {
                 m &= m - 1u;
                 return hidx;
             };
-#define K3_LOAD(h, g, Z0, Z1, Z2, Z3, U0, U1, U2, U3, V0, V1, WT)                                                          \
-    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(Z0), "=l"(Z1) : "r"(z_s + 32u * (h)));                           \
-    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(Z2), "=l"(Z3) : "r"(z_s + 32u * (h) + 16u));                     \
+#define K3_GW(h, G, WT) asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=r"(G), "=r"(WT) : "r"(gw_s + 8u * (h)));
+#define K3_LOAD(h, g, Z0, Z1, Z2, Z3, U0, U1, U2, U3, V0, V1)                                                              \
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(Z0), "=l"(Z1) : "r"(z_s + 16u * (h)));                           \
+    asm volatile("ld.shared.v2.b64 {%0, %1}, [%2];" : "=l"(Z2), "=l"(Z3) : "r"(z_s + kZHalf + 16u * (h)));                  \
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(U0), "=f"(U1), "=f"(U2), "=f"(U3) : "r"(cu + ((g) & 0xffffu))); \
-    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(V0), "=f"(V1) : "r"(cv + ((g) >> 16)));                          \
-    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(WT) : "r"(w_s + 4u * (h)));
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(V0), "=f"(V1) : "r"(cv + ((g) >> 16)));
 #define K3_FMA(Z0, Z1, Z2, Z3, U0, U1, U2, U3, V0, V1, WT)                                                                 \
     {                                                                                                                      \
-        const float kvw[2] = {V0 * WT, V1 * WT};                                                                           \
+        const float kvw[2] = {V0 * __uint_as_float(WT), V1 * __uint_as_float(WT)};                                                                         \
         const float kuu[4] = {U0, U1, U2, U3};                                                                             \
         _Pragma("unroll") for (int i = 0; i < 2; ++i) _Pragma("unroll") for (int j = 0; j < 4; ++j) {                       \
             const float kq = kvw[i] * kuu[j];                                                                              \
@@ -225,31 +225,35 @@ gather_kernel(const GatherParams P) {
     }
             if (steps > 0) {
                 u64 az0, az1, az2, az3, bz0, bz1, bz2, bz3;
-                float au0, au1, au2, au3, av0, av1, aw, bu0, bu1, bu2, bu3, bv0, bv1, bw;
+                float au0, au1, au2, au3, av0, av1, bu0, bu1, bu2, bu3, bv0, bv1;
+                unsigned aw, bw;                                           // weights (bits) of the visits in flight
                 const unsigned h0 = next_hit();
                 unsigned h1 = next_hit(), h2 = next_hit();
-                unsigned g1, g2;
+                unsigned g1, g2, w2;
                 {
                     unsigned g0;
-                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g0) : "r"(geo_s + 4u * h0));
-                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g1) : "r"(geo_s + 4u * h1));
-                    K3_LOAD(h0, g0, az0, az1, az2, az3, au0, au1, au2, au3, av0, av1, aw)
+                    K3_GW(h0, g0, aw)
+                    K3_GW(h1, g1, bw)
+                    K3_LOAD(h0, g0, az0, az1, az2, az3, au0, au1, au2, au3, av0, av1)
                 }
 #pragma unroll 1
                 for (int v = 0; v < steps; v += 2) {
-                    K3_LOAD(h1, g1, bz0, bz1, bz2, bz3, bu0, bu1, bu2, bu3, bv0, bv1, bw)
-                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g2) : "r"(geo_s + 4u * h2));
+                    K3_LOAD(h1, g1, bz0, bz1, bz2, bz3, bu0, bu1, bu2, bu3, bv0, bv1)
+                    K3_GW(h2, g2, w2)
                     const unsigned h3 = next_hit();
                     K3_FMA(az0, az1, az2, az3, au0, au1, au2, au3, av0, av1, aw)
                     if (v + 1 >= steps) break;
-                    K3_LOAD(h2, g2, az0, az1, az2, az3, au0, au1, au2, au3, av0, av1, aw)
-                    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(g1) : "r"(geo_s + 4u * h3));
+                    aw = w2;
+                    K3_LOAD(h2, g2, az0, az1, az2, az3, au0, au1, au2, au3, av0, av1)
+                    const unsigned wb_cur = bw;
+                    K3_GW(h3, g1, bw)
                     const unsigned h4 = next_hit();
-                    K3_FMA(bz0, bz1, bz2, bz3, bu0, bu1, bu2, bu3, bv0, bv1, bw)
+                    K3_FMA(bz0, bz1, bz2, bz3, bu0, bu1, bu2, bu3, bv0, bv1, wb_cur)
                     h1 = h3;
                     h2 = h4;
                 }
             }
+#undef K3_GW
 #undef K3_LOAD
 #undef K3_FMA
             __syncwarp();
@@ -336,16 +340,16 @@ gather_kernel(const GatherParams P) {
                 if (n_buf + cnt > kCap) { consume(n_buf); n_buf = 0; }
                 if (hit) {
                     const int slot = n_buf + __popc(ball & lt_mask);
-                    wsm->geo[slot] = geo;
+                    wsm->gw[slot].x = geo;
                     wsm->mask[slot] = mask;
                     // the sample's 32 B of visibilities and its weight go straight to the buffer, asynchronously: they land
                     // while the scan goes on
                     const size_t sidx = (size_t)row * P.n_chan + c;
                     const float4* src = P.vis + 2 * sidx;
-                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(z_s + 32u * slot), "l"(src) : "memory");
-                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(z_s + 32u * slot + 16u), "l"(src + 1) : "memory");
-                    if (has_w) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(w_s + 4u * slot), "l"(P.weights + sidx) : "memory");
-                    else wsm->w[slot] = 1.0f;
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(z_s + 16u * slot), "l"(src) : "memory");
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(z_s + kZHalf + 16u * slot), "l"(src + 1) : "memory");
+                    if (has_w) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(gw_s + 8u * slot + 4u), "l"(P.weights + sidx) : "memory");
+                    else wsm->gw[slot].y = __float_as_uint(1.0f);
                 }
                 n_buf += cnt;
             }
