@@ -279,18 +279,21 @@ gather_kernel(const GatherParams P) {
             const int total = __shfl_sync(0xffffffffu, incl, 31);
             const int excl = incl - len;
             if (total == 0) continue;
+            // groups of 8 consecutive candidates (one 128 B line of uv records, one sector of row ids) are the unit that is
+            // scattered: group position gj -> group (gj * S) mod ng
+            const int ng = (total + 7) >> 3;
             int S = 1;
-            if (total >= 64) {
-                S = (int)(((long long)total * 618) / 1000) | 1;
+            if (ng >= 8) {
+                S = (int)(((long long)ng * 618) / 1000) | 1;
                 for (;; S += 2) {
-                    int ga = total, gb = S;
+                    int ga = ng, gb = S;
                     while (gb) { const int t = ga % gb; ga = gb; gb = t; }
                     if (ga == 1) break;
                 }
             }
-            const int step32 = (int)(((long long)32 * S) % total);
-            int f = (int)(((long long)lane * S) % total);
-            // candidate position of chunk `cb` for this lane, and its uv record one chunk ahead of its use
+            const int gstep = (int)(((long long)4 * S) % ng);
+            int gp = (int)(((long long)(lane >> 3) * S) % ng);               // the lane's current group
+            int f = gp * 8 + (lane & 7);
             auto locate = [&](int cb, int& row, double2& p) {
                 int lo = 0;                                                  // smallest bucket row with incl > f
 #pragma unroll
@@ -300,20 +303,21 @@ gather_kernel(const GatherParams P) {
                 }
                 lo = min(lo, 31);
                 const int k = __shfl_sync(0xffffffffu, k0, lo) + (f - __shfl_sync(0xffffffffu, excl, lo));
-                f += step32;
-                if (f >= total) f -= total;
                 p = make_double2(0.0, 0.0);
-                row = 0;
-                if (cb + lane < total) { p = __ldg(P.uv_sorted + k); row = __ldg(P.perm + k); }
+                row = -1;                                                    // -1: no candidate at this position
+                if ((cb >> 3) + (lane >> 3) < ng && f < total) { p = __ldg(P.uv_sorted + k); row = __ldg(P.perm + k); }   // positions >= ng would wrap around
+                gp += gstep;
+                if (gp >= ng) gp -= ng;
+                f = gp * 8 + (lane & 7);
             };
             int row_nx;
             double2 p_nx;
             locate(0, row_nx, p_nx);
-            for (int cb = 0; cb < total; cb += 32) {
-                const bool in_range = cb + lane < total;
+            for (int cb = 0; cb < ng * 8; cb += 32) {
                 const int row = row_nx;
+                const bool in_range = row >= 0;
                 const double2 p = p_nx;
-                if (cb + 32 < total) locate(cb + 32, row_nx, p_nx);
+                if (cb + 32 < ng * 8) locate(cb + 32, row_nx, p_nx);
                 bool hit = false;
                 unsigned geo = 0, mask = 0;
                 if (in_range) {
@@ -346,9 +350,17 @@ gather_kernel(const GatherParams P) {
                     // while the scan goes on
                     const size_t sidx = (size_t)row * P.n_chan + c;
                     const float4* src = P.vis + 2 * sidx;
+#ifdef K3_NO_L2_PREFETCH
                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(z_s + 16u * slot), "l"(src) : "memory");
                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(z_s + kZHalf + 16u * slot), "l"(src + 1) : "memory");
                     if (has_w) asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(gw_s + 8u * slot + 4u), "l"(P.weights + sidx) : "memory");
+#else
+                    // .L2::128B: a miss brings the whole 128 B line into L2 - the same sample's next 3 channels (visibilities)
+                    // or 31 channels (weights), which the items claimed with this one ask for within microseconds
+                    asm volatile("cp.async.cg.shared.global.L2::128B [%0], [%1], 16;" ::"r"(z_s + 16u * slot), "l"(src) : "memory");
+                    asm volatile("cp.async.cg.shared.global.L2::128B [%0], [%1], 16;" ::"r"(z_s + kZHalf + 16u * slot), "l"(src + 1) : "memory");
+                    if (has_w) asm volatile("cp.async.ca.shared.global.L2::128B [%0], [%1], 4;" ::"r"(gw_s + 8u * slot + 4u), "l"(P.weights + sidx) : "memory");
+#endif
                     else wsm->gw[slot].y = __float_as_uint(1.0f);
                 }
                 n_buf += cnt;
