@@ -156,6 +156,9 @@ def run_ours(args):
         cfg = scaled(cfg, n_chan=args.n_chan, f_lo_hz=cfg.f_hi_hz - step_hz * (args.n_chan - 1))
     dev = torch.device("cuda", lr)
     g = generate(cfg, device=dev)
+    if args.row_order == "baseline-major":          # comparison runs of design 2 (K3b): [baseline][integration] rows
+        from gen import baseline_major
+        g = baseline_major(g)
     plan = lib.Plan(cfg.grid_n, g.cell_du, cfg.support_W, cfg.oversample_O, g.kernel_table, design=args.design)
     lib.mwa_grid_plan_set_profiling(plan.handle, True)
     grid = torch.empty((cfg.n_chan, 4, cfg.grid_n, cfg.grid_n), dtype=torch.complex64, device=dev)
@@ -248,7 +251,7 @@ def run_ours(args):
         "config": {"workload": f"{cfg.name}: {cfg.n_ant} antennas, {cfg.n_vis} rows x {cfg.n_chan} channels x 4 pol, "
                                f"grid {cfg.grid_n}^2 per channel and pol, kernel {cfg.support_W}x{cfg.support_W} "
                                f"oversampling {cfg.oversample_O}",
-                   "design": args.design, "design_ran": ran, "per_gpu": "one full snapshot per rank",
+                   "design": args.design, "design_ran": ran, "row_order": args.row_order, "per_gpu": "one full snapshot per rank",
                    "cache": "256 MB L2 flush before every step" if small else
                             f"inputs+outputs {alg_bytes / 1e9:.1f} GB >> 126 MB L2, no flush"},
         "kernel_tap_updates_per_sec": value * cfg.support_W ** 2,
@@ -261,6 +264,7 @@ def run_ours(args):
                      "algorithmic_bytes_per_launch": alg_bytes,
                      "whole_call_frac": alg_bytes / (ms_per_step * 1e-3) / 1e9 / peak,
                      "fp32_peak_tflops_measured": {"fma.rn.f32": fp32_ffma, "fma.rn.f32x2": fp32_ffma2},
+                     "smem_atomic_peak_lane_ops_per_s": lib.mwa_grid_probe_smem_atomics(plan.handle),
                      "fp32_time_ms_at_measured_peak": cfg.tap_updates() * 4 / (fp32_peak * 1e12) * 1e3,
                      "hbm_time_ms_at_peak": alg_bytes / (peak * 1e9) * 1e3},
         "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
@@ -318,6 +322,8 @@ def main():
     ap.add_argument("--config", default="C4", choices=sorted(CONFIGS))
     ap.add_argument("--design", default="auto")
     ap.add_argument("--n-chan", type=int, default=0, help="profiling only: cut the config down to this many channels")
+    ap.add_argument("--row-order", default="generated", choices=["generated", "baseline-major"],
+                    help="comparison runs only: reorder the rows of a multi-integration config [baseline][integration]")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

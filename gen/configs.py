@@ -202,3 +202,16 @@ def generate(cfg: GridConfig, device="cpu", rows_per_chunk: int = 0) -> GridInpu
 
     table = torch.from_numpy(make_kernel_table(cfg.support_W, cfg.oversample_O))
     return GridInputs(cfg, uv, freqs_cpu.to(dev), vis, w, du, table, sky)
+
+
+def baseline_major(g: GridInputs) -> GridInputs:
+    """The same rows reordered [baseline][integration] (generated order is [integration][baseline]): consecutive rows are
+    then the consecutive integrations of one baseline, 1 - 3.4 cells apart in C5 - the order a correlator dump in
+    "baseline order" has and the one the register-ownership design (K3b) is made for.  No-op for a single integration."""
+    cfg = g.cfg
+    if cfg.n_int <= 1 or cfg.conjugates:
+        return g
+    nb = cfg.n_baselines
+    idx = (torch.arange(cfg.n_int, device=g.uv.device)[None, :] * nb + torch.arange(nb, device=g.uv.device)[:, None]).reshape(-1)
+    return GridInputs(cfg, g.uv[idx].contiguous(), g.freqs, g.vis[idx].contiguous(), g.weights[idx].contiguous(), g.cell_du,
+                      g.kernel_table, g.sources)

@@ -41,8 +41,10 @@ enum {
     MWA_GRID_DESIGN_ROMEIN = 3, /* K3b: threads own cells modulo W, register-resident, flush on cell change */
     MWA_GRID_DESIGN_GATHER = 4, /* K3c: tile-owned, lane = 4x2 cell block of one channel, registers              */
     MWA_GRID_DESIGN_CHAN = 5,   /* K5: tile-owned, lane = channel (32 adjacent channels per warp), registers     */
-    MWA_GRID_DESIGN_CHANWS = 6  /* K6: K5's ownership as a warp-specialised producer / consumer pipeline: exact-index
+    MWA_GRID_DESIGN_CHANWS = 6, /* K6: K5's ownership as a warp-specialised producer / consumer pipeline: exact-index
                                    pre-pass, TMA bulk loads, mbarrier hand-off, tensor-map TMA stores (k_chanws.cu) */
+    MWA_GRID_DESIGN_ROMEIN_SORTED = 7 /* K3b walking the rows in the uv-bucket order of the binning step instead of the
+                                   caller's: the comparison design with the spatial locality a3 can give it */
 };
 
 /* Create a plan (R5-R8 for the table).
@@ -98,10 +100,15 @@ int mwa_grid_plan_last_design(mwa_grid_plan* plan);
 int mwa_grid_plan_set_profiling(mwa_grid_plan* plan, int enabled);
 int mwa_grid_plan_stage_ms(mwa_grid_plan* plan, float* out_ms, int n);
 
-/* Measures the FP32 FMA throughput of the device with a register-only loop (the second term of the roofline of
+/* ---- measurement utilities (csrc/k_probe.cu): not part of the gridding path, used by bench.py and profiles/ only ----
+ * Measures the FP32 FMA throughput of the device with a register-only loop (the second term of the roofline of
  * BASELINE.json north_star needs a measured denominator): out_tflops[0] = fma.rn.f32, out_tflops[1] = fma.rn.f32x2,
  * both in TFLOP/s (2 flop per FMA).  HOST pointer to 2 doubles.  Synchronous; takes a few milliseconds. */
 int mwa_grid_probe_fp32(mwa_grid_plan* plan, double* out_tflops, void* stream);
+
+/* Conflict-free red.shared.add.f32 rate of the whole device in lane-atomics per second (every lane its own bank): the
+ * peak that K3a's shared-memory atomic throughput is compared with.  HOST pointer to 1 double.  Synchronous. */
+int mwa_grid_probe_smem_atomics(mwa_grid_plan* plan, double* out_rate, void* stream);
 
 /* Test / diagnostics query (synchronises with the device): counters the last K6 gridding call left behind, written
  * into HOST array `out` (up to 8 values): [0] pipeline error code (0 = none; non-zero means a bounded wait inside the

@@ -11,9 +11,9 @@ import torch
 
 from . import _build
 
-DESIGN_AUTO, DESIGN_ATOMIC, DESIGN_SMEM, DESIGN_ROMEIN, DESIGN_GATHER, DESIGN_CHAN, DESIGN_CHANWS = 0, 1, 2, 3, 4, 5, 6
+DESIGN_AUTO, DESIGN_ATOMIC, DESIGN_SMEM, DESIGN_ROMEIN, DESIGN_GATHER, DESIGN_CHAN, DESIGN_CHANWS, DESIGN_ROMEIN_SORTED = 0, 1, 2, 3, 4, 5, 6, 7
 DESIGNS = {"auto": DESIGN_AUTO, "atomic": DESIGN_ATOMIC, "smem": DESIGN_SMEM, "romein": DESIGN_ROMEIN,
-           "gather": DESIGN_GATHER, "chan": DESIGN_CHAN, "chanws": DESIGN_CHANWS}
+           "gather": DESIGN_GATHER, "chan": DESIGN_CHAN, "chanws": DESIGN_CHANWS, "romein_sorted": DESIGN_ROMEIN_SORTED}
 
 if not os.path.exists(_build.LIB):
     raise ImportError(f"{_build.LIB} is missing: the CUDA library has not been built "
@@ -52,13 +52,15 @@ _lib.mwa_image_from_grid.argtypes = [_P, _P, _P, _LL, _P]
 _lib.mwa_image_from_grid.restype = _I
 _lib.mwa_image_correction.argtypes = [_P, _P, _I]
 _lib.mwa_image_correction.restype = _I
+_lib.mwa_grid_probe_smem_atomics.argtypes = [_P, _P, _P]
+_lib.mwa_grid_probe_smem_atomics.restype = _I
 _lib.mwa_grid_last_error.argtypes = []
 _lib.mwa_grid_last_error.restype = ctypes.c_char_p
 
 EXPORTS = ["mwa_grid_plan_create", "mwa_grid_plan_destroy", "mwa_grid_visibilities", "mwa_grid_visibilities_host",
            "mwa_grid_compute_indices", "mwa_grid_plan_set_design", "mwa_grid_plan_set_profiling",
            "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_plan_last_design", "mwa_grid_plan_last_stats", "mwa_grid_plan_set_list_pool", "mwa_grid_probe_fp32", "mwa_grid_last_error",
-           "mwa_image_from_grid", "mwa_image_correction"]
+           "mwa_image_from_grid", "mwa_image_correction", "mwa_grid_probe_smem_atomics"]
 
 
 class MwaGridError(RuntimeError):
@@ -172,6 +174,13 @@ def mwa_grid_plan_last_stats(plan):
     _check(_lib.mwa_grid_plan_last_stats(plan, ctypes.cast(buf, ctypes.c_void_p), 32))
     return {"error": int(buf[0]), "items": int(buf[1]), "items_with_hits": int(buf[2]), "batches": int(buf[3]),
             "max_hits": int(buf[4]), "swept_items": int(buf[5]), "k5_dense_items": int(buf[6]), "timing": [int(x) for x in buf[8:32]]}
+
+
+def mwa_grid_probe_smem_atomics(plan, stream=None) -> float:
+    """Conflict-free red.shared.add.f32 lane-atomics per second of the whole device (measurement utility)."""
+    buf = (ctypes.c_double * 1)()
+    _check(_lib.mwa_grid_probe_smem_atomics(plan, ctypes.cast(buf, ctypes.c_void_p), _stream_ptr(stream)))
+    return float(buf[0])
 
 
 def mwa_grid_plan_set_list_pool(plan, entries: int) -> None:

@@ -164,7 +164,8 @@ static int grid_device(Plan* p, const double* uv, const double* freqs, const flo
         switch (design) {
             case MWA_GRID_DESIGN_ATOMIC: ok = launch_atomic(p, uv, vis, weights, n_vis, n_chan, grid, st); break;
             case MWA_GRID_DESIGN_SMEM: ok = launch_smem(p, vis, weights, n_vis, n_chan, grid, st); break;
-            case MWA_GRID_DESIGN_ROMEIN: ok = launch_romein(p, uv, vis, weights, n_vis, n_chan, grid, st); break;
+            case MWA_GRID_DESIGN_ROMEIN: ok = launch_romein(p, uv, vis, weights, n_vis, n_chan, grid, nullptr, st); break;
+            case MWA_GRID_DESIGN_ROMEIN_SORTED: ok = launch_romein(p, uv, vis, weights, n_vis, n_chan, grid, p->ws.d_perm, st); break;
             case MWA_GRID_DESIGN_GATHER: ok = launch_gather(p, vis, weights, n_vis, n_chan, grid, nullptr, st); break;
             case MWA_GRID_DESIGN_CHAN: ok = launch_chan(p, vis, weights, n_vis, n_chan, grid, nullptr, st); break;
             case MWA_GRID_DESIGN_CHANWS: ok = launch_chanws(p, vis, weights, n_vis, n_chan, grid, nullptr, st); break;
@@ -278,7 +279,7 @@ int mwa_image_correction(mwa_grid_plan* plan, double* out_corr, int n) {
 
 int mwa_grid_plan_set_design(mwa_grid_plan* plan, int design) {
     if (!plan) { set_error("plan is NULL"); return MWA_GRID_ERR_INVALID; }
-    if (design < MWA_GRID_DESIGN_AUTO || design > MWA_GRID_DESIGN_CHANWS) { set_error("unknown design"); return MWA_GRID_ERR_INVALID; }
+    if (design < MWA_GRID_DESIGN_AUTO || design > MWA_GRID_DESIGN_ROMEIN_SORTED) { set_error("unknown design"); return MWA_GRID_ERR_INVALID; }
     reinterpret_cast<Plan*>(plan)->design = design;
     return MWA_GRID_OK;
 }
@@ -309,6 +310,11 @@ int mwa_grid_probe_fp32(mwa_grid_plan* plan, double* out_tflops, void* stream) {
     if (!plan || !out_tflops) { set_error("bad argument"); return MWA_GRID_ERR_INVALID; }
     return probe_fp32(reinterpret_cast<Plan*>(plan), &out_tflops[0], &out_tflops[1], reinterpret_cast<cudaStream_t>(stream))
                ? MWA_GRID_OK : MWA_GRID_ERR_CUDA;
+}
+
+int mwa_grid_probe_smem_atomics(mwa_grid_plan* plan, double* out_rate, void* stream) {
+    if (!plan || !out_rate) { set_error("bad argument"); return MWA_GRID_ERR_INVALID; }
+    return probe_smem_atomics(reinterpret_cast<Plan*>(plan), out_rate, reinterpret_cast<cudaStream_t>(stream)) ? MWA_GRID_OK : MWA_GRID_ERR_CUDA;
 }
 
 int mwa_grid_plan_set_list_pool(mwa_grid_plan* plan, long long entries) {

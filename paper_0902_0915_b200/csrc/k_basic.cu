@@ -151,73 +151,3 @@ bool launch_atomic(Plan* p, const double* uv, const float* vis, const float* w, 
 }
 
 }  // namespace mwa
-
-// ---------------------------------------------------------------- FP32 peak probe (bench.py roofline denominator)
-// Register-only dependent-chain-free FMA loops: 8 independent accumulators per thread, 4 resident CTAs of 256 threads
-// per SM.  Variant 0 issues fma.rn.f32 (FFMA), variant 1 fma.rn.f32x2 (FFMA2, two fp32 FMAs per lane per instruction).
-namespace mwa {
-
-template <int VARIANT>
-__global__ void __launch_bounds__(256) fp32_probe_kernel(float* out, int iters, float seed) {
-    float a[8], b[8];
-#pragma unroll
-    for (int k = 0; k < 8; ++k) { a[k] = seed + k + threadIdx.x; b[k] = seed * 0.5f + k; }
-    const float m = 1.0000001f, c = 1e-7f;
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int r = 0; r < 8; ++r) {
-            if (VARIANT == 0) {
-#pragma unroll
-                for (int k = 0; k < 8; ++k) { a[k] = fmaf(a[k], m, c); b[k] = fmaf(b[k], m, c); }
-            } else {
-#pragma unroll
-                for (int k = 0; k < 8; ++k) {
-                    unsigned long long v, mm, cc;
-                    asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(a[k]), "f"(b[k]));
-                    asm("mov.b64 %0, {%1, %1};" : "=l"(mm) : "f"(m));
-                    asm("mov.b64 %0, {%1, %1};" : "=l"(cc) : "f"(c));
-                    asm("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(v) : "l"(mm), "l"(cc));
-                    asm("mov.b64 {%0, %1}, %2;" : "=f"(a[k]), "=f"(b[k]) : "l"(v));
-                }
-            }
-        }
-    }
-    float s = 0.f;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) s += a[k] + b[k];
-    if (s == 12345.678f) out[0] = s;                               // keeps the loop alive
-}
-
-// Returns TFLOP/s (2 flop per FMA) of the two variants; synchronous on `st`.
-bool probe_fp32(Plan* p, double* tflops_ffma, double* tflops_ffma2, cudaStream_t st) {
-    float* d = nullptr;
-    if (!cuda_ok(cudaMalloc((void**)&d, 4), "probe malloc")) return false;
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0);
-    cudaEventCreate(&e1);
-    const int iters = 4096, blocks = p->sm_count * 8;
-    double res[2] = {0, 0};
-    for (int v = 0; v < 2; ++v) {
-        float best = 1e30f;
-        for (int rep = 0; rep < 4; ++rep) {
-            cudaEventRecord(e0, st);
-            if (v == 0) fp32_probe_kernel<0><<<blocks, 256, 0, st>>>(d, iters, 1.0f);
-            else fp32_probe_kernel<1><<<blocks, 256, 0, st>>>(d, iters, 1.0f);
-            cudaEventRecord(e1, st);
-            cudaEventSynchronize(e1);
-            float ms = 0;
-            cudaEventElapsedTime(&ms, e0, e1);
-            if (rep > 0 && ms < best) best = ms;
-        }
-        const double fmas = (double)blocks * 256 * iters * 8 * 16;      // 16 fp32 FMAs per inner k-loop pass, 8 passes
-        res[v] = 2.0 * fmas / (best * 1e-3) / 1e12;
-    }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    cudaFree(d);
-    *tflops_ffma = res[0];
-    *tflops_ffma2 = res[1];
-    return cuda_ok(cudaGetLastError(), "fp32 probe");
-}
-
-}  // namespace mwa

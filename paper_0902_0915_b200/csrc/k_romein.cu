@@ -21,6 +21,7 @@ struct RomeinParams {
     GridGeom g;
     const double* scale;
     const double2* uv;          // [n_vis] caller order
+    const int* perm;            // walk order: position -> row (the uv-bucket order of k_bin.cu), or null = caller order
     const float4* vis;
     const float* weights;
     const float* table;
@@ -58,10 +59,11 @@ __global__ void romein_kernel(const RomeinParams P) {
     };
     for (long long rb = r0; rb < r1; rb += 32) {
         // lane = one sample of the batch
-        const long long n = rb + lane;
+        const long long pos = rb + lane;
         int iu = -1, iv = 0, ru = 0, rv = 0;
         float z[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-        if (n < r1) {
+        if (pos < r1) {
+            const long long n = P.perm ? (long long)__ldg(P.perm + pos) : pos;
             const double2 p = P.uv[n];
             SampleIndex s;
             if (sample_index(p.x, p.y, sc, g, s)) {
@@ -103,7 +105,7 @@ __global__ void romein_kernel(const RomeinParams P) {
 }
 
 bool launch_romein(Plan* p, const double* uv, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
-                   cudaStream_t st) {
+                   const int* perm, cudaStream_t st) {
     const size_t bytes = (size_t)n_chan * 4 * p->geom.N * p->geom.N * 8;
     if (!cuda_ok(cudaMemsetAsync(grid, 0, bytes, st), "memset grid")) return false;
     p->last_launches += 1;
@@ -111,6 +113,7 @@ bool launch_romein(Plan* p, const double* uv, const float* vis, const float* w, 
     P.g = p->geom;
     P.scale = p->ws.d_scale;
     P.uv = (const double2*)uv;
+    P.perm = perm;
     P.vis = (const float4*)vis;
     P.weights = w;
     P.table = p->d_table;

@@ -88,6 +88,7 @@ bool launch_binning(Plan* p, const double* uv, long long n_vis, int n_chan, cuda
 bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                    const int* dispatch, cudaStream_t st);
 bool probe_fp32(Plan* p, double* tflops_ffma, double* tflops_ffma2, cudaStream_t st);
+bool probe_smem_atomics(Plan* p, double* lane_atomics_per_s, cudaStream_t st);
 bool chan_supported(const Plan* p, int n_chan);
 bool launch_chan(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                  const int* dispatch, cudaStream_t st);
@@ -101,6 +102,6 @@ bool launch_image(Plan* p, const float* grid, float* image, long long n_planes, 
 const double* image_correction_host(Plan* p, cudaStream_t st);
 void image_release(Plan* p);
 bool launch_romein(Plan* p, const double* uv, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
-                   cudaStream_t st);
+                   const int* perm, cudaStream_t st);
 
 }  // namespace mwa

@@ -14,7 +14,7 @@ from parity import assert_parity
 
 pytestmark = pytest.mark.gpu
 C = 299792458.0
-DESIGNS = ["atomic", "smem", "romein", "gather", "chan", "chanws"]
+DESIGNS = ["atomic", "smem", "romein", "romein_sorted", "gather", "chan", "chanws"]
 
 
 @pytest.fixture(scope="module")
