@@ -222,8 +222,20 @@ class Plan:
 
     def grid(self, uv, freqs, vis, weights=None, out=None, stream=None):
         n_vis, n_chan = int(uv.shape[0]), int(freqs.shape[0])
+        # the C ABI takes bare pointers and sizes: a wrong shape or device here would read or write out of bounds
+        if tuple(uv.shape) != (n_vis, 2):
+            raise ValueError(f"uv must be [n_vis, 2], got {tuple(uv.shape)}")
+        if vis is not None and tuple(vis.shape) != (n_vis, n_chan, 4):
+            raise ValueError(f"vis must be [n_vis={n_vis}, n_chan={n_chan}, 4], got {tuple(vis.shape)}")
+        if weights is not None and tuple(weights.shape) != (n_vis, n_chan):
+            raise ValueError(f"weights must be [n_vis={n_vis}, n_chan={n_chan}], got {tuple(weights.shape)}")
         if out is None:
             out = torch.empty((n_chan, 4, self.grid_n, self.grid_n), dtype=torch.complex64, device=uv.device)
+        elif tuple(out.shape) != (n_chan, 4, self.grid_n, self.grid_n):
+            raise ValueError(f"out must be [n_chan={n_chan}, 4, {self.grid_n}, {self.grid_n}], got {tuple(out.shape)}")
+        for name, t in (("freqs", freqs), ("vis", vis), ("weights", weights), ("out", out)):
+            if t is not None and t.device != uv.device:
+                raise ValueError(f"{name} lives on {t.device}, uv on {uv.device}: all arguments must be on the plan's device")
         mwa_grid_visibilities(self.handle, uv, freqs, vis, weights, n_vis, n_chan, out, stream)
         return out
 

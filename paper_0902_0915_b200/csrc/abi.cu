@@ -77,7 +77,8 @@ static int ensure_workspace(Plan* p, long long n_vis, int n_chan) {
         ws.cap_tiles = n_tiles;
     }
     if (!ws.d_misc && !ensure(ws.d_misc, (size_t)kMiscInts, "misc")) return MWA_GRID_ERR_NOMEM;
-    const bool want_ws = (p->design == MWA_GRID_DESIGN_CHANWS || p->design == MWA_GRID_DESIGN_AUTO) && chanws_supported(p, n_chan);
+    const bool want_ws = (p->design == MWA_GRID_DESIGN_CHANWS || (p->design == MWA_GRID_DESIGN_AUTO && n_chan >= kChanMinChannels)) &&
+                         chanws_supported(p, n_chan);
     const size_t n_pre = want_ws ? (size_t)n_vis * (size_t)((n_chan + 31) / 32) * 32 : 0;
     if (n_pre > ws.cap_pre) {
         ws.cap_pre = 0;
@@ -173,6 +174,13 @@ static int grid_device(Plan* p, const double* uv, const double* freqs, const flo
                 // the choice is made on the device by scale_kernel (the host never reads freqs): both kernels
                 // are enqueued and the one that was not picked returns at once
                 ok = true;
+                if (n_chan < kChanMinChannels) {
+                    // the device-side rule can only pick the gather kernel: the channel-SIMD kernels and their pre-passes
+                    // are not enqueued at all (small single-channel calls are launch-bound)
+                    p->last_chanws = false;
+                    ok = launch_gather(p, vis, weights, n_vis, n_chan, grid, nullptr, st);
+                    break;
+                }
                 p->last_chanws = chanws_supported(p, n_chan);
                 if (p->last_chanws) ok = launch_chanws(p, vis, weights, n_vis, n_chan, grid, p->ws.d_dispatch, st);
                 else if (chan_supported(p, n_chan)) ok = launch_chan(p, vis, weights, n_vis, n_chan, grid, p->ws.d_dispatch, st);

@@ -12,7 +12,7 @@ namespace mwa {
 // needs the 32 channels of a group to see a baseline at almost the same cell.  drift = largest displacement,
 // in cells at the grid edge, between the extreme channels of any group.
 constexpr double kChanMaxDriftCells = 6.0;
-constexpr int kChanMinChannels = 8;
+
 
 __global__ void scale_kernel(const double* __restrict__ freqs, int n_chan, int half_n, int chan_ok,
                              double* __restrict__ scale, double* __restrict__ scale_ref, int* __restrict__ dispatch,

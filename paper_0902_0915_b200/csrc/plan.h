@@ -10,6 +10,7 @@ namespace mwa {
 // Binning geometry (a3).  Rows are sorted once per call by the bucket of their position at the TOP
 // frequency of the call (largest extent); every channel's position is a radial contraction of that one.
 constexpr int kBucketCells = 8;     // bucket side in cells at the reference scale
+constexpr int kChanMinChannels = 8; // AUTO picks a channel-SIMD kernel (K6 / K5) only from this many channels on
 constexpr int kTile = 16;           // gridding tile side in cells (one warp owns one tile of one channel)
 // d_misc (ints, zeroed by every call's binning step): [0..3] work counters, [4..11] diagnostics, [12..13] hit-list pool
 // cursor (u64), [14..15] K6 item counts, [16..] tile-weight histogram (4096), then the block states of chan_order_kernel

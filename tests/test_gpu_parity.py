@@ -423,3 +423,25 @@ def test_image_from_grid_matches_the_oracle_chain_and_the_direct_dft(lib, W, O, 
     # GPU chain is fp32 (gridding 1e-5 A per cell, cuFFT single precision) and the correction amplifies its rounding by
     # up to 1 / c^(N/4)^2 = 450 at the corner of the inner half: measured 1.9e-6, bound 5e-6
     assert err <= max(tol_q, 5e-6), err
+
+
+# ---------------------------------------------------------------------------- f4: channel-sharded driver
+def test_channel_sharded_driver_matches_the_unsharded_call(lib):
+    """Two (and three) ranks' calls, run one after the other on this one GPU, write disjoint planes of one grid_out that
+    passes parity against the oracle's whole-band grid.  (Not bit-identical to the unsharded call: a call bins its rows at
+    its OWN top frequency, so a shard sums the same taps in another order.)"""
+    from paper_0902_0915_b200.shard import grid_channel_shard
+    g = generate(_fine(dict(n_ant=64, core_ant=32, n_chan=100, grid_n=256)))
+    G, A, _ = _oracle(g)
+    _to_dev(g)
+    with _plan(lib, g) as p:
+        for ws in (2, 3):
+            out = torch.full((g.cfg.n_chan, 4, g.cfg.grid_n, g.cfg.grid_n), float("nan"), dtype=torch.complex64, device="cuda")
+            covered = []
+            for rank in range(ws):
+                part, (c0, c1) = grid_channel_shard(p, g.uv, g.freqs, g.vis, g.weights, ws, rank, out=out)
+                assert part.data_ptr() == out[c0:c1].data_ptr()
+                covered += list(range(c0, c1))
+            torch.cuda.synchronize()
+            assert covered == list(range(g.cfg.n_chan))
+            assert_parity(out.cpu().numpy(), G, A, f"{ws} channel shards")

@@ -7,7 +7,7 @@ import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
-from paper_0902_0915_b200.shard import GROUP, channel_range, shard_inputs
+from paper_0902_0915_b200.shard import GROUP, abi_arguments, channel_range, shard_inputs
 
 
 def test_channel_ranges_cover_every_channel_once():
@@ -48,6 +48,20 @@ def _worker(rank, ws, port, n_vis, n_chan, out):
     part[c0:c1] = (v.to(torch.complex128) * w[..., None]).sum(dim=(0, 2))
     parts = [torch.zeros_like(part) for _ in range(ws)]
     dist.all_gather(parts, part)                                      # test-only exchange
+    # the argument list each rank would hand to the C ABI (f4): rank 0 checks that the plane ranges tile grid_out
+    grid_n = 64
+    a = abi_arguments(n_vis, n_chan, grid_n, ws, rank)
+    assert a["n_chan"] == c1 - c0 and a["freqs_offset"] == c0 and a["vis_copy_elems"] == v.numel()
+    assert a["weights_copy_elems"] == w.numel() and a["grid_elem_offset"] % (grid_n * grid_n) == 0
+    mine = torch.tensor([a["grid_elem_offset"], a["grid_elems"], a["grid_plane_offset"], a["grid_planes"]], dtype=torch.int64)
+    every = [torch.zeros_like(mine) for _ in range(ws)]
+    dist.all_gather(every, mine)
+    if rank == 0:
+        pos = 0
+        for e in every:                                               # ranks in order: contiguous, no gap, no overlap
+            assert int(e[0]) == pos and int(e[2]) * grid_n * grid_n == pos
+            pos += int(e[1])
+        assert pos == n_chan * 4 * grid_n * grid_n
     if rank == 0:
         whole = (vis.to(torch.complex128) * wts[..., None]).sum(dim=(0, 2))
         out.put((float(t.item()), bool(torch.allclose(sum(parts), whole)),
