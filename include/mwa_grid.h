@@ -67,7 +67,11 @@ mwa_grid_plan* mwa_grid_plan_create(int grid_n, double cell_du, int support_W, i
  *   grid_out [n_chan][4][N][N][2]  float (re, im), row = v, column = u       16-byte aligned
  *            OVERWRITTEN entirely: every cell is written, zeros where no tap lands (R10).
  *   stream   cudaStream_t passed as void* (0 = legacy default stream)
- * Samples whose stamp would leave the grid are dropped whole (R11); that is not an error.
+ * Samples whose stamp would leave the grid are dropped whole (R11); that is not an error, and the visibilities and
+ * weights of dropped samples may hold anything (NaN flags included): they never reach a sum.  The visibilities and
+ * weights of all OTHER samples must be finite: a sample is accumulated into whole 4 x 2-cell register blocks with zero
+ * taps outside its stamp, so a NaN or Inf there would spread to up to 7 cells beyond the stamp (zero the flagged
+ * samples - weight 0 and visibility 0 - before the call).
  * n_chan == 0 is a no-op; n_vis == 0 zero-fills the grid.  Asynchronous: returns after enqueue; the caller's
  * arrays must stay valid until the stream reaches the end of the call. */
 int mwa_grid_visibilities(mwa_grid_plan* plan, const double* uv_f64, const double* freqs,

@@ -206,12 +206,15 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                 asm volatile("cp.async.commit_group;" ::: "memory");
                 // (ii) exact indices -> geo, block mask
                 const double sc = S.sc[gslot][lane];
+                unsigned dropped = 0u;                                             // bit k: this lane's sample of hit warp + k * kcWarps is dropped (R11)
 #pragma unroll 2
                 for (int hh = warp; hh < n; hh += kcWarps) {
                     const double2 p = S.hit_uv[sel[b0 + hh]];
                     SampleIndex s;
                     unsigned geo = zero_geo, mask = 0u;
-                    if (sample_index(p.x, p.y, sc, P.g, s) && cvalid) {
+                    const bool valid = sample_index(p.x, p.y, sc, P.g, s) && cvalid;
+                    if (!valid) dropped |= 1u << (hh / kcWarps);
+                    if (valid) {
                         const int tu_ = kcPadU + hW + X0 - s.iu, tv_ = kcPadV + hW + Y0 - s.iv;   // pad - (stamp origin relative to the tile)
                         const unsigned iu_ = (unsigned)(kcPadU + W - 1 - tu_), iv_ = (unsigned)(kcPadV + W - 1 - tv_);   // ou + W - 1, ov + W - 1
                         if (iu_ < (unsigned)(kcTileX + W - 1) && iv_ < (unsigned)(kcTileY + W - 1)) {
@@ -227,6 +230,14 @@ chan_kernel(const __grid_constant__ ChanParams P) {
                     if (lane == 0) S.hit_mask[hh] = mask;
                 }
                 asm volatile("cp.async.wait_group 0;" ::: "memory");              // visible to the other warps after the barrier
+                // a dropped sample contributes nothing, whatever its visibility holds (a flagged NaN times a zero tap would
+                // still be NaN): its staged visibility is overwritten with zeros.  Rare: only samples at the grid edge.
+                for (; dropped != 0u; dropped &= dropped - 1u) {
+                    const unsigned hh = (unsigned)warp + (unsigned)(__ffs(dropped) - 1) * kcWarps;
+                    asm volatile("st.shared.v4.f32 [%0], {%1, %1, %1, %1};" ::"r"(zs_s + 1024u * hh), "f"(0.0f) : "memory");
+                    asm volatile("st.shared.v4.f32 [%0], {%1, %1, %1, %1};" ::"r"(zs_s + 1024u * hh + 16u), "f"(0.0f) : "memory");
+                    if (HAS_W) asm volatile("st.shared.f32 [%0], %1;" ::"r"(wt_s + 128u * hh), "f"(0.0f) : "memory");
+                }
             };
 
             // ---- B: the warp's block against the n hits of the batch; every lane computes, zeros where it misses

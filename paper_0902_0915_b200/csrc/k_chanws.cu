@@ -959,9 +959,9 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 if (lane == 0) { S.st_n[s] = n; S.st_flags[s] = flags; S.st_tile[s] = tile_c; }
                 for (int hh = 0; hh < n; ++hh) {
                     const int r = __shfl_sync(full, row, hh);
+                    if ((slow_m >> hh) & 1u) continue;                       // uniform
                     if (HAS_W)
                         asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(wt_a + 128u * (unsigned)hh), "l"(P.weights + (size_t)r * P.n_chan + cc) : "memory");
-                    if ((slow_m >> hh) & 1u) continue;                       // uniform
                     asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(geo_a + 128u * (unsigned)hh), "l"(P.pre + (size_t)r * ncp + c0 + lane) : "memory");
 #ifndef K6_ABLATE_LOAD
                     const float* src = P.vis + ((size_t)r * P.n_chan + cc) * 8;
@@ -995,6 +995,8 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                     asm volatile("st.shared.u32 [%0], %1;" ::"r"(geo_a + 128u * (unsigned)hh), "r"(geo) : "memory");
                     const float* src = P.vis + ((size_t)r * P.n_chan + cc) * 8;
                     const unsigned sz = (cvalid && w32 != k6Invalid) ? 16u : 0u;   // zero-filled where the lane has no sample (R11)
+                    if (HAS_W)                                               // the weight as well: a flagged NaN must not reach a product
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(wt_a + 128u * (unsigned)hh), "l"(P.weights + (size_t)r * P.n_chan + cc), "r"(sz >> 2) : "memory");
                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(zs_a + 1024u * (unsigned)hh), "l"(src), "r"(sz) : "memory");
                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(zs_a + 1024u * (unsigned)hh + 512u), "l"(src + 4), "r"(sz) : "memory");
                 }

@@ -276,6 +276,39 @@ def test_single_visibility_stamp_and_dropped_rows(lib):
         assert np.count_nonzero(got[0, 0]) == 2 * W * W
 
 
+@pytest.mark.parametrize("design", DESIGNS + ["auto"])
+def test_dropped_samples_with_nonfinite_values_leave_no_trace(lib, design):
+    # R11: a sample whose stamp leaves the grid is dropped whole - whatever its visibility and weight hold.  Flagged data
+    # often carries NaN there; a kernel that multiplies it by a zero tap instead of skipping it would spread NaN.
+    N, W, O = 256, 7, 8
+    T = make_kernel_table(W, O)
+    n_chan = 40
+    fr = 155e6 + 40e3 * np.arange(n_chan)
+    du = 1.0
+    rs = np.random.RandomState(11)
+    s0 = fr[0] / C
+    edge = np.array([[124.4, 3.0], [-124.45, -60.2], [10.0, 124.3], [-124.0, 124.45], [123.9, -124.4]]) / s0   # valid at
+    uv = np.concatenate([edge, rs.uniform(-100, 100, (300, 2)) / s0])      # channel 0, dropped further up the band
+    idx = oracle.compute_indices(uv, fr, N, du, W, O)
+    drop = idx[:, :, 0] < 0
+    assert drop[:5].any() and not drop[:5].all() and not drop[5:].any()
+    vis = (rs.standard_normal((uv.shape[0], n_chan, 4)) + 1j * rs.standard_normal((uv.shape[0], n_chan, 4))).astype(np.complex64)
+    wts = rs.uniform(0.5, 1.5, (uv.shape[0], n_chan)).astype(np.float32)
+    G, A, _ = oracle.grid(uv, fr, vis, wts, N, du, W, O, T)
+    vis_bad, w_bad = vis.copy(), wts.copy()
+    vis_bad[drop] = np.nan + 1j * np.inf
+    w_bad[drop] = np.nan
+    with lib.Plan(N, du, W, O, T, design=design) as p:
+        t = [torch.from_numpy(x).cuda() for x in (uv, fr, vis_bad, w_bad)]
+        out = p.grid(*t).cpu().numpy()
+        assert np.isfinite(out.view(np.float32)).all(), design
+        assert_parity(out, G, A, design)
+        out2 = p.grid(t[0], t[1], t[2], None).cpu().numpy()              # NULL weights
+        assert np.isfinite(out2.view(np.float32)).all(), design
+    G1, A1, _ = oracle.grid(uv, fr, vis, None, N, du, W, O, T)
+    assert_parity(out2, G1, A1, design + " null weights")
+
+
 def test_empty_inputs_and_error_codes(lib):
     T = make_kernel_table(7, 8)
     with lib.Plan(64, 1.0, 7, 8, T) as p:
