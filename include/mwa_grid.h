@@ -144,6 +144,18 @@ int mwa_grid_plan_last_launches(const mwa_grid_plan* plan);
  * negative error code (MWA_GRID_ERR_CUDA with "cuFFT ... could not be loaded" if the library is missing). */
 int mwa_image_from_grid(mwa_grid_plan* plan, const float* grid, float* image, long long n_planes, void* stream);
 
+/* f2 - Stokes conversion ("the measured instrumental polarization is converted into a set of Stokes
+ * parameters by the application of a 4x4 matrix transformation.  This matrix is a function of time and position on the sky
+ * ... and must be calculated ... for each pixel"; Table 1 row "Stokes Conversion").  The paper gives no
+ * formula for the matrix, so the caller supplies it (R18):
+ *   stokes_out[c][k][q][p] = sum_{j=0..3} matrix[q][p][k][j] * image[c][j][q][p]          (complex, fp32)
+ *   image      [n_chan][4][N][N][2] float, DEVICE: the 4 instrumental planes XX, XY, YX, YY of every channel
+ *   matrix     [N][N][4][4][2]      float, DEVICE, 16-byte aligned: one 4 x 4 complex matrix per pixel, row k, column j,
+ *              shared by all channels of the call
+ *   stokes_out [n_chan][4][N][N][2] float, DEVICE: planes k = 0..3 (I, Q, U, V for a Stokes matrix); may be `image`
+ * One kernel, 32 B read + 32 B written per pixel and channel (HBM-bound).  Asynchronous on `stream`. */
+int mwa_image_stokes(mwa_grid_plan* plan, const float* image, const float* matrix, float* stokes_out, int n_chan, void* stream);
+
 /* The correction function of the plan: out_corr[p'] = c^(p' - N/2) for p' = 0..min(n, N)-1, HOST array of doubles.
  * Returns the number of values written.  Synchronous. */
 int mwa_image_correction(mwa_grid_plan* plan, double* out_corr, int n);

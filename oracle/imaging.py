@@ -38,3 +38,9 @@ def direct_dft(x_cells, y_cells, z, N):
     ex = np.exp(2j * np.pi * np.outer(x_cells, p) / N)      # [n, p]
     ey = np.exp(2j * np.pi * np.outer(y_cells, p) / N)      # [n, q]
     return np.einsum("n,nq,np->qp", np.asarray(z, dtype=np.complex128), ey, ex)
+
+
+def stokes(image, matrix):
+    """"converted into a set of Stokes parameters by the application of a 4x4 matrix transformation ...
+    calculated ... for each pixel".  out[c][k][q][p] = sum_j matrix[q][p][k][j] * image[c][j][q][p], in complex128."""
+    return np.einsum("qpkj,cjqp->ckqp", np.asarray(matrix, dtype=np.complex128), np.asarray(image, dtype=np.complex128))

@@ -50,6 +50,8 @@ _lib.mwa_grid_probe_fp32.argtypes = [_P, _P, _P]
 _lib.mwa_grid_probe_fp32.restype = _I
 _lib.mwa_image_from_grid.argtypes = [_P, _P, _P, _LL, _P]
 _lib.mwa_image_from_grid.restype = _I
+_lib.mwa_image_stokes.argtypes = [_P, _P, _P, _P, _I, _P]
+_lib.mwa_image_stokes.restype = _I
 _lib.mwa_image_correction.argtypes = [_P, _P, _I]
 _lib.mwa_image_correction.restype = _I
 _lib.mwa_grid_probe_smem_atomics.argtypes = [_P, _P, _P]
@@ -60,7 +62,7 @@ _lib.mwa_grid_last_error.restype = ctypes.c_char_p
 EXPORTS = ["mwa_grid_plan_create", "mwa_grid_plan_destroy", "mwa_grid_visibilities", "mwa_grid_visibilities_host",
            "mwa_grid_compute_indices", "mwa_grid_plan_set_design", "mwa_grid_plan_set_profiling",
            "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_plan_last_design", "mwa_grid_plan_last_stats", "mwa_grid_plan_set_list_pool", "mwa_grid_probe_fp32", "mwa_grid_last_error",
-           "mwa_image_from_grid", "mwa_image_correction", "mwa_grid_probe_smem_atomics"]
+           "mwa_image_from_grid", "mwa_image_correction", "mwa_image_stokes", "mwa_grid_probe_smem_atomics"]
 
 
 class MwaGridError(RuntimeError):
@@ -194,6 +196,13 @@ def mwa_image_from_grid(plan, grid, image, n_planes, stream=None) -> None:
                                     _ptr(image, torch.complex64, "cuda", "image"), int(n_planes), _stream_ptr(stream)))
 
 
+def mwa_image_stokes(plan, image, matrix, stokes_out, n_chan, stream=None) -> None:
+    """f2: stokes_out[c, k] = sum_j matrix[..., k, j] * image[c, j]; matrix complex64 [N, N, 4, 4]; in place allowed."""
+    _check(_lib.mwa_image_stokes(plan, _ptr(image, torch.complex64, "cuda", "image"),
+                                 _ptr(matrix, torch.complex64, "cuda", "matrix"),
+                                 _ptr(stokes_out, torch.complex64, "cuda", "stokes_out"), int(n_chan), _stream_ptr(stream)))
+
+
 def mwa_image_correction(plan, n: int):
     """The plan's correction function c^(p' - N/2), p' = 0..n-1, as a float64 CPU tensor."""
     out = torch.empty(int(n), dtype=torch.float64)
@@ -244,6 +253,15 @@ class Plan:
         if out is None:
             out = torch.empty_like(grid)
         mwa_image_from_grid(self.handle, grid, out, grid.numel() // (self.grid_n * self.grid_n), stream)
+        return out
+
+    def stokes(self, image, matrix, out=None, stream=None):
+        """Stokes conversion of [n_chan, 4, N, N] images with a [N, N, 4, 4] matrix field; in place when out is image."""
+        if tuple(matrix.shape) != (self.grid_n, self.grid_n, 4, 4) or tuple(image.shape[1:]) != (4, self.grid_n, self.grid_n):
+            raise ValueError("image must be [n_chan, 4, N, N] and matrix [N, N, 4, 4]")
+        if out is None:
+            out = torch.empty_like(image)
+        mwa_image_stokes(self.handle, image, matrix, out, int(image.shape[0]), stream)
         return out
 
     def indices(self, uv, freqs, stream=None):

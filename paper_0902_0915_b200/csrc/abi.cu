@@ -274,6 +274,28 @@ int mwa_image_from_grid(mwa_grid_plan* plan, const float* grid, float* image, lo
     return launch_image(p, grid, image, n_planes, reinterpret_cast<cudaStream_t>(stream)) ? MWA_GRID_OK : MWA_GRID_ERR_CUDA;
 }
 
+int mwa_image_stokes(mwa_grid_plan* plan, const float* image, const float* matrix, float* stokes_out, int n_chan, void* stream) {
+    g_last_error.clear();
+    Plan* p = reinterpret_cast<Plan*>(plan);
+    if (!p) { set_error("plan is NULL"); return MWA_GRID_ERR_INVALID; }
+    if (n_chan < 0) { set_error("n_chan must be >= 0"); return MWA_GRID_ERR_INVALID; }
+    p->last_launches = 0;
+    if (n_chan == 0) return MWA_GRID_OK;
+    if (!image || !matrix || !stokes_out || !aligned(image, 8) || !aligned(stokes_out, 8) || !aligned(matrix, 16)) {
+        set_error("image, matrix and stokes_out must be non-NULL; image / stokes_out 8-byte, matrix 16-byte aligned");
+        return MWA_GRID_ERR_INVALID;
+    }
+    if (image != stokes_out) {
+        const size_t bytes = (size_t)n_chan * 4 * p->geom.N * p->geom.N * 8;
+        const char *a = (const char*)image, *b = (const char*)stokes_out;
+        if (a < b + bytes && b < a + bytes) { set_error("image and stokes_out must be the same buffer or not overlap"); return MWA_GRID_ERR_INVALID; }
+    }
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev), "cudaGetDevice")) return MWA_GRID_ERR_CUDA;
+    if (dev != p->device) { set_error("the current CUDA device is not the device the plan was created on"); return MWA_GRID_ERR_INVALID; }
+    return launch_stokes(p, image, matrix, stokes_out, n_chan, reinterpret_cast<cudaStream_t>(stream)) ? MWA_GRID_OK : MWA_GRID_ERR_CUDA;
+}
+
 int mwa_image_correction(mwa_grid_plan* plan, double* out_corr, int n) {
     g_last_error.clear();
     Plan* p = reinterpret_cast<Plan*>(plan);

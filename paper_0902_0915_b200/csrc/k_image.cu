@@ -195,3 +195,64 @@ bool launch_image(Plan* p, const float* grid, float* image, long long n_planes, 
 }
 
 }  // namespace mwa
+
+// ------------------------------------------------------------------------------------------------ f2: Stokes conversion
+// "the measured instrumental polarization is converted into a set of Stokes parameters by the application of a
+// 4x4 matrix transformation.  This matrix is a function of time and position on the sky relative to the instrument and must
+// be calculated by the RTS for each pixel" (Table 1 row "Stokes Conversion").  The paper gives no formula for
+// the matrix, so it is an INPUT here (R18): one 4 x 4 complex matrix per pixel, shared by all channels of the
+// call ("a function of time and position"), applied across the 4 polarisation planes of every channel:
+//     out[c][k][q][p] = sum_j M[q][p][k][j] * image[c][j][q][p]
+// One thread per pixel keeps its matrix in registers and walks a range of channels: 32 B read + 32 B written per pixel
+// and channel (the 128 B matrix is read once per thread), bound by HBM.  In place is allowed (image == out).
+namespace mwa {
+
+__global__ void __launch_bounds__(256)
+stokes_kernel(const float2* __restrict__ image, const float4* __restrict__ matrix, float2* __restrict__ out, int N, int n_chan,
+              int chan_per_block) {
+    const long long npix = (long long)N * N;
+    const long long pix = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (pix >= npix) return;
+    float2 m[4][4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const float4 a = __ldg(matrix + pix * 8 + k * 2), b = __ldg(matrix + pix * 8 + k * 2 + 1);
+        m[k][0] = make_float2(a.x, a.y); m[k][1] = make_float2(a.z, a.w);
+        m[k][2] = make_float2(b.x, b.y); m[k][3] = make_float2(b.z, b.w);
+    }
+    const int c0 = blockIdx.y * chan_per_block, c1 = min(n_chan, c0 + chan_per_block);
+    for (int c = c0; c < c1; ++c) {
+        const float2* src = image + (long long)c * 4 * npix + pix;
+        float2 v[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) v[j] = src[(long long)j * npix];
+        float2* dst = out + (long long)c * 4 * npix + pix;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            float re = 0.0f, im = 0.0f;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                re = fmaf(m[k][j].x, v[j].x, re); re = fmaf(-m[k][j].y, v[j].y, re);
+                im = fmaf(m[k][j].x, v[j].y, im); im = fmaf(m[k][j].y, v[j].x, im);
+            }
+            dst[(long long)k * npix] = make_float2(re, im);
+        }
+    }
+}
+
+bool launch_stokes(Plan* p, const float* image, const float* matrix, float* out, int n_chan, cudaStream_t st) {
+    const int N = p->geom.N;
+    const long long npix = (long long)N * N;
+    const unsigned bx = (unsigned)((npix + 255) / 256);
+    // enough blocks to fill the device even for a small image: split the channels over blockIdx.y
+    int split = (int)(((long long)p->sm_count * 16 + bx - 1) / bx);
+    if (split < 1) split = 1;
+    if (split > n_chan) split = n_chan;
+    const int per = (n_chan + split - 1) / split;
+    dim3 grid(bx, (unsigned)((n_chan + per - 1) / per));
+    stokes_kernel<<<grid, 256, 0, st>>>((const float2*)image, (const float4*)matrix, (float2*)out, N, n_chan, per);
+    p->last_launches += 1;
+    return cuda_ok(cudaGetLastError(), "stokes_kernel");
+}
+
+}  // namespace mwa

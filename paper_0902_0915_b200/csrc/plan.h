@@ -101,6 +101,7 @@ bool launch_smem(Plan* p, const float* vis, const float* w, long long n_vis, int
                  cudaStream_t st);
 bool launch_image(Plan* p, const float* grid, float* image, long long n_planes, cudaStream_t st);
 const double* image_correction_host(Plan* p, cudaStream_t st);
+bool launch_stokes(Plan* p, const float* image, const float* matrix, float* out, int n_chan, cudaStream_t st);
 void image_release(Plan* p);
 bool launch_romein(Plan* p, const double* uv, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                    const int* perm, cudaStream_t st);

@@ -478,3 +478,22 @@ def test_channel_sharded_driver_matches_the_unsharded_call(lib):
             torch.cuda.synchronize()
             assert covered == list(range(g.cfg.n_chan))
             assert_parity(out.cpu().numpy(), G, A, f"{ws} channel shards")
+
+
+# ---------------------------------------------------------------------------- f2: Stokes conversion
+@pytest.mark.parametrize("N,n_chan", [(64, 5), (250, 2)])
+def test_stokes_conversion_matches_the_oracle(lib, N, n_chan):
+    from gen.stokes import stokes_matrix_field
+    from oracle import imaging
+    rs = np.random.RandomState(9)
+    img = (rs.standard_normal((n_chan, 4, N, N)) + 1j * rs.standard_normal((n_chan, 4, N, N))).astype(np.complex64)
+    M = stokes_matrix_field(N)
+    want = imaging.stokes(img, M)
+    bound = 1e-6 * np.einsum("qpkj,cjqp->ckqp", np.abs(M).astype(np.float64), np.abs(img).astype(np.float64)) + 1e-9
+    with lib.Plan(N, 1.0, 7, 8, make_kernel_table(7, 8)) as p:
+        d_img, d_M = torch.from_numpy(img).cuda(), torch.from_numpy(M).cuda()
+        out = p.stokes(d_img, d_M)
+        assert np.all(np.abs(out.cpu().numpy().astype(np.complex128) - want) <= bound)      # 16 fp32 FMAs per output
+        inplace = d_img.clone()
+        p.stokes(inplace, d_M, out=inplace)
+        assert torch.equal(inplace.view(torch.float32), out.view(torch.float32))

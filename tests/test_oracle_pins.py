@@ -216,3 +216,34 @@ def test_p5_imaging_chain_matches_direct_dft(W, O, tol_q):
     # sanity: the uncorrected image is far off, so the correction (and table addressing) matter
     raw = imaging.dirty_image(G[0, 0]).real
     assert np.max(np.abs(raw - Dq)[inner, inner]) > 0.05 * peak
+
+
+# ------------------------------------------------------------------ f2: Stokes conversion
+def test_stokes_oracle_against_the_textbook_definitions():
+    from gen.stokes import S0, jones_field, mueller_of, stokes_matrix_field
+    rs = np.random.RandomState(5)
+    N, n_chan = 16, 3
+    img = rs.standard_normal((n_chan, 4, N, N)) + 1j * rs.standard_normal((n_chan, 4, N, N))
+    # (1) the constant textbook matrix: I = (XX + YY)/2, Q = (XX - YY)/2, U = (XY + YX)/2, V = -i (XY - YX)/2
+    M0 = np.broadcast_to(S0, (N, N, 4, 4))
+    s = imaging.stokes(img, M0)
+    xx, xy, yx, yy = img[:, 0], img[:, 1], img[:, 2], img[:, 3]
+    assert np.allclose(s[:, 0], (xx + yy) / 2) and np.allclose(s[:, 1], (xx - yy) / 2)
+    assert np.allclose(s[:, 2], (xy + yx) / 2) and np.allclose(s[:, 3], -1j * (xy - yx) / 2)
+    # (2) the identity leaves the planes alone; the map is linear; a transposed matrix (k <-> j) is caught
+    eye = np.broadcast_to(np.eye(4), (N, N, 4, 4))
+    assert np.array_equal(imaging.stokes(img, eye), img)
+    assert np.allclose(imaging.stokes(2 * img + 1j * img[::-1], M0), 2 * s + 1j * imaging.stokes(img[::-1], M0))
+    E = np.zeros((N, N, 4, 4)); E[..., 1, 2] = 1.0                  # out plane 1 <- in plane 2
+    t = imaging.stokes(img, E)
+    assert np.array_equal(t[:, 1], img[:, 2]) and not t[:, [0, 2, 3]].any()
+    # (3) round trip through a direction-dependent instrument: known Stokes -> sky coherency -> J e J^H -> matrix field
+    stokes_true = rs.standard_normal((n_chan, 4, N, N))
+    coh = np.einsum("kj,cjqp->ckqp", np.linalg.inv(S0), stokes_true.astype(np.complex128))
+    measured = np.einsum("qpkj,cjqp->ckqp", mueller_of(jones_field(N)), coh)
+    back = imaging.stokes(measured, stokes_matrix_field(N).astype(np.complex128))
+    assert np.allclose(back, stokes_true, atol=2e-6)               # the field is stored in complex64
+    # per pixel: the matrix of pixel (q, p) is the one applied at (q, p)
+    q, p = 3, 11
+    M = stokes_matrix_field(N).astype(np.complex128)
+    assert np.allclose(imaging.stokes(measured, M)[1, :, q, p], M[q, p] @ measured[1, :, q, p])
