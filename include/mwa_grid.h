@@ -90,6 +90,20 @@ int mwa_grid_visibilities_host(mwa_grid_plan* plan, const double* uv_f64, const 
 int mwa_grid_compute_indices(mwa_grid_plan* plan, const double* uv_f64, const double* freqs,
                              long long n_vis, int n_chan, int* out_idx, void* stream);
 
+/* Dropped-sample counter: the number of (row, channel) samples mwa_grid_visibilities would
+ * drop for these coordinates (R11: a tap outside the grid, |x| >= N/2, or a non-finite coordinate), counted with the same
+ * index function.  out_count is a HOST pointer.  Synchronous (it reads the count back). */
+int mwa_grid_count_dropped(mwa_grid_plan* plan, const double* uv_f64, const double* freqs, long long n_vis, int n_chan,
+                           long long* out_count, void* stream);
+
+/* f3 - accumulate-into (the gridded data are "readily aggregated in frequency and time"; SURVEY.md section
+ * 8(f)-3).  When enabled, mwa_grid_visibilities ADDS the gridded samples to what grid_out holds instead of overwriting it
+ * (R10 then does not apply: cells no tap reaches are left as they are), so successive time steps or row batches can be
+ * gridded onto the same grids.  K6 writes with reduce-add tensor-map stores and skips its zero-fill, K3c reads, adds and
+ * writes its own cells, K0 / K3b skip their memset; the designs SMEM and CHAN return MWA_GRID_ERR_INVALID.  One fp32
+ * rounding is added per call and cell.  Takes effect at the next call. */
+int mwa_grid_plan_set_accumulate(mwa_grid_plan* plan, int enabled);
+
 /* Select the gridding design (MWA_GRID_DESIGN_*).  Takes effect at the next call. */
 int mwa_grid_plan_set_design(mwa_grid_plan* plan, int design);
 

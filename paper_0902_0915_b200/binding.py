@@ -32,6 +32,10 @@ _lib.mwa_grid_visibilities_host.argtypes = [_P, _P, _P, _P, _P, _LL, _I, _P, _P]
 _lib.mwa_grid_visibilities_host.restype = _I
 _lib.mwa_grid_compute_indices.argtypes = [_P, _P, _P, _LL, _I, _P, _P]
 _lib.mwa_grid_compute_indices.restype = _I
+_lib.mwa_grid_count_dropped.argtypes = [_P, _P, _P, _LL, _I, _P, _P]
+_lib.mwa_grid_count_dropped.restype = _I
+_lib.mwa_grid_plan_set_accumulate.argtypes = [_P, _I]
+_lib.mwa_grid_plan_set_accumulate.restype = _I
 _lib.mwa_grid_plan_set_design.argtypes = [_P, _I]
 _lib.mwa_grid_plan_set_design.restype = _I
 _lib.mwa_grid_plan_set_profiling.argtypes = [_P, _I]
@@ -62,7 +66,7 @@ _lib.mwa_grid_last_error.restype = ctypes.c_char_p
 EXPORTS = ["mwa_grid_plan_create", "mwa_grid_plan_destroy", "mwa_grid_visibilities", "mwa_grid_visibilities_host",
            "mwa_grid_compute_indices", "mwa_grid_plan_set_design", "mwa_grid_plan_set_profiling",
            "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_plan_last_design", "mwa_grid_plan_last_stats", "mwa_grid_plan_set_list_pool", "mwa_grid_probe_fp32", "mwa_grid_last_error",
-           "mwa_image_from_grid", "mwa_image_correction", "mwa_image_stokes", "mwa_grid_probe_smem_atomics"]
+           "mwa_image_from_grid", "mwa_image_correction", "mwa_image_stokes", "mwa_grid_probe_smem_atomics", "mwa_grid_count_dropped", "mwa_grid_plan_set_accumulate"]
 
 
 class MwaGridError(RuntimeError):
@@ -143,6 +147,20 @@ def mwa_grid_compute_indices(plan, uv_f64, freqs, n_vis, n_chan, out_idx, stream
     _check(_lib.mwa_grid_compute_indices(plan, _ptr(uv_f64, torch.float64, "cuda", "uv_f64"),
                                          _ptr(freqs, torch.float64, "cuda", "freqs"), int(n_vis), int(n_chan),
                                          _ptr(out_idx, torch.int32, "cuda", "out_idx"), _stream_ptr(stream)))
+
+
+def mwa_grid_count_dropped(plan, uv_f64, freqs, n_vis, n_chan, stream=None) -> int:
+    """Number of (row, channel) samples the gridder drops (R11) for these coordinates.  Synchronises."""
+    out = ctypes.c_longlong(0)
+    _check(_lib.mwa_grid_count_dropped(plan, _ptr(uv_f64, torch.float64, "cuda", "uv_f64"),
+                                       _ptr(freqs, torch.float64, "cuda", "freqs"), int(n_vis), int(n_chan),
+                                       ctypes.cast(ctypes.pointer(out), ctypes.c_void_p), _stream_ptr(stream)))
+    return int(out.value)
+
+
+def mwa_grid_plan_set_accumulate(plan, enabled: bool) -> None:
+    """f3: grid_out += gridded samples instead of grid_out = (cells nothing reaches stay as they are)."""
+    _check(_lib.mwa_grid_plan_set_accumulate(plan, 1 if enabled else 0))
 
 
 def mwa_grid_plan_set_design(plan, design) -> None:

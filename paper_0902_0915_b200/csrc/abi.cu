@@ -158,10 +158,16 @@ static int grid_device(Plan* p, const double* uv, const double* freqs, const flo
         if (!launch_binning(p, uv, n_vis, n_chan, st)) return MWA_GRID_ERR_CUDA;
     if (prof) cudaEventRecord(p->ev[1], st);
     bool ok = false;
-    if (n_vis == 0) {
+    if (n_vis == 0 && p->accumulate) {
+        ok = true;                                // nothing to add
+    } else if (n_vis == 0) {
         ok = cuda_ok(cudaMemsetAsync(grid, 0, (size_t)n_chan * 4 * p->geom.N * p->geom.N * 8, st), "memset grid");
         p->last_launches += 1;
     } else {
+        if (p->accumulate && (design == MWA_GRID_DESIGN_SMEM || design == MWA_GRID_DESIGN_CHAN)) {
+            set_error("accumulate-into is implemented by the designs AUTO, GATHER, CHANWS, ATOMIC and ROMEIN only");
+            return MWA_GRID_ERR_INVALID;
+        }
         switch (design) {
             case MWA_GRID_DESIGN_ATOMIC: ok = launch_atomic(p, uv, vis, weights, n_vis, n_chan, grid, st); break;
             case MWA_GRID_DESIGN_SMEM: ok = launch_smem(p, vis, weights, n_vis, n_chan, grid, st); break;
@@ -183,7 +189,7 @@ static int grid_device(Plan* p, const double* uv, const double* freqs, const flo
                 }
                 p->last_chanws = chanws_supported(p, n_chan);
                 if (p->last_chanws) ok = launch_chanws(p, vis, weights, n_vis, n_chan, grid, p->ws.d_dispatch, st);
-                else if (chan_supported(p, n_chan)) ok = launch_chan(p, vis, weights, n_vis, n_chan, grid, p->ws.d_dispatch, st);
+                else if (chan_supported(p, n_chan) && !p->accumulate) ok = launch_chan(p, vis, weights, n_vis, n_chan, grid, p->ws.d_dispatch, st);
                 ok = ok && launch_gather(p, vis, weights, n_vis, n_chan, grid, p->ws.d_dispatch, st);
                 break;
             default: set_error("unknown design"); return MWA_GRID_ERR_INVALID;
@@ -314,6 +320,12 @@ int mwa_grid_plan_set_design(mwa_grid_plan* plan, int design) {
     return MWA_GRID_OK;
 }
 
+int mwa_grid_plan_set_accumulate(mwa_grid_plan* plan, int enabled) {
+    if (!plan) { set_error("plan is NULL"); return MWA_GRID_ERR_INVALID; }
+    reinterpret_cast<Plan*>(plan)->accumulate = enabled != 0;
+    return MWA_GRID_OK;
+}
+
 int mwa_grid_plan_set_profiling(mwa_grid_plan* plan, int enabled) {
     if (!plan) { set_error("plan is NULL"); return MWA_GRID_ERR_INVALID; }
     Plan* p = reinterpret_cast<Plan*>(plan);
@@ -395,6 +407,30 @@ int mwa_grid_compute_indices(mwa_grid_plan* plan, const double* uv_f64, const do
     p->last_launches = 0;
     if (!launch_scale(p, freqs, n_chan, st)) return MWA_GRID_ERR_CUDA;
     if (!launch_indices(p, uv_f64, n_vis, n_chan, out_idx, st)) return MWA_GRID_ERR_CUDA;
+    return MWA_GRID_OK;
+}
+
+int mwa_grid_count_dropped(mwa_grid_plan* plan, const double* uv_f64, const double* freqs, long long n_vis, int n_chan,
+                           long long* out_count, void* stream) {
+    g_last_error.clear();
+    Plan* p = reinterpret_cast<Plan*>(plan);
+    int rc = check_common(p, uv_f64, freqs, n_vis, n_chan);
+    if (rc != MWA_GRID_OK) return rc;
+    if (!out_count) { set_error("out_count is NULL"); return MWA_GRID_ERR_INVALID; }
+    *out_count = 0;
+    if (n_vis == 0 || n_chan == 0) return MWA_GRID_OK;
+    rc = ensure_workspace(p, n_vis, n_chan);
+    if (rc != MWA_GRID_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    p->last_launches = 0;
+    unsigned long long* d_count = reinterpret_cast<unsigned long long*>(p->ws.d_misc + 12);   // the call's scratch counter
+    if (!cuda_ok(cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), st), "memset counter")) return MWA_GRID_ERR_CUDA;
+    if (!launch_scale(p, freqs, n_chan, st)) return MWA_GRID_ERR_CUDA;
+    if (!launch_count_dropped(p, uv_f64, n_vis, n_chan, d_count, st)) return MWA_GRID_ERR_CUDA;
+    unsigned long long h = 0;
+    if (!cuda_ok(cudaMemcpyAsync(&h, d_count, sizeof(h), cudaMemcpyDeviceToHost, st), "read counter") ||
+        !cuda_ok(cudaStreamSynchronize(st), "count_dropped_kernel")) return MWA_GRID_ERR_CUDA;
+    *out_count = (long long)h;
     return MWA_GRID_OK;
 }
 

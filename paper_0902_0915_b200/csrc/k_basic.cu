@@ -90,6 +90,32 @@ __global__ void indices_kernel(GridGeom g, const double2* __restrict__ uv, const
     }
 }
 
+// ---------------------------------------------------------------- dropped-sample counter
+__global__ void count_dropped_kernel(GridGeom g, const double2* __restrict__ uv, const double* __restrict__ scale, long long n_vis,
+                                     int n_chan, unsigned long long* __restrict__ count) {
+    const long long total = n_vis * (long long)n_chan;
+    unsigned long long mine = 0;
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < total; k += (long long)gridDim.x * blockDim.x) {
+        const long long n = k / n_chan;
+        const int c = (int)(k - n * n_chan);
+        const double2 p = uv[n];
+        SampleIndex s;
+        mine += sample_index(p.x, p.y, scale[c], g, s) ? 0 : 1;
+    }
+    mine = __reduce_add_sync(0xffffffffu, (unsigned)mine);               // < 2^32 per warp pass: a thread sees < 2^27 samples
+    if ((threadIdx.x & 31) == 0 && mine) atomicAdd(count, mine);
+}
+
+bool launch_count_dropped(Plan* p, const double* uv, long long n_vis, int n_chan, unsigned long long* d_count, cudaStream_t st) {
+    const long long total = n_vis * (long long)n_chan;
+    long long blocks = (total + 255) / 256;
+    if (blocks > (long long)p->sm_count * 64) blocks = (long long)p->sm_count * 64;
+    if (blocks < 1) blocks = 1;
+    count_dropped_kernel<<<(unsigned)blocks, 256, 0, st>>>(p->geom, (const double2*)uv, p->ws.d_scale, n_vis, n_chan, d_count);
+    p->last_launches += 1;
+    return cuda_ok(cudaGetLastError(), "count_dropped_kernel");
+}
+
 bool launch_indices(Plan* p, const double* uv, long long n_vis, int n_chan, int* out_idx, cudaStream_t st) {
     const long long total = n_vis * (long long)n_chan;
     if (total == 0) return true;
@@ -138,8 +164,10 @@ __global__ void atomic_grid_kernel(GridGeom g, const double2* __restrict__ uv, c
 bool launch_atomic(Plan* p, const double* uv, const float* vis, const float* w, long long n_vis, int n_chan,
                    float* grid, cudaStream_t st) {
     const size_t bytes = (size_t)n_chan * 4 * p->geom.N * p->geom.N * 8;
-    if (!cuda_ok(cudaMemsetAsync(grid, 0, bytes, st), "memset grid")) return false;
-    p->last_launches += 1;
+    if (!p->accumulate) {                                       // accumulate-into: the atomics add onto what is there
+        if (!cuda_ok(cudaMemsetAsync(grid, 0, bytes, st), "memset grid")) return false;
+        p->last_launches += 1;
+    }
     const long long total = n_vis * (long long)n_chan * p->geom.W;
     if (total == 0) return true;
     long long blocks = (total + 255) / 256;

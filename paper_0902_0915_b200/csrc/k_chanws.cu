@@ -97,6 +97,7 @@ struct K6Params {
     const float* weights;        // [n_vis][n_chan] or null
     const float* table;          // [(O+1)][W]
     float* grid;                 // [n_chan][4][N][N][2] (zero-fill of untouched items; everything else goes through the tensor map)
+    int accumulate;              // 1: grid += (f3 accumulate-into: reduce-add stores, no zero-fill), 0: grid = (R10)
     int n_vis, n_chan, n_groups, nb;
     int ntx, nty;                // tiles per row / column
     int rlu, rlv, n_tu, n_tv;    // padded row lengths and sizes (floats) of the shifted table copies
@@ -221,6 +222,11 @@ __device__ __forceinline__ void tma_store4(const CUtensorMap* m, unsigned src, i
     asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.bulk_group.L2::cache_hint [%0, {%1, %2, %3, %4}], [%5], %6;"
                  ::"l"(m), "r"(d0), "r"(d1), "r"(d2), "r"(d3), "r"(src), "l"(policy) : "memory");
 #endif
+}
+// the same box as a reduction: grid += stage (fp32 add in L2), through a tensor map whose elements are floats
+__device__ __forceinline__ void tma_reduce_add4(const CUtensorMap* m, unsigned src, int d0, int d1, int d2, int d3) {
+    asm volatile("cp.reduce.async.bulk.tensor.4d.global.shared::cta.add.tile.bulk_group [%0, {%1, %2, %3, %4}], [%5];"
+                 ::"l"(m), "r"(d0), "r"(d1), "r"(d2), "r"(d3), "r"(src) : "memory");
 }
 __device__ __forceinline__ void k6_unpack2(u64 v, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
 __device__ __forceinline__ u64 k6_pack2(float a, float b) {
@@ -500,7 +506,7 @@ chan_order_kernel(const int* __restrict__ list_cnt, const unsigned* __restrict__
 template <bool HAS_W>
 __global__ void __launch_bounds__(k6Threads, 1)
 chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtensorMap map_out,
-              const __grid_constant__ CUtensorMap map_zero) {
+              const __grid_constant__ CUtensorMap map_zero, const __grid_constant__ CUtensorMap map_acc) {
     if (P.dispatch != nullptr && *P.dispatch != P.dispatch_want) return;
     extern __shared__ __align__(1024) unsigned char smem_dyn[];
     unsigned char* base = smem_dyn;
@@ -1052,7 +1058,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                     const int tx = z_cur % P.ntx, ty = (z_cur / P.ntx) % P.nty, grp = z_cur / (P.ntx * P.nty);
                     zX0 = tx * k6TileX; zY0 = ty * k6TileY; zc0 = grp * 32;
                 };
-                z_advance();
+                if (!P.accumulate) z_advance();                          // accumulate-into leaves the cells nothing reaches alone
                 unsigned remaining = 0xfu;                                   // block rows of consumer item ci still to store
                 long long t_so_rel = 0, t_so_idle = 0, t_so_zero = 0, t_so_all = 0;
                 (void)t_so_rel; (void)t_so_idle; (void)t_so_zero; (void)t_so_all;
@@ -1074,7 +1080,10 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                                 const unsigned par = (unsigned)((2 * ci + (r >> 1)) & 1);
                                 if (((remaining >> r) & 1u) && (r < 2 || !((remaining >> (r - 2)) & 1u)) && mbar_try(smem_u32(&S.wo_full[r & 1]), par)) {
 #ifndef K6_ABLATE_STORE
-                                    if (Y0 + 2 * r < N) tma_store4(&map_out, wo0 + 32768u * (r & 1), X0, c0, Y0 + 2 * r, 0, pol_first);
+                                    if (Y0 + 2 * r < N) {
+                                        if (P.accumulate) tma_reduce_add4(&map_acc, wo0 + 32768u * (r & 1), 2 * X0, c0, Y0 + 2 * r, 0);
+                                        else tma_store4(&map_out, wo0 + 32768u * (r & 1), X0, c0, Y0 + 2 * r, 0, pol_first);
+                                    }
 #endif
                                     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
                                     K6_TIC(s0);
@@ -1169,14 +1178,16 @@ static EncodeTiledFn encode_tiled_fn() {
 }
 
 // grid_out [n_chan][4][N][N] complex64 seen as a 4-D tensor of 8-byte elements with dimension order (u, channel, v, pol)
-static bool make_grid_map(CUtensorMap* map, float* grid, int N, int n_chan, int box_v, int box_pol, bool swizzle) {
+static bool make_grid_map(CUtensorMap* map, float* grid, int N, int n_chan, int box_v, int box_pol, bool swizzle,
+                          bool as_floats = false) {
     EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) { set_error("cuTensorMapEncodeTiled is not available from the driver"); return false; }
-    const cuuint64_t dims[4] = {(cuuint64_t)N, (cuuint64_t)n_chan, (cuuint64_t)N, 4};
+    // as_floats: the same memory as 4-byte elements (u is 2 N floats long, the box 32 floats wide) - what a reduce-add needs
+    const cuuint64_t dims[4] = {(cuuint64_t)(as_floats ? 2 * N : N), (cuuint64_t)n_chan, (cuuint64_t)N, 4};
     const cuuint64_t strides[3] = {(cuuint64_t)4 * N * N * 8, (cuuint64_t)N * 8, (cuuint64_t)N * N * 8};
-    const cuuint32_t box[4] = {16, 32, (cuuint32_t)box_v, (cuuint32_t)box_pol};
+    const cuuint32_t box[4] = {as_floats ? 32u : 16u, 32, (cuuint32_t)box_v, (cuuint32_t)box_pol};
     const cuuint32_t es[4] = {1, 1, 1, 1};
-    const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT64, 4, grid, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+    const CUresult r = enc(map, as_floats ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_UINT64, 4, grid, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                            swizzle ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { set_error("cuTensorMapEncodeTiled failed (CUresult " + std::to_string((int)r) + ")"); return false; }
@@ -1219,9 +1230,11 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
     P.nty = (p->geom.N + k6TileY - 1) / k6TileY;
     P.n_items = (long long)P.ntx * P.nty * P.n_groups;
     if (P.n_items >= 0x7fffffffLL) { set_error("design CHANWS: too many work items"); return false; }
-    CUtensorMap map_out, map_zero;
+    CUtensorMap map_out, map_zero, map_acc;
+    P.accumulate = p->accumulate ? 1 : 0;
     if (!make_grid_map(&map_out, grid, p->geom.N, n_chan, 2, 4, true)) return false;
     if (!make_grid_map(&map_zero, grid, p->geom.N, n_chan, k6ZeroV, 1, false)) return false;
+    if (!make_grid_map(&map_acc, grid, p->geom.N, n_chan, 2, 4, true, true)) return false;
 
     long long iblocks = (n_vis + 7) / 8;                                      // one warp per sorted row at a time
     if (iblocks > (long long)p->sm_count * 8) iblocks = (long long)p->sm_count * 8;
@@ -1244,7 +1257,7 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
         return false;
     long long blocks = p->sm_count;
     if (blocks > P.n_items) blocks = P.n_items;
-    kern<<<(unsigned)blocks, k6Threads, smem, st>>>(P, map_out, map_zero);
+    kern<<<(unsigned)blocks, k6Threads, smem, st>>>(P, map_out, map_zero, map_acc);
     p->last_launches += 4;
     return cuda_ok(cudaGetLastError(), "chanws_kernel");
 }

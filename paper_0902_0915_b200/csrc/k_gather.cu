@@ -43,6 +43,7 @@ struct GatherParams {
     int n_chan, nb, nt;
     int rlu, rlv;               // padded row lengths of the shifted table copies
     long long n_items;
+    int accumulate;             // 1: grid += (f3 accumulate-into), 0: grid = (R10)
     int chunk;                  // consecutive work items per claim (1..8; amortises the round trip of the work counter)
 };
 
@@ -382,11 +383,19 @@ gather_kernel(const GatherParams P) {
                         if (x + 1 < g.N) {
                             unpack2(acc[i][0][p], a0, a1);
                             unpack2(acc[i][1][p], a2, a3);
+                            if (P.accumulate) {                             // the warp owns these cells: a plain read-modify-write
+                                const float4 o = *reinterpret_cast<const float4*>(dst);
+                                a0 += o.x; a1 += o.y; a2 += o.z; a3 += o.w;
+                            }
                             st_stream_v4(dst, a0, a1, a2, a3);
                         }
                         if (x + 3 < g.N) {
                             unpack2(acc[i][2][p], a0, a1);
                             unpack2(acc[i][3][p], a2, a3);
+                            if (P.accumulate) {
+                                const float4 o = *reinterpret_cast<const float4*>(dst + 4);
+                                a0 += o.x; a1 += o.y; a2 += o.z; a3 += o.w;
+                            }
                             st_stream_v4(dst + 4, a0, a1, a2, a3);
                         }
                     }
@@ -415,6 +424,7 @@ bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, i
     P.table = p->d_table;
     P.grid = grid;
     P.n_chan = n_chan;
+    P.accumulate = p->accumulate ? 1 : 0;
     P.nb = (p->geom.N + kBucketCells - 1) / kBucketCells;
     P.nt = (p->geom.N + kTile - 1) / kTile;
     P.rlu = (p->geom.W + 6 + 3) & ~3;

@@ -107,8 +107,10 @@ __global__ void romein_kernel(const RomeinParams P) {
 bool launch_romein(Plan* p, const double* uv, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                    const int* perm, cudaStream_t st) {
     const size_t bytes = (size_t)n_chan * 4 * p->geom.N * p->geom.N * 8;
-    if (!cuda_ok(cudaMemsetAsync(grid, 0, bytes, st), "memset grid")) return false;
-    p->last_launches += 1;
+    if (!p->accumulate) {                                       // accumulate-into: the reductions add onto what is there
+        if (!cuda_ok(cudaMemsetAsync(grid, 0, bytes, st), "memset grid")) return false;
+        p->last_launches += 1;
+    }
     RomeinParams P;
     P.g = p->geom;
     P.scale = p->ws.d_scale;

@@ -73,6 +73,7 @@ struct Plan {
     double* h_corr = nullptr;        // [N] c^(p' - N/2), host copy (fp64)
     int fft_handle[2] = {0, 0};      // cached cuFFT plans ...
     int fft_batch[2] = {0, 0};       // ... and the batch sizes they were made for (0 = none)
+    bool accumulate = false;         // f3: grid_out += instead of = (mwa_grid_plan_set_accumulate)
     long long pool_limit = 0;        // diagnostics: cap on K6's hit-list pool in entries (0 = default sizing)
     bool last_chanws = false;        // AUTO: the channel-SIMD kernel enqueued by the last call was K6 (else K5)
 };
@@ -82,6 +83,7 @@ bool cuda_ok(cudaError_t e, const char* what);
 
 // launchers (each returns false after set_error on failure and adds its launches to plan->last_launches)
 bool launch_scale(Plan* p, const double* freqs, int n_chan, cudaStream_t st);
+bool launch_count_dropped(Plan* p, const double* uv, long long n_vis, int n_chan, unsigned long long* d_count, cudaStream_t st);
 bool launch_indices(Plan* p, const double* uv, long long n_vis, int n_chan, int* out_idx, cudaStream_t st);
 bool launch_atomic(Plan* p, const double* uv, const float* vis, const float* w, long long n_vis, int n_chan,
                    float* grid, cudaStream_t st);

@@ -73,6 +73,9 @@ def test_indices_lattice_halfway_edges_and_nonfinite(lib):
         got = p.indices(torch.from_numpy(uv).cuda(), torch.from_numpy(fr).cuda()).cpu().numpy()
     assert np.array_equal(got, want)
     assert (want[:, 0, 0] == -1).any() and (want[:, 0, 0] >= 0).any()
+    with lib.Plan(N, 1.0, W, O, make_kernel_table(W, O)) as p:                # the dropped-sample counter agrees with the oracle
+        n_drop = lib.mwa_grid_count_dropped(p.handle, torch.from_numpy(uv).cuda(), torch.from_numpy(fr).cuda(), uv.shape[0], 3)
+    assert n_drop == int((want[:, :, 0] == -1).sum()) and n_drop > 0
 
 
 # ---------------------------------------------------------------------------- values
@@ -497,3 +500,35 @@ def test_stokes_conversion_matches_the_oracle(lib, N, n_chan):
         inplace = d_img.clone()
         p.stokes(inplace, d_M, out=inplace)
         assert torch.equal(inplace.view(torch.float32), out.view(torch.float32))
+
+
+# ---------------------------------------------------------------------------- f3: accumulate-into
+@pytest.mark.parametrize("design", ["auto", "gather", "chanws", "atomic", "romein"])
+@pytest.mark.parametrize("fine", [True, False])
+def test_accumulate_into_adds_row_batches_onto_one_grid(lib, design, fine):
+    """Two row batches gridded one after the other with accumulate-into equal the oracle's grid of all rows (the
+    aggregation in time of PAPER.md:23), and what the grid held before is kept, not overwritten."""
+    if fine:
+        g = generate(_fine(dict(n_ant=64, core_ant=32, n_chan=40, grid_n=250)))
+    else:
+        if design == "chanws":
+            pytest.skip("coarse channels: covered by the other designs")
+        g = generate(scaled(CONFIGS["C2"], n_ant=48, n_chan=5, grid_n=256))
+    G, A, _ = _oracle(g)
+    _to_dev(g)
+    half = g.cfg.n_vis // 2
+    rs = np.random.RandomState(2)
+    prev = (rs.standard_normal(G.shape) + 1j * rs.standard_normal(G.shape)).astype(np.complex64)
+    with _plan(lib, g, design) as p:
+        lib.mwa_grid_plan_set_accumulate(p.handle, True)
+        out = torch.from_numpy(prev).cuda()
+        for r0, r1 in ((0, half), (half, g.cfg.n_vis)):
+            p.grid(g.uv[r0:r1].contiguous(), g.freqs, g.vis[r0:r1].contiguous(), g.weights[r0:r1].contiguous(), out=out)
+        got = out.cpu().numpy()
+        lib.mwa_grid_plan_set_accumulate(p.handle, False)
+        again = p.grid(g.uv, g.freqs, g.vis, g.weights, out=out).cpu().numpy()    # back to overwrite (R10)
+    want = prev.astype(np.complex128) + G
+    # the fp32 tolerance of the gridded part, plus one rounding of the running sum per call
+    bound = 1e-5 * A + 1e-7 + 3 * 2.0 ** -24 * (np.abs(prev) + np.abs(want))
+    assert np.all(np.abs(got.astype(np.complex128) - want) <= bound), float(np.max(np.abs(got - want) / bound))
+    assert_parity(again, G, A, f"{design} overwrite after accumulate")
