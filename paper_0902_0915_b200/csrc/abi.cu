@@ -5,6 +5,7 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "../../include/mwa_grid.h"
 #include "plan.h"
@@ -121,14 +122,16 @@ static int ensure_workspace(Plan* p, long long n_vis, int n_chan) {
 
 static bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) % a) == 0; }
 
-static int check_common(Plan* p, const double* uv, const double* freqs, long long n_vis, int n_chan) {
+static int check_common(Plan* p, const double* uv, const double* freqs, long long n_vis, int n_chan, bool device_pointers = true) {
     if (!p) { set_error("plan is NULL"); return MWA_GRID_ERR_INVALID; }
     if (n_vis < 0 || n_chan < 0) { set_error("n_vis and n_chan must be >= 0"); return MWA_GRID_ERR_INVALID; }
     if (n_vis > 0x7fffffffLL) { set_error("n_vis must fit in 31 bits"); return MWA_GRID_ERR_INVALID; }
     if (n_chan > 0 && !freqs) { set_error("freqs is NULL"); return MWA_GRID_ERR_INVALID; }
     if (n_vis > 0 && n_chan > 0 && !uv) { set_error("uv_f64 is NULL"); return MWA_GRID_ERR_INVALID; }
-    if (!aligned(uv, 16)) { set_error("uv_f64 must be 16-byte aligned"); return MWA_GRID_ERR_INVALID; }
-    if (!aligned(freqs, 8)) { set_error("freqs must be 8-byte aligned"); return MWA_GRID_ERR_INVALID; }
+    if (device_pointers) {                        // the kernels read uv as double2; host buffers are only copied
+        if (!aligned(uv, 16)) { set_error("uv_f64 must be 16-byte aligned"); return MWA_GRID_ERR_INVALID; }
+        if (!aligned(freqs, 8)) { set_error("freqs must be 8-byte aligned"); return MWA_GRID_ERR_INVALID; }
+    }
     return MWA_GRID_OK;
 }
 
@@ -255,6 +258,8 @@ void mwa_grid_plan_destroy(mwa_grid_plan* plan) {
     for (void* q : ptrs)
         if (q) cudaFree(q);
     image_release(p);
+    for (auto& cs : p->copy_stream)
+        if (cs) cudaStreamDestroy(cs);
     for (auto& e : p->ev)
         if (e) cudaEventDestroy(e);
     delete[] p->h_table;
@@ -451,18 +456,28 @@ int mwa_grid_visibilities_host(mwa_grid_plan* plan, const double* uv_f64, const 
                                const float* weights, long long n_vis, int n_chan, float* grid_out, void* stream) {
     g_last_error.clear();
     Plan* p = reinterpret_cast<Plan*>(plan);
-    int rc = check_common(p, uv_f64, freqs, n_vis, n_chan);
+    int rc = check_common(p, uv_f64, freqs, n_vis, n_chan, false);
     if (rc != MWA_GRID_OK) return rc;
     if (n_chan == 0) { p->last_launches = 0; return MWA_GRID_OK; }
     if (!grid_out) { set_error("grid_out is NULL"); return MWA_GRID_ERR_INVALID; }
     if (n_vis > 0 && !vis_c64) { set_error("vis_c64 is NULL"); return MWA_GRID_ERR_INVALID; }
+    if (p->accumulate) { set_error("accumulate-into works on device grids only (mwa_grid_visibilities)"); return MWA_GRID_ERR_INVALID; }
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     auto up = [](size_t b) { return (b + 255) & ~size_t(255); };
-    const size_t samples = (size_t)n_vis * n_chan;
-    const size_t b_uv = up((size_t)n_vis * 16), b_fr = up((size_t)n_chan * 8), b_vis = up(samples * 32);
-    const size_t b_w = weights ? up(samples * 4) : 0;
-    const size_t b_grid = (size_t)n_chan * 4 * p->geom.N * p->geom.N * 8;
-    const size_t total = b_uv + b_fr + b_vis + b_w + up(b_grid);
+    // Channels own their grids, so the call is pipelined over channel chunks (multiples of 32 channels, ~8 per call):
+    // the upload of chunk k + 1 (copy stream) and the download of chunk k - 1's grids (second copy stream) run under the
+    // gridding of chunk k on the caller's stream.  PCIe carries both directions at once; what stays exposed is the first
+    // upload and the last download.
+    const int n_chunks_want = 8;
+    int cc = ((n_chan + n_chunks_want - 1) / n_chunks_want + 31) / 32 * 32;
+    if (cc > n_chan) cc = n_chan;
+    const int n_chunks = (n_chan + cc - 1) / cc;
+    const size_t plane_bytes = (size_t)p->geom.N * p->geom.N * 8;
+    const size_t b_uv = up((size_t)n_vis * 16), b_fr = up((size_t)n_chan * 8);
+    const size_t b_vis = up((size_t)n_vis * cc * 32), b_w = weights ? up((size_t)n_vis * cc * 4) : 0;
+    const size_t b_grid = (size_t)n_chan * 4 * plane_bytes;
+    const int n_in = n_chunks > 1 ? 2 : 1;                                   // input chunk buffers (double-buffered)
+    const size_t total = b_uv + b_fr + n_in * (b_vis + b_w) + up(b_grid);
     if (total > p->ws.cap_stage) {
         if (p->ws.d_stage) cudaFree(p->ws.d_stage);
         p->ws.d_stage = nullptr;
@@ -471,23 +486,68 @@ int mwa_grid_visibilities_host(mwa_grid_plan* plan, const double* uv_f64, const 
         if (e != cudaSuccess) { cudaGetLastError(); set_error("staging allocation failed"); return MWA_GRID_ERR_NOMEM; }
         p->ws.cap_stage = total;
     }
+    if (n_chunks > 1 && !p->copy_stream[0]) {
+        for (int k = 0; k < 2; ++k)
+            if (!cuda_ok(cudaStreamCreateWithFlags(&p->copy_stream[k], cudaStreamNonBlocking), "cudaStreamCreate")) return MWA_GRID_ERR_CUDA;
+    }
     char* base = (char*)p->ws.d_stage;
     double* d_uv = (double*)base;
     double* d_fr = (double*)(base + b_uv);
-    float* d_vis = (float*)(base + b_uv + b_fr);
-    float* d_w = weights ? (float*)(base + b_uv + b_fr + b_vis) : nullptr;
-    float* d_grid = (float*)(base + b_uv + b_fr + b_vis + b_w);
-    if (n_vis > 0) {
-        if (!cuda_ok(cudaMemcpyAsync(d_uv, uv_f64, (size_t)n_vis * 16, cudaMemcpyHostToDevice, st), "H2D uv")) return MWA_GRID_ERR_CUDA;
-        if (!cuda_ok(cudaMemcpyAsync(d_vis, vis_c64, samples * 32, cudaMemcpyHostToDevice, st), "H2D vis")) return MWA_GRID_ERR_CUDA;
-        if (weights && !cuda_ok(cudaMemcpyAsync(d_w, weights, samples * 4, cudaMemcpyHostToDevice, st), "H2D weights")) return MWA_GRID_ERR_CUDA;
-    }
+    char* d_in = base + b_uv + b_fr;
+    float* d_grid = (float*)(d_in + n_in * (b_vis + b_w));
+    if (n_vis > 0 && !cuda_ok(cudaMemcpyAsync(d_uv, uv_f64, (size_t)n_vis * 16, cudaMemcpyHostToDevice, st), "H2D uv")) return MWA_GRID_ERR_CUDA;
     if (!cuda_ok(cudaMemcpyAsync(d_fr, freqs, (size_t)n_chan * 8, cudaMemcpyHostToDevice, st), "H2D freqs")) return MWA_GRID_ERR_CUDA;
-    rc = grid_device(p, d_uv, d_fr, d_vis, d_w, n_vis, n_chan, d_grid, st);
-    if (rc != MWA_GRID_OK) return rc;
-    if (!cuda_ok(cudaMemcpyAsync(grid_out, d_grid, b_grid, cudaMemcpyDeviceToHost, st), "D2H grid")) return MWA_GRID_ERR_CUDA;
-    if (!cuda_ok(cudaStreamSynchronize(st), "stream synchronize")) return MWA_GRID_ERR_CUDA;
-    return MWA_GRID_OK;
+    cudaStream_t s_up = n_chunks > 1 ? p->copy_stream[0] : st, s_down = n_chunks > 1 ? p->copy_stream[1] : st;
+    std::vector<cudaEvent_t> ev_up(n_chunks, nullptr), ev_done(n_chunks, nullptr);
+    bool ok = true;
+    int launches = 0;
+    auto fail = [&](int code) { rc = code; ok = false; };
+    if (n_chunks > 1) {
+        for (int k = 0; k < n_chunks && ok; ++k)
+            if (cudaEventCreateWithFlags(&ev_up[k], cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&ev_done[k], cudaEventDisableTiming) != cudaSuccess) { set_error("cudaEventCreate failed"); fail(MWA_GRID_ERR_CUDA); }
+    }
+    for (int k = 0; k < n_chunks && ok; ++k) {
+        const int c0 = k * cc, nc = (c0 + cc <= n_chan) ? cc : n_chan - c0;
+        char* in = d_in + (size_t)(k % n_in) * (b_vis + b_w);
+        float* d_vis = (float*)in;
+        float* d_w = weights ? (float*)(in + b_vis) : nullptr;
+        if (n_chunks > 1 && k >= 2 && cudaStreamWaitEvent(s_up, ev_done[k - 2], 0) != cudaSuccess) { set_error("cudaStreamWaitEvent failed"); fail(MWA_GRID_ERR_CUDA); break; }
+        if (n_vis > 0) {
+            // the channel slice of the [row][chan] host arrays: a strided (2-D) copy into a contiguous chunk
+            if (!cuda_ok(cudaMemcpy2DAsync(d_vis, (size_t)nc * 32, (const char*)vis_c64 + (size_t)c0 * 32, (size_t)n_chan * 32, (size_t)nc * 32,
+                                           (size_t)n_vis, cudaMemcpyHostToDevice, s_up), "H2D vis")) { fail(MWA_GRID_ERR_CUDA); break; }
+            if (weights && !cuda_ok(cudaMemcpy2DAsync(d_w, (size_t)nc * 4, (const char*)weights + (size_t)c0 * 4, (size_t)n_chan * 4, (size_t)nc * 4,
+                                                      (size_t)n_vis, cudaMemcpyHostToDevice, s_up), "H2D weights")) { fail(MWA_GRID_ERR_CUDA); break; }
+        }
+        float* g = d_grid + (size_t)c0 * 4 * (plane_bytes / 4);
+        if (n_chunks > 1) {
+            cudaEventRecord(ev_up[k], s_up);
+            cudaStreamWaitEvent(st, ev_up[k], 0);
+        }
+        const int r = grid_device(p, d_uv, d_fr + c0, d_vis, d_w, n_vis, nc, g, st);
+        if (r != MWA_GRID_OK) { fail(r); break; }
+        launches += p->last_launches;
+        if (n_chunks > 1) {
+            cudaEventRecord(ev_done[k], st);
+            cudaStreamWaitEvent(s_down, ev_done[k], 0);
+        }
+        if (!cuda_ok(cudaMemcpyAsync((char*)grid_out + (size_t)c0 * 4 * plane_bytes, g, (size_t)nc * 4 * plane_bytes, cudaMemcpyDeviceToHost, s_down),
+                     "D2H grid")) { fail(MWA_GRID_ERR_CUDA); break; }
+    }
+    // synchronous by contract: everything enqueued above has finished when the call returns (also after a failure)
+    bool sync_ok = cuda_ok(cudaStreamSynchronize(st), "stream synchronize");
+    if (n_chunks > 1) {
+        sync_ok = cuda_ok(cudaStreamSynchronize(s_up), "copy stream synchronize") && sync_ok;
+        sync_ok = cuda_ok(cudaStreamSynchronize(s_down), "copy stream synchronize") && sync_ok;
+        for (int k = 0; k < n_chunks; ++k) {
+            if (ev_up[k]) cudaEventDestroy(ev_up[k]);
+            if (ev_done[k]) cudaEventDestroy(ev_done[k]);
+        }
+    }
+    p->last_launches = launches;
+    if (!ok) return rc;
+    return sync_ok ? MWA_GRID_OK : MWA_GRID_ERR_CUDA;
 }
 
 }  // extern "C"

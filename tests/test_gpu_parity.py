@@ -348,6 +348,23 @@ def test_host_entry_point_matches_device_call(lib):
         assert lib.mwa_grid_plan_last_launches(p.handle) > 0
 
 
+def test_host_entry_point_pipelined_over_channel_chunks(lib):
+    # 100 fine channels -> 4 chunks (32, 32, 32, 4): upload, gridding and download of different chunks overlap
+    g = generate(_fine(dict(n_ant=48, core_ant=24, n_chan=100, grid_n=128)))
+    G, A, _ = _oracle(g)
+    cfg = g.cfg
+    with _plan(lib, g) as p:
+        out = torch.full((cfg.n_chan, 4, cfg.grid_n, cfg.grid_n), float("nan"), dtype=torch.complex64).pin_memory()
+        for weights in (g.weights.pin_memory(), None):
+            out.fill_(float("nan"))
+            lib.mwa_grid_visibilities_host(p.handle, g.uv.pin_memory(), g.freqs.pin_memory(), g.vis.pin_memory(), weights,
+                                           cfg.n_vis, cfg.n_chan, out)
+            assert_parity(out.numpy(), G, A, "host entry, 4 channel chunks")
+        pageable = torch.empty_like(out)                                    # pageable buffers work too
+        lib.mwa_grid_visibilities_host(p.handle, g.uv, g.freqs, g.vis, g.weights, cfg.n_vis, cfg.n_chan, pageable)
+        assert_parity(pageable.numpy(), G, A, "host entry, pageable")
+
+
 def test_plan_reuse_changing_sizes(lib):
     # workspace growth and reuse: small call, larger call, small again on the same plan
     T = make_kernel_table(7, 8)
