@@ -161,7 +161,9 @@ def run_ours(args):
         g = baseline_major(g)
     plan = lib.Plan(cfg.grid_n, g.cell_du, cfg.support_W, cfg.oversample_O, g.kernel_table, design=args.design)
     lib.mwa_grid_plan_set_profiling(plan.handle, True)
-    grid = torch.empty((cfg.n_chan, 4, cfg.grid_n, cfg.grid_n), dtype=torch.complex64, device=dev)
+    if args.mfs:                                  # comparison runs only: all channels onto one shared grid (f3)
+        plan.set_mfs(True)
+    grid = torch.empty((1 if args.mfs else cfg.n_chan, 4, cfg.grid_n, cfg.grid_n), dtype=torch.complex64, device=dev)
     alg_bytes = cfg.algorithmic_bytes()
     small = alg_bytes < 512e6                     # fits (mostly) in the 126 MB L2: flush between iterations
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if small else None
@@ -251,7 +253,7 @@ def run_ours(args):
         "config": {"workload": f"{cfg.name}: {cfg.n_ant} antennas, {cfg.n_vis} rows x {cfg.n_chan} channels x 4 pol, "
                                f"grid {cfg.grid_n}^2 per channel and pol, kernel {cfg.support_W}x{cfg.support_W} "
                                f"oversampling {cfg.oversample_O}",
-                   "design": args.design, "design_ran": ran, "row_order": args.row_order, "per_gpu": "one full snapshot per rank",
+                   "design": args.design, "design_ran": ran, "row_order": args.row_order, "mfs": bool(args.mfs), "per_gpu": "one full snapshot per rank",
                    "cache": "256 MB L2 flush before every step" if small else
                             f"inputs+outputs {alg_bytes / 1e9:.1f} GB >> 126 MB L2, no flush"},
         "kernel_tap_updates_per_sec": value * cfg.support_W ** 2,
@@ -324,9 +326,12 @@ def main():
     ap.add_argument("--n-chan", type=int, default=0, help="profiling only: cut the config down to this many channels")
     ap.add_argument("--row-order", default="generated", choices=["generated", "baseline-major"],
                     help="comparison runs only: reorder the rows of a multi-integration config [baseline][integration]")
+    ap.add_argument("--mfs", action="store_true", help="comparison runs only: multi-frequency synthesis onto one shared grid (implies --no-e2e)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
+    if args.mfs:
+        args.no_e2e = True
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         # not under torchrun: launch the ranks the way the driver does and hand over
         import socket

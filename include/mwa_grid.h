@@ -108,6 +108,15 @@ int mwa_grid_count_dropped(mwa_grid_plan* plan, const double* uv_f64, const doub
  * rounding is added per call and cell.  Takes effect at the next call. */
 int mwa_grid_plan_set_accumulate(mwa_grid_plan* plan, int enabled);
 
+/* f3 - multi-frequency synthesis onto one shared grid ("readily aggregated in frequency"; SURVEY.md section
+ * 8(f)-3).  When enabled, the samples of ALL channels of a call are summed onto ONE set of grids: grid_out is
+ * [4][N][N][2] floats (n_chan = 1 planes) = sum over c of the per-channel grids of the default mode, overwritten (or
+ * added to, with accumulate-into).  Different channels now write the same cells, so ownership ends at the tile: K3c adds
+ * its register tiles with red.global.add.v4.f32, K0 and K3b (register ownership with flush on cell change - the workload
+ * that design is made for) reduce as they always do; summation order and hence the last bits vary from run to run.
+ * Designs: AUTO (= GATHER), GATHER, ATOMIC, ROMEIN, ROMEIN_SORTED; others return MWA_GRID_ERR_INVALID.  Next call on. */
+int mwa_grid_plan_set_mfs(mwa_grid_plan* plan, int enabled);
+
 /* Select the gridding design (MWA_GRID_DESIGN_*).  Takes effect at the next call. */
 int mwa_grid_plan_set_design(mwa_grid_plan* plan, int design);
 

@@ -34,6 +34,8 @@ _lib.mwa_grid_compute_indices.argtypes = [_P, _P, _P, _LL, _I, _P, _P]
 _lib.mwa_grid_compute_indices.restype = _I
 _lib.mwa_grid_count_dropped.argtypes = [_P, _P, _P, _LL, _I, _P, _P]
 _lib.mwa_grid_count_dropped.restype = _I
+_lib.mwa_grid_plan_set_mfs.argtypes = [_P, _I]
+_lib.mwa_grid_plan_set_mfs.restype = _I
 _lib.mwa_grid_plan_set_accumulate.argtypes = [_P, _I]
 _lib.mwa_grid_plan_set_accumulate.restype = _I
 _lib.mwa_grid_plan_set_design.argtypes = [_P, _I]
@@ -66,7 +68,7 @@ _lib.mwa_grid_last_error.restype = ctypes.c_char_p
 EXPORTS = ["mwa_grid_plan_create", "mwa_grid_plan_destroy", "mwa_grid_visibilities", "mwa_grid_visibilities_host",
            "mwa_grid_compute_indices", "mwa_grid_plan_set_design", "mwa_grid_plan_set_profiling",
            "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_plan_last_design", "mwa_grid_plan_last_stats", "mwa_grid_plan_set_list_pool", "mwa_grid_probe_fp32", "mwa_grid_last_error",
-           "mwa_image_from_grid", "mwa_image_correction", "mwa_image_stokes", "mwa_grid_probe_smem_atomics", "mwa_grid_count_dropped", "mwa_grid_plan_set_accumulate"]
+           "mwa_image_from_grid", "mwa_image_correction", "mwa_image_stokes", "mwa_grid_probe_smem_atomics", "mwa_grid_count_dropped", "mwa_grid_plan_set_accumulate", "mwa_grid_plan_set_mfs"]
 
 
 class MwaGridError(RuntimeError):
@@ -158,6 +160,11 @@ def mwa_grid_count_dropped(plan, uv_f64, freqs, n_vis, n_chan, stream=None) -> i
     return int(out.value)
 
 
+def mwa_grid_plan_set_mfs(plan, enabled: bool) -> None:
+    """f3: multi-frequency synthesis - all channels of a call are summed onto one grid [4, N, N]."""
+    _check(_lib.mwa_grid_plan_set_mfs(plan, 1 if enabled else 0))
+
+
 def mwa_grid_plan_set_accumulate(plan, enabled: bool) -> None:
     """f3: grid_out += gridded samples instead of grid_out = (cells nothing reaches stay as they are)."""
     _check(_lib.mwa_grid_plan_set_accumulate(plan, 1 if enabled else 0))
@@ -240,9 +247,14 @@ class Plan:
 
     def __init__(self, grid_n, cell_du, support_W, oversample_O, kernel_table, design="auto"):
         self.grid_n, self.support_W, self.oversample_O = int(grid_n), int(support_W), int(oversample_O)
+        self.mfs = False
         self.handle = mwa_grid_plan_create(grid_n, cell_du, support_W, oversample_O, kernel_table)
         if design != "auto":
             mwa_grid_plan_set_design(self.handle, design)
+
+    def set_mfs(self, enabled: bool):
+        mwa_grid_plan_set_mfs(self.handle, enabled)
+        self.mfs = bool(enabled)
 
     def set_design(self, design):
         mwa_grid_plan_set_design(self.handle, design)
@@ -257,9 +269,9 @@ class Plan:
         if weights is not None and tuple(weights.shape) != (n_vis, n_chan):
             raise ValueError(f"weights must be [n_vis={n_vis}, n_chan={n_chan}], got {tuple(weights.shape)}")
         if out is None:
-            out = torch.empty((n_chan, 4, self.grid_n, self.grid_n), dtype=torch.complex64, device=uv.device)
-        elif tuple(out.shape) != (n_chan, 4, self.grid_n, self.grid_n):
-            raise ValueError(f"out must be [n_chan={n_chan}, 4, {self.grid_n}, {self.grid_n}], got {tuple(out.shape)}")
+            out = torch.empty((1 if self.mfs else n_chan, 4, self.grid_n, self.grid_n), dtype=torch.complex64, device=uv.device)
+        elif tuple(out.shape) != (1 if self.mfs else n_chan, 4, self.grid_n, self.grid_n):
+            raise ValueError(f"out must be [{'1' if self.mfs else n_chan}, 4, {self.grid_n}, {self.grid_n}], got {tuple(out.shape)}")
         for name, t in (("freqs", freqs), ("vis", vis), ("weights", weights), ("out", out)):
             if t is not None and t.device != uv.device:
                 raise ValueError(f"{name} lives on {t.device}, uv on {uv.device}: all arguments must be on the plan's device")

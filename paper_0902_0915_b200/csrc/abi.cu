@@ -161,12 +161,18 @@ static int grid_device(Plan* p, const double* uv, const double* freqs, const flo
         if (!launch_binning(p, uv, n_vis, n_chan, st)) return MWA_GRID_ERR_CUDA;
     if (prof) cudaEventRecord(p->ev[1], st);
     bool ok = false;
+    const int out_chan = p->mfs ? 1 : n_chan;              // grids the call writes
     if (n_vis == 0 && p->accumulate) {
         ok = true;                                // nothing to add
     } else if (n_vis == 0) {
-        ok = cuda_ok(cudaMemsetAsync(grid, 0, (size_t)n_chan * 4 * p->geom.N * p->geom.N * 8, st), "memset grid");
+        ok = cuda_ok(cudaMemsetAsync(grid, 0, (size_t)out_chan * 4 * p->geom.N * p->geom.N * 8, st), "memset grid");
         p->last_launches += 1;
     } else {
+        if (p->mfs && design != MWA_GRID_DESIGN_AUTO && design != MWA_GRID_DESIGN_GATHER && design != MWA_GRID_DESIGN_ATOMIC &&
+            design != MWA_GRID_DESIGN_ROMEIN && design != MWA_GRID_DESIGN_ROMEIN_SORTED) {
+            set_error("multi-frequency synthesis is implemented by the designs AUTO (= GATHER), GATHER, ATOMIC and ROMEIN only");
+            return MWA_GRID_ERR_INVALID;
+        }
         if (p->accumulate && (design == MWA_GRID_DESIGN_SMEM || design == MWA_GRID_DESIGN_CHAN)) {
             set_error("accumulate-into is implemented by the designs AUTO, GATHER, CHANWS, ATOMIC and ROMEIN only");
             return MWA_GRID_ERR_INVALID;
@@ -183,7 +189,7 @@ static int grid_device(Plan* p, const double* uv, const double* freqs, const flo
                 // the choice is made on the device by scale_kernel (the host never reads freqs): both kernels
                 // are enqueued and the one that was not picked returns at once
                 ok = true;
-                if (n_chan < kChanMinChannels) {
+                if (n_chan < kChanMinChannels || p->mfs) {
                     // the device-side rule can only pick the gather kernel: the channel-SIMD kernels and their pre-passes
                     // are not enqueued at all (small single-channel calls are launch-bound)
                     p->last_chanws = false;
@@ -331,6 +337,12 @@ int mwa_grid_plan_set_accumulate(mwa_grid_plan* plan, int enabled) {
     return MWA_GRID_OK;
 }
 
+int mwa_grid_plan_set_mfs(mwa_grid_plan* plan, int enabled) {
+    if (!plan) { set_error("plan is NULL"); return MWA_GRID_ERR_INVALID; }
+    reinterpret_cast<Plan*>(plan)->mfs = enabled != 0;
+    return MWA_GRID_OK;
+}
+
 int mwa_grid_plan_set_profiling(mwa_grid_plan* plan, int enabled) {
     if (!plan) { set_error("plan is NULL"); return MWA_GRID_ERR_INVALID; }
     Plan* p = reinterpret_cast<Plan*>(plan);
@@ -461,7 +473,7 @@ int mwa_grid_visibilities_host(mwa_grid_plan* plan, const double* uv_f64, const 
     if (n_chan == 0) { p->last_launches = 0; return MWA_GRID_OK; }
     if (!grid_out) { set_error("grid_out is NULL"); return MWA_GRID_ERR_INVALID; }
     if (n_vis > 0 && !vis_c64) { set_error("vis_c64 is NULL"); return MWA_GRID_ERR_INVALID; }
-    if (p->accumulate) { set_error("accumulate-into works on device grids only (mwa_grid_visibilities)"); return MWA_GRID_ERR_INVALID; }
+    if (p->accumulate || p->mfs) { set_error("accumulate-into and multi-frequency synthesis work on device grids only (mwa_grid_visibilities)"); return MWA_GRID_ERR_INVALID; }
     cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
     auto up = [](size_t b) { return (b + 255) & ~size_t(255); };
     // Channels own their grids, so the call is pipelined over channel chunks (multiples of 32 channels, ~8 per call):

@@ -135,7 +135,7 @@ __device__ __forceinline__ void red_add_v2(float* addr, float a, float b) {
 __global__ void atomic_grid_kernel(GridGeom g, const double2* __restrict__ uv, const double* __restrict__ scale,
                                    const float4* __restrict__ vis, const float* __restrict__ weights,
                                    const float* __restrict__ table, long long n_vis, int n_chan,
-                                   float* __restrict__ grid) {
+                                   float* __restrict__ grid, int mfs) {
     const long long total = n_vis * (long long)n_chan * g.W;
     const size_t plane = (size_t)g.N * g.N;
     for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < total;
@@ -151,7 +151,7 @@ __global__ void atomic_grid_kernel(GridGeom g, const double2* __restrict__ uv, c
         const float4 va = vis[2 * sample], vb = vis[2 * sample + 1];
         const float z[8] = {wt * va.x, wt * va.y, wt * va.z, wt * va.w, wt * vb.x, wt * vb.y, wt * vb.z, wt * vb.w};
         const float kv = table[s.rv * g.W + tv];
-        float* base = grid + ((size_t)c * 4 * plane + (size_t)(s.iv + tv - g.h) * g.N + (size_t)(s.iu - g.h)) * 2;
+        float* base = grid + ((size_t)(mfs ? 0 : c) * 4 * plane + (size_t)(s.iv + tv - g.h) * g.N + (size_t)(s.iu - g.h)) * 2;
         for (int tu = 0; tu < g.W; ++tu) {
             const float kk = kv * table[s.ru * g.W + tu];
 #pragma unroll
@@ -163,7 +163,7 @@ __global__ void atomic_grid_kernel(GridGeom g, const double2* __restrict__ uv, c
 
 bool launch_atomic(Plan* p, const double* uv, const float* vis, const float* w, long long n_vis, int n_chan,
                    float* grid, cudaStream_t st) {
-    const size_t bytes = (size_t)n_chan * 4 * p->geom.N * p->geom.N * 8;
+    const size_t bytes = (size_t)(p->mfs ? 1 : n_chan) * 4 * p->geom.N * p->geom.N * 8;
     if (!p->accumulate) {                                       // accumulate-into: the atomics add onto what is there
         if (!cuda_ok(cudaMemsetAsync(grid, 0, bytes, st), "memset grid")) return false;
         p->last_launches += 1;
@@ -173,7 +173,7 @@ bool launch_atomic(Plan* p, const double* uv, const float* vis, const float* w, 
     long long blocks = (total + 255) / 256;
     if (blocks > (long long)p->sm_count * 32) blocks = (long long)p->sm_count * 32;
     atomic_grid_kernel<<<(unsigned)blocks, 256, 0, st>>>(p->geom, (const double2*)uv, p->ws.d_scale,
-                                                         (const float4*)vis, w, p->d_table, n_vis, n_chan, grid);
+                                                         (const float4*)vis, w, p->d_table, n_vis, n_chan, grid, p->mfs ? 1 : 0);
     p->last_launches += 1;
     return cuda_ok(cudaGetLastError(), "atomic_grid_kernel");
 }

@@ -44,6 +44,8 @@ struct GatherParams {
     int rlu, rlv;               // padded row lengths of the shifted table copies
     long long n_items;
     int accumulate;             // 1: grid += (f3 accumulate-into), 0: grid = (R10)
+    int mfs;                    // 1: all channels add into ONE grid [4][N][N] (f3 multi-frequency synthesis): the write-out of a
+                                //    (tile, channel) item is a reduction (red.global.add.v4.f32) into the zero-filled shared grid
     int chunk;                  // consecutive work items per claim (1..8; amortises the round trip of the work counter)
 };
 
@@ -173,6 +175,7 @@ gather_kernel(const GatherParams P) {
                 for (int p = 0; p < 4; ++p) acc[i][j][p] = 0ull;
 
         int n_buf = 0;
+        bool any_hit = false;                                              // MFS: an item without hits has nothing to add
 
         // consume the buffered hits: loads of w*V, transpose, per-lane walk
         auto consume = [&](int n) {
@@ -342,6 +345,7 @@ gather_kernel(const GatherParams P) {
                 const unsigned ball = __ballot_sync(0xffffffffu, hit);
                 const int cnt = __popc(ball);
                 if (cnt == 0) continue;
+                any_hit = true;
                 if (n_buf + cnt > kCap) { consume(n_buf); n_buf = 0; }
                 if (hit) {
                     const int slot = n_buf + __popc(ball & lt_mask);
@@ -370,7 +374,32 @@ gather_kernel(const GatherParams P) {
         if (n_buf > 0) consume(n_buf);
 
         // ---- a5: write the lane's 4x2 block of all 4 planes, once
-        {
+        if (P.mfs) {
+            if (any_hit) {
+                const int x = X0 + 4 * bx;
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    const int y = Y0 + 2 * by + i;
+                    if (y < g.N) {
+#pragma unroll
+                        for (int p = 0; p < 4; ++p) {
+                            float* dst = P.grid + ((size_t)p * plane + (size_t)y * g.N + x) * 2;
+                            float a0, a1, a2, a3;
+                            if (x + 1 < g.N) {
+                                unpack2(acc[i][0][p], a0, a1);
+                                unpack2(acc[i][1][p], a2, a3);
+                                asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(a0), "f"(a1), "f"(a2), "f"(a3) : "memory");
+                            }
+                            if (x + 3 < g.N) {
+                                unpack2(acc[i][2][p], a0, a1);
+                                unpack2(acc[i][3][p], a2, a3);
+                                asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst + 4), "f"(a0), "f"(a1), "f"(a2), "f"(a3) : "memory");
+                            }
+                        }
+                    }
+                }
+            }
+        } else {
             const int x = X0 + 4 * bx;
 #pragma unroll
             for (int i = 0; i < 2; ++i) {
@@ -425,6 +454,11 @@ bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, i
     P.grid = grid;
     P.n_chan = n_chan;
     P.accumulate = p->accumulate ? 1 : 0;
+    P.mfs = p->mfs ? 1 : 0;
+    if (p->mfs && !p->accumulate) {                             // the reductions need a zeroed grid
+        if (!cuda_ok(cudaMemsetAsync(grid, 0, (size_t)4 * p->geom.N * p->geom.N * 8, st), "memset grid")) return false;
+        p->last_launches += 1;
+    }
     P.nb = (p->geom.N + kBucketCells - 1) / kBucketCells;
     P.nt = (p->geom.N + kTile - 1) / kTile;
     P.rlu = (p->geom.W + 6 + 3) & ~3;

@@ -28,6 +28,7 @@ struct RomeinParams {
     float* grid;
     long long n_vis;
     int n_chan, n_chunks;
+    int mfs;                    // 1: every channel adds into the one shared grid [4][N][N] (multi-frequency synthesis)
 };
 
 __device__ __forceinline__ void rom_red_v2(float* addr, float a, float b) {
@@ -52,7 +53,7 @@ __global__ void romein_kernel(const RomeinParams P) {
     int cx = -1, cy = -1;                                            // the cell the sums belong to
     auto flush = [&]() {
         if (cx >= 0) {
-            float* base = P.grid + ((size_t)c * 4 * plane + (size_t)cy * g.N + cx) * 2;
+            float* base = P.grid + ((size_t)(P.mfs ? 0 : c) * 4 * plane + (size_t)cy * g.N + cx) * 2;
 #pragma unroll
             for (int p = 0; p < 4; ++p) rom_red_v2(base + p * plane * 2, acc[2 * p], acc[2 * p + 1]);
         }
@@ -106,7 +107,7 @@ __global__ void romein_kernel(const RomeinParams P) {
 
 bool launch_romein(Plan* p, const double* uv, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                    const int* perm, cudaStream_t st) {
-    const size_t bytes = (size_t)n_chan * 4 * p->geom.N * p->geom.N * 8;
+    const size_t bytes = (size_t)(p->mfs ? 1 : n_chan) * 4 * p->geom.N * p->geom.N * 8;
     if (!p->accumulate) {                                       // accumulate-into: the reductions add onto what is there
         if (!cuda_ok(cudaMemsetAsync(grid, 0, bytes, st), "memset grid")) return false;
         p->last_launches += 1;
@@ -122,6 +123,7 @@ bool launch_romein(Plan* p, const double* uv, const float* vis, const float* w, 
     P.grid = grid;
     P.n_vis = n_vis;
     P.n_chan = n_chan;
+    P.mfs = p->mfs ? 1 : 0;
     P.n_chunks = (int)((n_vis + krChunk - 1) / krChunk);
     const long long blocks = (long long)P.n_chunks * n_chan;
     if (blocks == 0) return true;

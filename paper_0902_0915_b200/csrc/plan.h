@@ -74,6 +74,7 @@ struct Plan {
     int fft_handle[2] = {0, 0};      // cached cuFFT plans ...
     int fft_batch[2] = {0, 0};       // ... and the batch sizes they were made for (0 = none)
     cudaStream_t copy_stream[2] = {nullptr, nullptr};   // host entry point: upload / download streams of the channel-chunk pipeline
+    bool mfs = false;                // f3: all channels of a call are summed onto ONE grid [4][N][N] (mwa_grid_plan_set_mfs)
     bool accumulate = false;         // f3: grid_out += instead of = (mwa_grid_plan_set_accumulate)
     long long pool_limit = 0;        // diagnostics: cap on K6's hit-list pool in entries (0 = default sizing)
     bool last_chanws = false;        // AUTO: the channel-SIMD kernel enqueued by the last call was K6 (else K5)

@@ -549,3 +549,24 @@ def test_accumulate_into_adds_row_batches_onto_one_grid(lib, design, fine):
     bound = 1e-5 * A + 1e-7 + 3 * 2.0 ** -24 * (np.abs(prev) + np.abs(want))
     assert np.all(np.abs(got.astype(np.complex128) - want) <= bound), float(np.max(np.abs(got - want) / bound))
     assert_parity(again, G, A, f"{design} overwrite after accumulate")
+
+
+# ---------------------------------------------------------------------------- f3: multi-frequency synthesis
+@pytest.mark.parametrize("design", ["auto", "gather", "atomic", "romein", "romein_sorted"])
+def test_multi_frequency_synthesis_sums_the_channels_onto_one_grid(lib, design):
+    g = generate(scaled(CONFIGS["C2"], n_ant=48, n_chan=12, grid_n=250))
+    G, A, _ = _oracle(g)
+    G, A = G.sum(axis=0, keepdims=True), A.sum(axis=0, keepdims=True)      # the definition: one grid = sum over channels
+    _to_dev(g)
+    with _plan(lib, g, design) as p:
+        p.set_mfs(True)
+        out = p.grid(g.uv, g.freqs, g.vis, g.weights)
+        assert tuple(out.shape) == (1, 4, 250, 250)
+        assert_parity(out.cpu().numpy(), G, A, f"MFS {design}")
+        lib.mwa_grid_plan_set_accumulate(p.handle, True)                    # MFS + accumulate-into: a second pass doubles it
+        p.grid(g.uv, g.freqs, g.vis, g.weights, out=out)
+        assert_parity(out.cpu().numpy(), 2 * G, 2 * A, f"MFS {design} accumulated twice")
+        lib.mwa_grid_plan_set_accumulate(p.handle, False)
+        p.set_mfs(False)
+        back = p.grid(g.uv, g.freqs, g.vis, g.weights)                      # and back to one grid per channel
+        assert tuple(back.shape) == (12, 4, 250, 250)
