@@ -27,49 +27,64 @@ __global__ void bin_count_kernel(GridGeom g, const double2* __restrict__ uv, con
     }
 }
 
-// Exclusive scan of count[0..n] in place (count[n] receives the total); one block, 1024 threads.
-__global__ void bin_scan_kernel(int* __restrict__ count, int n, int* __restrict__ cursor) {
+// Exclusive scan of count[0..n] in place (count[n] receives the total).  A block of 1024 threads takes 4096 consecutive
+// entries, publishes its sum in blk_state (zeroed by the call's memset; flag bit 30) and adds up the sums of the blocks
+// before it - they were scheduled before it, so the wait cannot deadlock (the one-level decoupled scan of
+// chan_order_kernel; a single block needed 15 - 60 us for the 16 K - 262 K buckets of C4 - C5).
+constexpr int kScanPerBlock = 4096;
+constexpr int kScanFlag = 1 << 30;
+
+__global__ void __launch_bounds__(1024)
+bin_scan_kernel(int* __restrict__ count, int n, int* __restrict__ cursor, volatile int* blk_state) {
     __shared__ int warp_sum[32];
-    __shared__ int carry_s;
-    if (threadIdx.x == 0) carry_s = 0;
-    __syncthreads();
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    for (int base = 0; base < n; base += 1024 * 4) {
-        const int i0 = base + threadIdx.x * 4;
-        int v[4];
+    __shared__ int prefix_s;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, b = blockIdx.x;
+    const int i0 = b * kScanPerBlock + threadIdx.x * 4;
+    int v[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) v[k] = (i0 + k < n) ? count[i0 + k] : 0;
-        const int tsum = v[0] + v[1] + v[2] + v[3];
-        int inc = tsum;
+    for (int k = 0; k < 4; ++k) v[k] = (i0 + k < n) ? count[i0 + k] : 0;
+    const int tsum = v[0] + v[1] + v[2] + v[3];
+    int inc = tsum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) warp_sum[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        int ws = warp_sum[lane];
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            const int t = __shfl_up_sync(0xffffffffu, inc, o);
-            if (lane >= o) inc += t;
+            const int t = __shfl_up_sync(0xffffffffu, ws, o);
+            if (lane >= o) ws += t;
         }
-        if (lane == 31) warp_sum[wid] = inc;
-        __syncthreads();
-        if (wid == 0) {
-            int ws = warp_sum[lane];
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int t = __shfl_up_sync(0xffffffffu, ws, o);
-                if (lane >= o) ws += t;
+        warp_sum[lane] = ws;                     // inclusive over warps
+        const int total = __shfl_sync(0xffffffffu, ws, 31);
+        if (lane == 0) blk_state[b] = total | kScanFlag;
+        int sum = 0;
+        for (int j0 = 0; j0 < b; j0 += 32) {
+            const int j = j0 + lane;
+            int t = 0;
+            if (j < b) {
+                do { t = blk_state[j]; } while (!(t & kScanFlag));
+                t &= ~kScanFlag;
             }
-            warp_sum[lane] = ws;                 // inclusive over warps
+            sum += t;
         }
-        __syncthreads();
-        const int carry = carry_s;
-        int excl = carry + (wid > 0 ? warp_sum[wid - 1] : 0) + inc - tsum;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            if (i0 + k < n) { count[i0 + k] = excl; cursor[i0 + k] = excl; }
-            excl += v[k];
+        sum = __reduce_add_sync(0xffffffffu, sum);
+        if (lane == 0) {
+            prefix_s = sum;
+            if (b == (int)gridDim.x - 1) count[n] = sum + total;
         }
-        __syncthreads();
-        if (threadIdx.x == 1023) carry_s = carry + warp_sum[31];
-        __syncthreads();
     }
-    if (threadIdx.x == 0) count[n] = carry_s;
+    __syncthreads();
+    int excl = prefix_s + (wid > 0 ? warp_sum[wid - 1] : 0) + inc - tsum;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        if (i0 + k < n) { count[i0 + k] = excl; cursor[i0 + k] = excl; }
+        excl += v[k];
+    }
 }
 
 __global__ void bin_scatter_kernel(GridGeom g, const double2* __restrict__ uv, const double* __restrict__ s_ref_p,
@@ -149,19 +164,126 @@ __global__ void tile_order_scatter_kernel(const int* __restrict__ weight, int n_
     }
 }
 
+// ---------------------------------------------------------------- small problems: the whole of a3 in one CTA
+// C1-sized calls (<= 4096 rows, <= 2048 buckets, <= 1024 tiles) are launch-bound: seven binning kernels and a memset
+// for a problem whose roofline is below a microsecond.  One block of 1024 threads does the same steps in shared memory -
+// histogram, scan, scatter, ascending row order inside every bucket, tile weights and the heaviest-first tile order - and
+// writes the same arrays (bucket_start, perm, uv_sorted, row_sorted, tile_weight, tile_order) with the same contents,
+// except that equal-weight tiles are ordered by index here (the multi-kernel path orders them as its atomics fall).
+constexpr int kSmallRows = 4096, kSmallBuckets = 2048, kSmallTiles = 1024;   // 36 KB of static shared memory
+
+__global__ void __launch_bounds__(1024)
+bin_small_kernel(GridGeom g, const double2* __restrict__ uv, const double* __restrict__ s_ref_p, int n_vis, int nb, int nt,
+                 int* __restrict__ bucket_start, int* __restrict__ perm, double2* __restrict__ uv_sorted,
+                 double4* __restrict__ row_sorted, int* __restrict__ tile_weight, int* __restrict__ tile_order) {
+    __shared__ int s_start[kSmallBuckets + 1];      // counts, then exclusive starts
+    __shared__ int s_cursor[kSmallBuckets];
+    __shared__ unsigned short s_tmp[kSmallRows];    // rows in bucket order, arbitrary inside a bucket
+    __shared__ unsigned short s_bkt[kSmallRows];    // bucket of row n
+    __shared__ int s_warp[32];
+    __shared__ int s_tw[kSmallTiles];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int n_buckets = nb * nb, n_tiles = nt * nt;
+    const double s_ref = *s_ref_p;
+    for (int b = tid; b <= n_buckets; b += 1024) s_start[b] = 0;
+    __syncthreads();
+    for (int n = tid; n < n_vis; n += 1024) {
+        const double2 p = uv[n];
+        const int b = bucket_coord(p.y, s_ref, g.inv_du, g.N, nb) * nb + bucket_coord(p.x, s_ref, g.inv_du, g.N, nb);
+        s_bkt[n] = (unsigned short)b;
+        atomicAdd(&s_start[b], 1);
+    }
+    __syncthreads();
+    // exclusive scan of up to 4096 counts: 4 per thread, warp scan, scan of the warp sums
+    {
+        const int i0 = tid * 4;
+        int v[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) v[k] = (i0 + k < n_buckets) ? s_start[i0 + k] : 0;
+        const int tsum = v[0] + v[1] + v[2] + v[3];
+        int inc = tsum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) s_warp[wid] = inc;
+        __syncthreads();
+        if (wid == 0) {
+            int ws = s_warp[lane];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, ws, o);
+                if (lane >= o) ws += t;
+            }
+            s_warp[lane] = ws;
+        }
+        __syncthreads();
+        int excl = (wid > 0 ? s_warp[wid - 1] : 0) + inc - tsum;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (i0 + k < n_buckets) { s_start[i0 + k] = excl; s_cursor[i0 + k] = excl; bucket_start[i0 + k] = excl; }
+            excl += v[k];
+        }
+        if (tid == 0) { s_start[n_buckets] = n_vis; bucket_start[n_buckets] = n_vis; }
+    }
+    __syncthreads();
+    for (int n = tid; n < n_vis; n += 1024) s_tmp[atomicAdd(&s_cursor[s_bkt[n]], 1)] = (unsigned short)n;
+    __syncthreads();
+    // ascending row order inside every bucket: rank = number of smaller row ids of the same bucket
+    for (int i = tid; i < n_vis; i += 1024) {
+        const int row = s_tmp[i], b = s_bkt[row];
+        const int k0 = s_start[b], k1 = s_start[b + 1];
+        int rank = 0;
+        for (int j = k0; j < k1; ++j) rank += s_tmp[j] < row;
+        const double2 p = uv[row];
+        perm[k0 + rank] = row;
+        uv_sorted[k0 + rank] = p;
+        row_sorted[k0 + rank] = make_double4(p.x, p.y, (double)row, 0.0);
+    }
+    // tile weights (rows whose bucket lies under the tile) and the heaviest-first order (ties by tile index)
+    const int per = kTile / kBucketCells;
+    for (int t = tid; t < n_tiles; t += 1024) {
+        const int ty = t / nt, tx = t - ty * nt;
+        int w = 0;
+        for (int dy = 0; dy < per; ++dy) {
+            const int by = ty * per + dy;
+            if (by >= nb) break;
+            const int b0 = by * nb + tx * per, b1 = by * nb + min(nb, tx * per + per);
+            if (b0 < b1) w += s_start[b1] - s_start[b0];
+        }
+        s_tw[t] = w;
+        tile_weight[t] = w;
+    }
+    __syncthreads();
+    for (int t = tid; t < n_tiles; t += 1024) {
+        const int w = s_tw[t];
+        int rank = 0;
+        for (int u = 0; u < n_tiles; ++u) rank += (s_tw[u] > w) || (s_tw[u] == w && u < t);
+        tile_order[rank] = t;
+    }
+}
+
 bool launch_binning(Plan* p, const double* uv, long long n_vis, int /*n_chan*/, cudaStream_t st) {
     Workspace& ws = p->ws;
     const int nb = (p->geom.N + kBucketCells - 1) / kBucketCells;
     const int n_buckets = nb * nb;
     const int nt = (p->geom.N + kTile - 1) / kTile;
+    if (!cuda_ok(cudaMemsetAsync(ws.d_misc, 0, (size_t)kMiscInts * sizeof(int), st), "memset misc")) return false;
+    if (n_vis <= kSmallRows && n_buckets <= kSmallBuckets && nt * nt <= kSmallTiles) {
+        bin_small_kernel<<<1, 1024, 0, st>>>(p->geom, (const double2*)uv, ws.d_scale_ref, (int)n_vis, nb, nt, ws.d_bucket_count,
+                                             ws.d_perm, ws.d_uv_sorted, (double4*)ws.d_row_sorted, ws.d_tile_weight, ws.d_tile_order);
+        p->last_launches += 2;
+        return cuda_ok(cudaGetLastError(), "bin_small_kernel");
+    }
     if (!cuda_ok(cudaMemsetAsync(ws.d_bucket_count, 0, ((size_t)n_buckets + 1) * sizeof(int), st), "memset buckets"))
         return false;
-    if (!cuda_ok(cudaMemsetAsync(ws.d_misc, 0, (size_t)kMiscInts * sizeof(int), st), "memset misc")) return false;
     int blocks = (int)((n_vis + 255) / 256);
     if (blocks > p->sm_count * 8) blocks = p->sm_count * 8;
     bin_count_kernel<<<blocks, 256, 0, st>>>(p->geom, (const double2*)uv, ws.d_scale_ref, (int)n_vis, nb,
                                              ws.d_bucket_count);
-    bin_scan_kernel<<<1, 1024, 0, st>>>(ws.d_bucket_count, n_buckets, ws.d_bucket_cursor);
+    bin_scan_kernel<<<(n_buckets + kScanPerBlock - 1) / kScanPerBlock, 1024, 0, st>>>(ws.d_bucket_count, n_buckets, ws.d_bucket_cursor,
+                                                                                     ws.d_misc + kMiscScanState);
     bin_scatter_kernel<<<blocks, 256, 0, st>>>(p->geom, (const double2*)uv, ws.d_scale_ref, (int)n_vis, nb,
                                                ws.d_bucket_cursor, ws.d_perm_tmp);
     {

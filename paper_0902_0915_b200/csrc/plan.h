@@ -15,7 +15,8 @@ constexpr int kTile = 16;           // gridding tile side in cells (one warp own
 // d_misc (ints, zeroed by every call's binning step): [0..3] work counters, [4..11] diagnostics, [12..13] hit-list pool
 // cursor (u64), [14..15] K6 item counts, [16..] tile-weight histogram (4096), then the block states of chan_order_kernel
 constexpr int kMiscOrderState = 16 + 4096;
-constexpr int kMiscInts = kMiscOrderState + 2048;
+constexpr int kMiscScanState = kMiscOrderState + 2048;   // block states of bin_scan_kernel (<= 1024 blocks: 4 M buckets)
+constexpr int kMiscInts = kMiscScanState + 1024;
 
 struct Workspace {
     // a1
