@@ -102,13 +102,25 @@ __global__ void bin_scatter_kernel(GridGeom g, const double2* __restrict__ uv, c
 // ~8 rows on average, a few hundred in the core) and writes the sorted copies.  With this the bucket-sorted order is a
 // pure function of the input, so K3c and K5 - which add the taps of a cell in list order, with no atomics - give
 // bit-identical grids from run to run.
+// A bucket of more than kOrderWarpMax rows (a degenerate input: a compact array, a coarse du, many rows at uv = 0) is
+// not ranked here - k^2 / 32 steps per lane would look like a hang - but put on a list for bin_order_large_kernel.
+constexpr int kOrderWarpMax = 2048;
+constexpr int kBigListCap = 1023;                      // n_vis / kOrderWarpMax big buckets at most: 2 M rows and more
+
 __global__ void bin_order_kernel(const double2* __restrict__ uv, const int* __restrict__ bucket_start, int n_buckets,
                                  const int* __restrict__ perm_tmp, int* __restrict__ perm,
-                                 double2* __restrict__ uv_sorted, double4* __restrict__ row_sorted) {
+                                 double2* __restrict__ uv_sorted, double4* __restrict__ row_sorted, int* __restrict__ big_list) {
     const int lane = threadIdx.x & 31;
     const int warps = (gridDim.x * blockDim.x) >> 5;
     for (int b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; b < n_buckets; b += warps) {
         const int k0 = bucket_start[b], k1 = bucket_start[b + 1];
+        if (k1 - k0 > kOrderWarpMax) {
+            if (lane == 0) {
+                const int slot = atomicAdd(big_list, 1);
+                if (slot < kBigListCap) big_list[1 + slot] = b;
+            }
+            continue;
+        }
         for (int i = k0 + lane; i < k1; i += 32) {
             const int row = perm_tmp[i];
             int rank = 0;
@@ -118,6 +130,44 @@ __global__ void bin_order_kernel(const double2* __restrict__ uv, const int* __re
             uv_sorted[k0 + rank] = p;
             row_sorted[k0 + rank] = make_double4(p.x, p.y, (double)row, 0.0);      // K5: uv and row id in one 32 B record
         }
+    }
+}
+
+// The big buckets: one block each sorts the bucket's row ids ascending in place - a bitonic network in its all-ascending
+// form (first step of a merge mirrors inside the block of size k, the rest are half-cleaners), so a length that is not a
+// power of two needs no padding: a partner index beyond the end stands for +infinity, which is already in place - and
+// writes the sorted copies.  O(k log^2 k): 1 M rows in ~2 ms.  Returns at once when the list is empty (every normal call).
+__global__ void __launch_bounds__(1024)
+bin_order_large_kernel(const double2* __restrict__ uv, const int* __restrict__ bucket_start, int* __restrict__ perm_tmp,
+                       int* __restrict__ perm, double2* __restrict__ uv_sorted, double4* __restrict__ row_sorted,
+                       const int* __restrict__ big_list) {
+    const int n_big = min(big_list[0], kBigListCap);
+    for (int q = blockIdx.x; q < n_big; q += gridDim.x) {
+        const int b = big_list[1 + q];
+        const int k0 = bucket_start[b], n = bucket_start[b + 1] - k0;
+        int* a = perm_tmp + k0;
+        for (int k = 2; (k >> 1) < n; k <<= 1) {
+            for (int i = threadIdx.x; i < n; i += 1024) {            // mirror step
+                const int j = i ^ (k - 1);
+                if (j > i && j < n) { const int x = a[i], y = a[j]; if (x > y) { a[i] = y; a[j] = x; } }
+            }
+            __syncthreads();
+            for (int d = k >> 2; d > 0; d >>= 1) {                   // half-cleaners
+                for (int i = threadIdx.x; i < n; i += 1024) {
+                    const int j = i ^ d;
+                    if (j > i && j < n) { const int x = a[i], y = a[j]; if (x > y) { a[i] = y; a[j] = x; } }
+                }
+                __syncthreads();
+            }
+        }
+        for (int i = threadIdx.x; i < n; i += 1024) {
+            const int row = a[i];
+            const double2 p = uv[row];
+            perm[k0 + i] = row;
+            uv_sorted[k0 + i] = p;
+            row_sorted[k0 + i] = make_double4(p.x, p.y, (double)row, 0.0);
+        }
+        __syncthreads();
     }
 }
 
@@ -290,7 +340,13 @@ bool launch_binning(Plan* p, const double* uv, long long n_vis, int /*n_chan*/, 
         long long oblocks = ((long long)n_buckets * 32 + 255) / 256;
         if (oblocks > p->sm_count * 16) oblocks = p->sm_count * 16;
         bin_order_kernel<<<(unsigned)oblocks, 256, 0, st>>>((const double2*)uv, ws.d_bucket_count, n_buckets, ws.d_perm_tmp, ws.d_perm,
-                                                            ws.d_uv_sorted, (double4*)ws.d_row_sorted);
+                                                            ws.d_uv_sorted, (double4*)ws.d_row_sorted, ws.d_misc + kMiscBigList);
+        if (n_vis > kOrderWarpMax) {                           // else no bucket can be big
+            bin_order_large_kernel<<<p->sm_count < 64 ? p->sm_count : 64, 1024, 0, st>>>((const double2*)uv, ws.d_bucket_count, ws.d_perm_tmp, ws.d_perm,
+                                                                                         ws.d_uv_sorted, (double4*)ws.d_row_sorted,
+                                                                                         ws.d_misc + kMiscBigList);
+            p->last_launches += 1;
+        }
     }
     int* hist = ws.d_misc + 16;
     int tblocks = (nt * nt + 255) / 256;

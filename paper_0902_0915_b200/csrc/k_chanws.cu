@@ -53,8 +53,14 @@ constexpr int k6TileX = 16, k6TileY = 8;
 constexpr int k6Batch = K6_BATCH;                     // hits per batch
 constexpr int k6Stages = K6_STAGES;                   // batches in flight: 6 x 16 hits (measured on C4: 8 x 8 9.43 ms, 14 x 8 8.44, 7 x 16 8.37, 6 x 16 8.34, 28 x 4 9.8)
 constexpr int k6Stagers = 2;                          // stager warps; batch b is staged by stager b % 2 into stage b % 4
-constexpr int k6BatchRing = 32;                       // batch descriptors / queue segments between sweeper and stagers
-constexpr int k6ItemRing = 16;                        // consumer-item descriptors between sweeper and store warp
+#ifndef K6_BATCH_RING
+#define K6_BATCH_RING 32
+#endif
+#ifndef K6_ITEM_RING
+#define K6_ITEM_RING 16
+#endif
+constexpr int k6BatchRing = K6_BATCH_RING;                       // batch descriptors / queue segments between sweeper and stagers
+constexpr int k6ItemRing = K6_ITEM_RING;                        // consumer-item descriptors between sweeper and store warp
 constexpr int k6ZeroChunk = 16;                       // zero items per claim of the store warp
 constexpr unsigned k6ExitItem = 0xffffffffu;
 constexpr int k6Drift = 8;                            // largest spread (cells) of the stamp origins over the 32 channels of a fast hit

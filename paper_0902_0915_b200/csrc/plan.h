@@ -16,7 +16,8 @@ constexpr int kTile = 16;           // gridding tile side in cells (one warp own
 // cursor (u64), [14..15] K6 item counts, [16..] tile-weight histogram (4096), then the block states of chan_order_kernel
 constexpr int kMiscOrderState = 16 + 4096;
 constexpr int kMiscScanState = kMiscOrderState + 2048;   // block states of bin_scan_kernel (<= 1024 blocks: 4 M buckets)
-constexpr int kMiscInts = kMiscScanState + 1024;
+constexpr int kMiscBigList = kMiscScanState + 1024;    // [0] number of big buckets of bin_order_kernel, [1..1023] their ids
+constexpr int kMiscInts = kMiscBigList + 1024;
 
 struct Workspace {
     // a1

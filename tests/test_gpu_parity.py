@@ -312,6 +312,29 @@ def test_dropped_samples_with_nonfinite_values_leave_no_trace(lib, design):
     assert_parity(out2, G1, A1, design + " null weights")
 
 
+@pytest.mark.parametrize("design", ["gather", "chanws"])
+def test_degenerate_input_with_a_huge_uv_bucket(lib, design):
+    # 3000 rows inside one 8 x 8-cell uv bucket (plus a few elsewhere): above 2048 rows the in-bucket ordering switches from
+    # ranking every row against every other one (quadratic: a million-row bucket would look like a hang) to a bitonic sort
+    N, W, O = 128, 7, 8
+    T = make_kernel_table(W, O)
+    rs = np.random.RandomState(4)
+    n_chan = 32 if design == "chanws" else 2
+    fr = 155e6 + 40e3 * np.arange(n_chan)
+    s0 = fr[-1] / C
+    uv = np.concatenate([rs.uniform(16.5, 23.5, (3000, 2)), rs.uniform(-50, 50, (200, 2))]) / s0
+    # partially coherent (random-sign terms would cancel and leave the Frobenius norm of the grid tiny; identical terms are
+    # the worst case of sequential fp32 summation): unit amplitude, phases within +-1 rad; ~2300 terms per cell
+    vis = np.exp(1j * rs.uniform(-1.0, 1.0, (uv.shape[0], n_chan, 4))).astype(np.complex64)
+    G, A, _ = oracle.grid(uv, fr, vis, None, N, 1.0, W, O, T)
+    with lib.Plan(N, 1.0, W, O, T, design=design) as p:
+        t = [torch.from_numpy(x).cuda() for x in (uv, fr, vis)]
+        out = p.grid(*t)
+        out2 = p.grid(*t)
+        assert torch.equal(out.view(torch.float32), out2.view(torch.float32))       # still a deterministic order
+        assert_parity(out.cpu().numpy(), G, A, f"huge bucket {design}")
+
+
 def test_empty_inputs_and_error_codes(lib):
     T = make_kernel_table(7, 8)
     with lib.Plan(64, 1.0, 7, 8, T) as p:
