@@ -527,10 +527,15 @@ int mwa_grid_visibilities_host(mwa_grid_plan* plan, const double* uv_f64, const 
         if (n_chunks > 1 && k >= 2 && cudaStreamWaitEvent(s_up, ev_done[k - 2], 0) != cudaSuccess) { set_error("cudaStreamWaitEvent failed"); fail(MWA_GRID_ERR_CUDA); break; }
         if (n_vis > 0) {
             // the channel slice of the [row][chan] host arrays: a strided (2-D) copy into a contiguous chunk
-            if (!cuda_ok(cudaMemcpy2DAsync(d_vis, (size_t)nc * 32, (const char*)vis_c64 + (size_t)c0 * 32, (size_t)n_chan * 32, (size_t)nc * 32,
-                                           (size_t)n_vis, cudaMemcpyHostToDevice, s_up), "H2D vis")) { fail(MWA_GRID_ERR_CUDA); break; }
-            if (weights && !cuda_ok(cudaMemcpy2DAsync(d_w, (size_t)nc * 4, (const char*)weights + (size_t)c0 * 4, (size_t)n_chan * 4, (size_t)nc * 4,
-                                                      (size_t)n_vis, cudaMemcpyHostToDevice, s_up), "H2D weights")) { fail(MWA_GRID_ERR_CUDA); break; }
+            if (nc == n_chan) {                                             // one chunk: plain contiguous copies
+                if (!cuda_ok(cudaMemcpyAsync(d_vis, vis_c64, (size_t)n_vis * n_chan * 32, cudaMemcpyHostToDevice, s_up), "H2D vis")) { fail(MWA_GRID_ERR_CUDA); break; }
+                if (weights && !cuda_ok(cudaMemcpyAsync(d_w, weights, (size_t)n_vis * n_chan * 4, cudaMemcpyHostToDevice, s_up), "H2D weights")) { fail(MWA_GRID_ERR_CUDA); break; }
+            } else {
+                if (!cuda_ok(cudaMemcpy2DAsync(d_vis, (size_t)nc * 32, (const char*)vis_c64 + (size_t)c0 * 32, (size_t)n_chan * 32, (size_t)nc * 32,
+                                               (size_t)n_vis, cudaMemcpyHostToDevice, s_up), "H2D vis")) { fail(MWA_GRID_ERR_CUDA); break; }
+                if (weights && !cuda_ok(cudaMemcpy2DAsync(d_w, (size_t)nc * 4, (const char*)weights + (size_t)c0 * 4, (size_t)n_chan * 4, (size_t)nc * 4,
+                                                          (size_t)n_vis, cudaMemcpyHostToDevice, s_up), "H2D weights")) { fail(MWA_GRID_ERR_CUDA); break; }
+            }
         }
         float* g = d_grid + (size_t)c0 * 4 * (plane_bytes / 4);
         if (n_chunks > 1) {
