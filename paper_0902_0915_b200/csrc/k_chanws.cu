@@ -6,30 +6,38 @@
 // What changed is everything around the FMA loop.  K5 ran its phases (bucket sweep, fp64 index, staging, FMA,
 // write-out) one after the other on all warps of a CTA, separated by CTA-wide barriers, and repeated the sweep and
 // index work for each 16x4 strip: 5.8 G warp instructions for C4, 80 % of them overhead, issue slot use 42 %
-// (profiles/r01_chan_v8_c4x128.md).  K6 is a producer / consumer pipeline with no CTA-wide barrier in steady state:
+// (profiles/r01_chan_v8_c4x128.md).  K6 is a producer / consumer pipeline with no CTA-wide barrier in steady state
+// (profiles/r02_chanws_c4.md: 4.2 G warp instructions, C4 in 8.05 ms against 11.9 ms):
 //
 //   chan_index_kernel (pre-pass, once per call): the exact fp64 index (index.cuh) of every (row, channel), packed in
 //       32 bits (stamp origin + table row per axis), and per (row, 32-channel group) the bounding box of the stamp
 //       origins over the group's channels.  After it nothing on the path touches fp64 per sample.
+//   chan_list_kernel (pre-pass): one warp per item = (16 x 8 cell tile, 32-channel group) sweeps the uv buckets
+//       (k_bin.cu) under the tile with integer box tests and writes the item's hit list (row, 16-bit block mask) into a
+//       pool; chan_order_kernel splits the items into those with hits and the empty ones.
 //
-//   chanws_kernel, persistent, one CTA of 20 warps per SM; item = (16 x 8 cell tile, 32-channel group):
-//     warp 16  "sweeper"  walks the uv buckets (k_bin.cu) under the item's tile, tests the bounding boxes (integer
-//                         compares), and appends the hits (row, 16-bit block mask) to a queue in batches of 32;
-//     warp 17, 18 "stagers"  one batch each in turn: one bulk-async copy (TMA engine, mbarrier complete_tx) of the
-//                         32 channels x 32 B of visibilities per hit, the packed indices -> per-lane table offsets,
-//                         the weights;
-//     warp 0..15 "consumers" (4 x 4 blocks of 4 x 2 cells): wait on the batch's mbarrier, run the FFMA2 loop of K5
-//                         over the hits that touch their block, release the batch; at the end of an item put the
-//                         accumulators into a 128 B-swizzled stage and signal the store warp;
-//     warp 19  "store"    one cp.async.bulk.tensor store per (2 tile rows x 32 channels x 4 pol) box through a 4-D
-//                         tensor map of grid_out with dimension order (u, channel, v, pol); items nothing reaches
-//                         are zero-filled by this warp from a small zero buffer, involving no other warp.
+//   chanws_kernel, persistent, one CTA of 20 warps per SM:
+//     warp 16  "sweeper"  claims items with hits four at a time and streams their hit lists into a shared-memory queue
+//                         in batches of 16, reading each list in a fixed scattered order (see load_entries); an item
+//                         whose list found no room in the pool is swept here instead;
+//     warp 17, 18 "stagers"  one batch each in turn: cp.async (LDGSTS) of the 32 channels x 32 B of visibilities, the
+//                         packed indices (raw table offsets; the consumer adds its tile term) and the weights of every hit
+//                         straight into one of 6 stages, completion signalled on the stage's mbarrier by
+//                         cp.async.mbarrier.arrive.noinc - a stager never waits for its copies;
+//     warp 0..15 "consumers" (4 x 4 blocks of 4 x 2 cells): wait on the batch's mbarrier (parked try_wait), run the
+//                         FFMA2 loop of K5 over the hits that touch their block, release the batch; at the end of an
+//                         item put the accumulators into a 128 B-swizzled stage slot and signal the store warp;
+//     warp 19  "store"    one thread: one cp.async.bulk.tensor store per (2 tile rows x 32 channels x 4 pol) box through a
+//                         4-D tensor map of grid_out with dimension order (u, channel, v, pol), evict-first in L2;
+//                         claims the empty items from their own list and zero-fills them with 16 KB boxes from a zero
+//                         buffer, paced by the sweeper's progress, involving no other warp.  With accumulate-into the
+//                         boxes go out as tensor-map reduce-adds and the empty items are skipped.
 //
 // No atomics on grid data, every cell of grid_out is written exactly once (R10), the hit order is a pure function
 // of the sorted rows, so the grid is bit-identical from run to run.  Registers: the kernel is compiled for 96 per
 // thread (640 threads); with setmaxnreg the consumers raise themselves to 104 (64 accumulators + two operand sets, no
-// spills) and the four service warps drop to 64: 16 x 104 + 4 x 64 = 20 x 96, exactly the CTA's register pool (an
-// increase that the pool cannot serve blocks for ever).
+// spills) and the four service warps drop to 64: five warps per SM sub-partition, 4 x 104 + 64 <= 512 (an increase
+// that the pool cannot serve blocks for ever - a 21st warp would not fit).
 #include <cuda.h>
 
 #include <cstdint>

@@ -8,16 +8,24 @@
 // how a lane finds its values without scanning everything:
 //
 //   phase A (lane = candidate row): walk the buckets of k_bin.cu that can reach the tile at this channel's
-//            scale, run the exact index function (index.cuh) on each candidate, keep the rows whose WxW
-//            stamp overlaps the tile; per hit store w*V, the table offsets and a 32-bit mask of the lanes
-//            (4x2 blocks) the stamp overlaps.
+//            scale - in a fixed scattered order, groups of 8 sorted rows at a time, so that a buffer of 128 hits is a
+//            spatially mixed sample and the per-lane lists of phase B are balanced - run the exact index function
+//            (index.cuh) on each candidate, keep the rows whose WxW stamp overlaps the tile; per hit store the table
+//            offsets and a 32-bit mask of the lanes (4x2 blocks) the stamp overlaps, and request its visibilities and
+//            weight with cp.async straight into the buffer (they land while the scan goes on).
 //   transpose: a 32x32 bit-matrix transpose by warp shuffles turns "blocks per hit" into "hits per block".
-//   phase B (lane = block owner): each lane walks ITS OWN hit list; all 32 lanes do useful FMAs on
-//            different hits.  Per hit a lane reads w*V (2 x LDS.128), 4 u-taps (LDS.128) and 2 v-taps (LDS.64)
-//            from zero-padded, pre-shifted copies of the kernel table, and issues 32 packed fma.rn.f32x2.
-//   write-out: 16 x STG.128 per lane, streaming (evict-first) so the grid does not push vis lines out of L2.
+//   phase B (lane = block owner): each lane walks ITS OWN hit list, branch-free: a lane whose list is exhausted takes
+//            a null hit (zero visibility, zero weight), so the warp runs one instruction stream with two operand sets in
+//            flight.  Per visit a lane reads V (2 x LDS.128 from the two half planes), geo + weight (LDS.64), 4 u-taps
+//            (LDS.128) and 2 v-taps (LDS.64) from zero-padded, pre-shifted copies of the kernel table, and issues 10 FMUL
+//            and 32 packed fma.rn.f32x2.
+//   write-out: 16 x STG.128 per lane, streaming (evict-first) so the grid does not push vis lines out of L2; with
+//            accumulate-into a read-modify-write of the warp's own cells; with multi-frequency synthesis (all channels
+//            onto one grid) a red.global.add.v4.f32 per 16 B.
 //
-// Work items (tile, channel) are taken from a global counter, channel fastest, tiles heaviest first.
+// Work items (tile, channel) are taken from a global counter up to 8 at a time, channel fastest, tiles heaviest first.
+// profiles/r02_gather_c5.md: C5 in 23.0 ms (round 1: 36.4 ms); bound by the shared-memory pipe (the LDS of phase B are
+// lane-scattered by construction).
 #include "plan.h"
 
 namespace mwa {
