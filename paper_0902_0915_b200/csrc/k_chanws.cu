@@ -100,6 +100,7 @@ struct K6Params {
     const int4* c_desc;          // [n_c] (item, hits or -1, list offset, 0) of the items with hits, in item order (chan_order_kernel)
     const unsigned* z_list;      // [n_z] the items nothing reaches, in item order
     const int* n_cz;             // [2] n_c, n_z
+    const int* n_hits;           // [1] hits of all items (swept items count 64)
     int* zcounter;               // work counter of the zero list
     const uint2* lists;          // [pool_cap] pool of hit lists: (row, mask) entries, an item's hits contiguous and in sweep order
     unsigned pool_cap;           // entries in the pool; 0 = no lists at all
@@ -132,7 +133,7 @@ struct K6Ctrl {
     int b_x0[k6BatchRing], b_y0[k6BatchRing], b_g[k6BatchRing];
     unsigned c_item[k6ItemRing];                            // consumer items in order: tx | ty << 10 | group << 20, k6ExitItem = exit
     volatile int pub_batches, pub_c, done_c;
-    volatile int c_pos;                                     // sweeper: index (in the global list of items with hits) of the item it is on
+    volatile int c_hits;                                    // sweeper: hits of all items before the one it is on (the global work measure)
     volatile int done_batches[k6Stagers];
     volatile int abort;
     alignas(16) int z_ids[k6ZeroChunk];                     // store warp: the zero items of its current claim
@@ -329,6 +330,13 @@ __device__ __forceinline__ K6Item k6_describe(const K6Params& P, int X0, int Y0,
     return it;
 }
 
+// Item numbering: tile column fastest, then the tile row, then the channel group: neighbouring tiles and tile rows are
+// worked on at about the same time and share their halo rows in L2 (with the tile row outermost the call was 0.5 ms
+// slower).  The items of the LAST group are re-ordered heaviest first by chan_tail_sort_kernel.
+__device__ __forceinline__ void k6_item_decode(const K6Params& P, int item, int& tx, int& ty, int& grp) {
+    tx = item % P.ntx; ty = (item / P.ntx) % P.nty; grp = item / (P.ntx * P.nty);
+}
+
 // One warp walks the sorted rows of the item's bucket window (lane = candidate, 128 candidates' bounding boxes in
 // flight), tests them against the tile with integer compares and calls emit(hit, row, mask, ballot, popc(ballot)) for
 // every 32 candidates with at least one hit, in sorted-row order.  mask: bits 0..15 = the 4 x 4 blocks (4 x 2 cells)
@@ -414,7 +422,8 @@ chan_list_kernel(const __grid_constant__ K6Params P, int* __restrict__ list_cnt,
     const int n_items = (int)P.n_items;
     const unsigned lt_mask = (1u << lane) - 1u;
     for (int item = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; item < n_items; item += warps) {
-        const int tx = item % P.ntx, ty = (item / P.ntx) % P.nty, grp = item / (P.ntx * P.nty);
+        int tx, ty, grp;
+        k6_item_decode(P, item, tx, ty, grp);
         const double4 gi = P.group[grp];
         const K6Item it = k6_describe(P, tx * k6TileX, ty * k6TileY, grp, gi.z, gi.w);
         int cand = 0;
@@ -448,72 +457,138 @@ chan_list_kernel(const __grid_constant__ K6Params P, int* __restrict__ list_cnt,
 // order, so neighbouring tiles are still worked on at about the same time and share their halo rows in L2.
 // A block takes `per_block` consecutive items, publishes its number of items with hits in blk_state (zeroed by the
 // call's memset; flag bit 30) and sums the counts of the blocks before it (they were scheduled before it, so the wait
-// cannot deadlock) - a one-level decoupled scan, enough for the <= 2048 blocks the launcher uses.
-constexpr int k6OrderBlocksMax = 2048;
+// cannot deadlock) - a one-level decoupled scan, enough for the <= 1024 blocks the launcher uses.  The same scan runs over the hit counts: c_desc.w is the
+// number of hits of all items before this one, the work measure that paces the zero-fill.
+constexpr int k6OrderBlocksMax = 1024;                 // two state arrays of this length in d_misc (counts, hits)
 constexpr int k6OrderFlag = 1 << 30;
 
 __global__ void __launch_bounds__(1024)
 chan_order_kernel(const int* __restrict__ list_cnt, const unsigned* __restrict__ list_off, int n_items, int per_block,
-                  int4* __restrict__ c_desc, unsigned* __restrict__ z_list, int* __restrict__ n_cz, volatile int* blk_state,
-                  const int* __restrict__ dispatch, int dispatch_want) {
+                  int4* __restrict__ c_desc, unsigned* __restrict__ z_list, int* __restrict__ n_cz, int* __restrict__ n_hits,
+                  volatile int* blk_state, const int* __restrict__ dispatch, int dispatch_want) {
     if (dispatch != nullptr && *dispatch != dispatch_want) return;
-    __shared__ int s_warp[32];
-    __shared__ int s_prefix;
+    __shared__ int s_warp[32], s_hwarp[32];
+    __shared__ int s_prefix, s_hprefix;
     const unsigned full = 0xffffffffu;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int b = blockIdx.x;
     const int i0 = min(n_items, b * per_block), i1 = min(n_items, i0 + per_block);
-    int nz = 0;
-    for (int i = i0 + tid; i < i1; i += 1024) nz += list_cnt[i] != 0 ? 1 : 0;
+    volatile int* hit_state = blk_state + k6OrderBlocksMax;          // second scan: the hits of the items (the work measure)
+    // a swept item (-1: its list is unknown) counts as 64 hits in the work measure
+    int nz = 0, nh = 0;
+    for (int i = i0 + tid; i < i1; i += 1024) {
+        const int c = list_cnt[i];
+        nz += c != 0 ? 1 : 0;
+        nh += c < 0 ? 64 : c;
+    }
     nz = __reduce_add_sync(full, nz);
-    if (lane == 0) s_warp[warp] = nz;
+    nh = __reduce_add_sync(full, nh);
+    if (lane == 0) { s_warp[warp] = nz; s_hwarp[warp] = nh; }
     __syncthreads();
     if (warp == 0) {
-        const int total = __reduce_add_sync(full, s_warp[lane]);
-        if (lane == 0) blk_state[b] = total | k6OrderFlag;
-        int sum = 0;
+        const int total = __reduce_add_sync(full, s_warp[lane]), htotal = __reduce_add_sync(full, s_hwarp[lane]);
+        if (lane == 0) { blk_state[b] = total | k6OrderFlag; hit_state[b] = htotal | k6OrderFlag; }
+        int sum = 0, hsum = 0;
         for (int j0 = 0; j0 < b; j0 += 32) {
             const int j = j0 + lane;
-            int v = 0;
+            int v = 0, h = 0;
             if (j < b) {
                 do { v = blk_state[j]; } while (!(v & k6OrderFlag));
-                v &= ~k6OrderFlag;
+                do { h = hit_state[j]; } while (!(h & k6OrderFlag));
+                v &= ~k6OrderFlag; h &= ~k6OrderFlag;
             }
-            sum += v;
+            sum += v; hsum += h;
         }
         sum = __reduce_add_sync(full, sum);
+        hsum = __reduce_add_sync(full, hsum);
         if (lane == 0) {
-            s_prefix = sum;
-            if (b == (int)gridDim.x - 1) { n_cz[0] = sum + total; n_cz[1] = n_items - (sum + total); }
+            s_prefix = sum; s_hprefix = hsum;
+            if (b == (int)gridDim.x - 1) { n_cz[0] = sum + total; n_cz[1] = n_items - (sum + total); *n_hits = hsum + htotal; }
         }
     }
     __syncthreads();
-    int cb = s_prefix;                                               // items with hits before the current chunk
+    int cb = s_prefix, hb = s_hprefix;                               // items with hits / hits before the current chunk
     const unsigned lt_mask = (1u << lane) - 1u;
     for (int s0 = i0; s0 < i1; s0 += 1024) {
         const int i = s0 + tid;
         const bool valid = i < i1;
         const int cnt = valid ? list_cnt[i] : 0;
+        const int hits = cnt < 0 ? 64 : cnt;
         const unsigned bm = __ballot_sync(full, valid && cnt != 0);
-        __syncthreads();                                             // s_warp is free again
-        if (lane == 0) s_warp[warp] = __popc(bm);
-        __syncthreads();
-        const int t = s_warp[lane];
-        int incl = t;
+        int hincl = hits;                                            // inclusive scan of the hits inside the warp
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            const int u = __shfl_up_sync(full, incl, o);
-            if (lane >= o) incl += u;
+            const int u = __shfl_up_sync(full, hincl, o);
+            if (lane >= o) hincl += u;
+        }
+        __syncthreads();                                             // s_warp / s_hwarp are free again
+        if (lane == 0) s_warp[warp] = __popc(bm);
+        if (lane == 31) s_hwarp[warp] = hincl;
+        __syncthreads();
+        const int t = s_warp[lane], ht = s_hwarp[lane];
+        int incl = t, hinc2 = ht;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int u = __shfl_up_sync(full, incl, o), hu = __shfl_up_sync(full, hinc2, o);
+            if (lane >= o) { incl += u; hinc2 += hu; }
         }
         const int before = __shfl_sync(full, incl - t, warp);        // items with hits in the warps before this one
-        const int chunk_total = __shfl_sync(full, incl, 31);
+        const int hbefore = __shfl_sync(full, hinc2 - ht, warp);     // their hits
+        const int chunk_total = __shfl_sync(full, incl, 31), hchunk_total = __shfl_sync(full, hinc2, 31);
         if (valid) {
             const int cpos = cb + before + __popc(bm & lt_mask);     // items with hits before item i
-            if (cnt != 0) c_desc[cpos] = make_int4(i, cnt, (int)list_off[i], 0);
+            if (cnt != 0) c_desc[cpos] = make_int4(i, cnt, (int)list_off[i], hb + hbefore + hincl - hits);   // .w: hits before it
             else z_list[i - cpos] = (unsigned)i;
         }
         cb += chunk_total;
+        hb += hchunk_total;
     }
+}
+
+// Fourth pre-pass, one block: the items with hits of the LAST channel group - the tail of c_desc, which is in item order -
+// are sorted heaviest first (ties by item number: deterministic).  The dense centre tiles of a group take 0.1 - 0.2 ms
+// each and are claimed four at a time; in item order the last group's centre rows come 0.15 ms before the end of the
+// kernel and the SMs that claimed them finished 0.3 - 0.4 ms after all others (measured with per-CTA end times).  Heaviest
+// first, every SM starts the last group with dense items and the sparse ones fill the end evenly.
+constexpr int k6TailMax = 8192;                                      // entries sorted (128 KB of shared memory)
+
+__global__ void __launch_bounds__(1024)
+chan_tail_sort_kernel(int4* __restrict__ c_desc, const int* __restrict__ n_cz, int first_item_of_last_group,
+                      const int* __restrict__ dispatch, int dispatch_want) {
+    if (dispatch != nullptr && *dispatch != dispatch_want) return;
+    extern __shared__ int4 s_e[];
+    __shared__ int s_lo;
+    const int n_c = n_cz[0];
+    if (threadIdx.x == 0) {                                          // first entry of the last group (binary search on the item number)
+        int lo = 0, hi = n_c;
+        while (lo < hi) { const int mid = (lo + hi) >> 1; if (c_desc[mid].x < first_item_of_last_group) lo = mid + 1; else hi = mid; }
+        s_lo = max(lo, n_c - k6TailMax);
+    }
+    __syncthreads();
+    const int lo = s_lo, n = n_c - lo;
+    if (n < 2) return;
+    for (int i = threadIdx.x; i < n; i += 1024) s_e[i] = c_desc[lo + i];
+    __syncthreads();
+    // heavier first: a before b iff hits(a) > hits(b), or equal hits and the smaller item number (swept items, -1, last)
+    auto before = [](const int4& a, const int4& b) { return a.y > b.y || (a.y == b.y && a.x < b.x); };
+    for (int k = 2; (k >> 1) < n; k <<= 1) {                         // bitonic network, all-ascending form (k_bin.cu)
+        for (int i = threadIdx.x; i < n; i += 1024) {
+            const int j = i ^ (k - 1);
+            if (j > i && j < n) { const int4 x = s_e[i], y = s_e[j]; if (before(y, x)) { s_e[i] = y; s_e[j] = x; } }
+        }
+        __syncthreads();
+        for (int d = k >> 2; d > 0; d >>= 1) {
+            for (int i = threadIdx.x; i < n; i += 1024) {
+                const int j = i ^ d;
+                if (j > i && j < n) { const int4 x = s_e[i], y = s_e[j]; if (before(y, x)) { s_e[i] = y; s_e[j] = x; } }
+            }
+            __syncthreads();
+        }
+    }
+    // written back interleaved: the sweepers claim four consecutive entries at a time, so claim k gets the entries k,
+    // k + n/4, k + n/2, k + 3n/4 of the sorted order - one of the heaviest with three lighter ones, not the four heaviest
+    const int n4 = n & ~3, q = n4 >> 2;
+    for (int i = threadIdx.x; i < n; i += 1024) c_desc[lo + i] = s_e[i < n4 ? (i & 3) * q + (i >> 2) : i];
 }
 
 // ------------------------------------------------------------------------------------------------ main kernel
@@ -528,6 +603,13 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
         if (threadIdx.x == 0 && P.stats) atomicMax(P.stats, 100);
         return;
     }
+#ifdef K6_TRACE
+    if (threadIdx.x == 0) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        reinterpret_cast<unsigned long long*>(const_cast<uint2*>(P.lists) + 34000000)[512 + blockIdx.x] = t;
+    }
+#endif
     const K6Layout L = k6_layout(P.n_tu, P.n_tv);
     float* tu = reinterpret_cast<float*>(base + L.tu);
     float* tv = reinterpret_cast<float*>(base + L.tv);
@@ -702,6 +784,13 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 K6_TOC(t_wo, c3);
             }
         }
+#ifdef K6_TRACE
+        if (warp == 0 && lane == 0) {
+            unsigned long long t;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+            reinterpret_cast<unsigned long long*>(const_cast<uint2*>(P.lists) + 34000000)[256 + blockIdx.x] = t;
+        }
+#endif
         K6_ADD(0, t_full); K6_ADD(1, t_visit); K6_ADD(2, t_woe); K6_ADD(3, t_wo); K6_ADD(4, n_vis_cnt); K6_ADD(5, n_bat);
     } else {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
@@ -806,7 +895,8 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                     d4_n = load_desc(base_n);
                 }
                 const int item = __shfl_sync(full, d4.x, sub), c = __shfl_sync(full, d4.y, sub);
-                if (lane == 0) S.c_pos = ci;
+                const int hits_before = __shfl_sync(full, d4.w, sub);
+                if (lane == 0) S.c_hits = hits_before;
                 const unsigned off = (unsigned)__shfl_sync(full, d4.z, sub);
                 const int ci_n = sub == 3 ? base_n : ci + 1;
                 const bool valid_n = ci_n < n_c && ci_n >= 0;
@@ -816,7 +906,8 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 const int S_n = stride_of(c_n);
                 load_entries(off_n, c_n, S_n, 0, ea_n, eb_n);
                 // ---- this item
-                const int tx = item % P.ntx, ty = (item / P.ntx) % P.nty, grp = item / (P.ntx * P.nty);
+                int tx, ty, grp;
+        k6_item_decode(P, item, tx, ty, grp);
                 const int X0 = tx * k6TileX, Y0 = ty * k6TileY;
                 int cnt = 0;
                 if (c > 0) {
@@ -904,7 +995,7 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 S_cur = S_n;
                 ea = ea_n; eb = eb_n;
             }
-            if (lane == 0) S.c_pos = n_c;                    // nothing left to claim: the store warp may zero-fill at full speed
+            if (lane == 0) S.c_hits = 0x7fffffff;            // nothing left to claim: the store warp may zero-fill at full speed
             // exit: one flagged batch per stager (consumers stop at the first one), one flagged item for the store warp
             if (!*abort_flag) {
                 bool ok = true;
@@ -1051,8 +1142,8 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 // flight while this one is stored (one exposed L2 round trip per 16 items of ~3 us each)
                 const int n_z = __ldg(P.n_cz + 1);
                 int z_cur = -1, z_k = 0, z_n = 0, zX0 = 0, zY0 = 0, zc0 = 0, z_pos = 0;
-                const int n_c = __ldg(P.n_cz);
-                const long long z_lead = (long long)n_c * K6_ZERO_LEAD_PCT / 100 + 8;
+                const long long n_hits = max(__ldg(P.n_hits), 1);
+                const long long z_lead = n_hits * K6_ZERO_LEAD_PCT / 100 + 64;
                 int z_base_next = atomicAdd(P.zcounter, k6ZeroChunk);
                 int zb_cur = 0;
                 auto z_advance = [&]() {
@@ -1069,7 +1160,8 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                     }
                     z_pos = zb_cur + z_k;
                     z_cur = S.z_ids[z_k++];
-                    const int tx = z_cur % P.ntx, ty = (z_cur / P.ntx) % P.nty, grp = z_cur / (P.ntx * P.nty);
+                    int tx, ty, grp;
+                    k6_item_decode(P, z_cur, tx, ty, grp);
                     zX0 = tx * k6TileX; zY0 = ty * k6TileY; zc0 = grp * 32;
                 };
                 if (!P.accumulate) z_advance();                          // accumulate-into leaves the cells nothing reaches alone
@@ -1112,10 +1204,10 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                         }
                     }
                     // Zero-fill is paced by the progress of the consumer items (both lists are global and claimed in order): the
-                    // share of the zero list that is done stays within K6_ZERO_LEAD_PCT of the share of the consumer list the
-                    // sweeper has reached.  Unpaced, every SM zero-fills flat out at the start of the kernel and the write
+                    // share of the zero list that is done stays within K6_ZERO_LEAD_PCT of the share of all HITS that lie before
+                    // the item the sweeper is on (c_desc.w) - the work measure, so the zeros flow while the consumers are busy.  Unpaced, every SM zero-fills flat out at the start of the kernel and the write
                     // stream starves the visibility loads of the dense tiles (measured: 8.2 - 8.6 ms against 7.9).
-                    if (z_cur >= 0 && (long long)z_pos * n_c <= ((long long)S.c_pos + z_lead) * n_z) {
+                    if (z_cur >= 0 && (long long)z_pos * n_hits <= ((long long)S.c_hits + z_lead) * n_z) {
                         K6_TIC(s2);
                         // one box of [v 4][chan 32][16 cells] per look, and never more than K6_ZERO_INFLIGHT + 1 of them queued in
                         // the TMA engine: a consumer row that becomes ready must not wait behind a long run of zero boxes
@@ -1151,6 +1243,14 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
     }
     __syncthreads();
     if (tid == 0 && S.abort && P.stats) atomicMax(P.stats, S.abort);
+#ifdef K6_TRACE
+    // diagnostics build only: per-CTA end time and the time its consumers finished, in the unused tail of the list pool
+    if (tid == 0) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        reinterpret_cast<unsigned long long*>(const_cast<uint2*>(P.lists) + 34000000)[blockIdx.x] = t;
+    }
+#endif
 }
 
 // ------------------------------------------------------------------------------------------------ host side
@@ -1226,6 +1326,7 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
     P.c_desc = (const int4*)ws.d_c_desc;
     P.z_list = ws.d_z_list;
     P.n_cz = ws.d_misc + 14;
+    P.n_hits = ws.d_misc + 11;
     P.zcounter = ws.d_misc + 3;
     P.lists = (const uint2*)ws.d_lists;
     P.counter = ws.d_misc + 2;
@@ -1263,7 +1364,10 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
         int per_block = (int)(((P.n_items + k6OrderBlocksMax - 1) / k6OrderBlocksMax + 1023) / 1024) * 1024;
         const int oblocks = (int)((P.n_items + per_block - 1) / per_block);
         chan_order_kernel<<<oblocks, 1024, 0, st>>>(ws.d_list_cnt, ws.d_list_off, (int)P.n_items, per_block, (int4*)ws.d_c_desc,
-                                                    ws.d_z_list, ws.d_misc + 14, ws.d_misc + kMiscOrderState, dispatch, 1);
+                                                    ws.d_z_list, ws.d_misc + 14, ws.d_misc + 11, ws.d_misc + kMiscOrderState, dispatch, 1);
+        if (!cuda_ok(cudaFuncSetAttribute(chan_tail_sort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, k6TailMax * 16), "tail sort smem attribute"))
+            return false;
+        chan_tail_sort_kernel<<<1, 1024, k6TailMax * 16, st>>>((int4*)ws.d_c_desc, ws.d_misc + 14, (P.n_groups - 1) * P.ntx * P.nty, dispatch, 1);
     }
     const size_t smem = k6_layout(P.n_tu, P.n_tv).total;
     auto kern = w ? chanws_kernel<true> : chanws_kernel<false>;
@@ -1272,7 +1376,7 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
     long long blocks = p->sm_count;
     if (blocks > P.n_items) blocks = P.n_items;
     kern<<<(unsigned)blocks, k6Threads, smem, st>>>(P, map_out, map_zero, map_acc);
-    p->last_launches += 4;
+    p->last_launches += 5;
     return cuda_ok(cudaGetLastError(), "chanws_kernel");
 }
 
