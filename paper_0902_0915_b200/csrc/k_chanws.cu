@@ -465,7 +465,8 @@ constexpr int k6OrderFlag = 1 << 30;
 __global__ void __launch_bounds__(1024)
 chan_order_kernel(const int* __restrict__ list_cnt, const unsigned* __restrict__ list_off, int n_items, int per_block,
                   int4* __restrict__ c_desc, unsigned* __restrict__ z_list, int* __restrict__ n_cz, int* __restrict__ n_hits,
-                  volatile int* blk_state, const int* __restrict__ dispatch, int dispatch_want) {
+                  int first_item_of_last_group, int* __restrict__ tail_start, volatile int* blk_state,
+                  const int* __restrict__ dispatch, int dispatch_want) {
     if (dispatch != nullptr && *dispatch != dispatch_want) return;
     __shared__ int s_warp[32], s_hwarp[32];
     __shared__ int s_prefix, s_hprefix;
@@ -537,6 +538,7 @@ chan_order_kernel(const int* __restrict__ list_cnt, const unsigned* __restrict__
         const int chunk_total = __shfl_sync(full, incl, 31), hchunk_total = __shfl_sync(full, hinc2, 31);
         if (valid) {
             const int cpos = cb + before + __popc(bm & lt_mask);     // items with hits before item i
+            if (i == first_item_of_last_group) *tail_start = cpos;   // where the last channel group begins in c_desc
             if (cnt != 0) c_desc[cpos] = make_int4(i, cnt, (int)list_off[i], hb + hbefore + hincl - hits);   // .w: hits before it
             else z_list[i - cpos] = (unsigned)i;
         }
@@ -546,49 +548,49 @@ chan_order_kernel(const int* __restrict__ list_cnt, const unsigned* __restrict__
 }
 
 // Fourth pre-pass, one block: the items with hits of the LAST channel group - the tail of c_desc, which is in item order -
-// are sorted heaviest first (ties by item number: deterministic).  The dense centre tiles of a group take 0.1 - 0.2 ms
+// are sorted heaviest first (by weight class).  The dense centre tiles of a group take 0.1 - 0.2 ms
 // each and are claimed four at a time; in item order the last group's centre rows come 0.15 ms before the end of the
 // kernel and the SMs that claimed them finished 0.3 - 0.4 ms after all others (measured with per-CTA end times).  Heaviest
 // first, every SM starts the last group with dense items and the sparse ones fill the end evenly.
-constexpr int k6TailMax = 8192;                                      // entries sorted (128 KB of shared memory)
+constexpr int k6TailMax = 8192;                                      // entries sorted (128 KB of entries + 64 KB of keys in shared memory)
 
 __global__ void __launch_bounds__(1024)
-chan_tail_sort_kernel(int4* __restrict__ c_desc, const int* __restrict__ n_cz, int first_item_of_last_group,
+chan_tail_sort_kernel(int4* __restrict__ c_desc, const int* __restrict__ n_cz, const int* __restrict__ tail_start,
                       const int* __restrict__ dispatch, int dispatch_want) {
     if (dispatch != nullptr && *dispatch != dispatch_want) return;
-    extern __shared__ int4 s_e[];
-    __shared__ int s_lo;
+    extern __shared__ __align__(16) unsigned char s_raw[];
+    int4* s_e = reinterpret_cast<int4*>(s_raw);                                   // the entries, in item order
+    unsigned long long* s_k = reinterpret_cast<unsigned long long*>(s_raw + (size_t)k6TailMax * 16);   // sort keys
     const int n_c = n_cz[0];
-    if (threadIdx.x == 0) {                                          // first entry of the last group (binary search on the item number)
-        int lo = 0, hi = n_c;
-        while (lo < hi) { const int mid = (lo + hi) >> 1; if (c_desc[mid].x < first_item_of_last_group) lo = mid + 1; else hi = mid; }
-        s_lo = max(lo, n_c - k6TailMax);
-    }
-    __syncthreads();
-    const int lo = s_lo, n = n_c - lo;
+    const int lo = max(*tail_start, n_c - k6TailMax), n = n_c - lo;
     if (n < 2) return;
-    for (int i = threadIdx.x; i < n; i += 1024) s_e[i] = c_desc[lo + i];
+    // a counting sort by weight class (floor(log2 hits), heaviest class first; swept items, -1, in the lightest): within a
+    // factor of two of heaviest-first, which is all the balancing needs, and three passes instead of a 78-step network.
+    // The order inside a class is whatever the atomics give - the order of the ITEMS does not touch any grid value.
+    __shared__ int s_hist[32], s_cur[32];
+    if (threadIdx.x < 32) s_hist[threadIdx.x] = 0;
     __syncthreads();
-    // heavier first: a before b iff hits(a) > hits(b), or equal hits and the smaller item number (swept items, -1, last)
-    auto before = [](const int4& a, const int4& b) { return a.y > b.y || (a.y == b.y && a.x < b.x); };
-    for (int k = 2; (k >> 1) < n; k <<= 1) {                         // bitonic network, all-ascending form (k_bin.cu)
-        for (int i = threadIdx.x; i < n; i += 1024) {
-            const int j = i ^ (k - 1);
-            if (j > i && j < n) { const int4 x = s_e[i], y = s_e[j]; if (before(y, x)) { s_e[i] = y; s_e[j] = x; } }
-        }
-        __syncthreads();
-        for (int d = k >> 2; d > 0; d >>= 1) {
-            for (int i = threadIdx.x; i < n; i += 1024) {
-                const int j = i ^ d;
-                if (j > i && j < n) { const int4 x = s_e[i], y = s_e[j]; if (before(y, x)) { s_e[i] = y; s_e[j] = x; } }
-            }
-            __syncthreads();
-        }
+    for (int i = threadIdx.x; i < n; i += 1024) {
+        const int4 e = c_desc[lo + i];
+        s_e[i] = e;
+        atomicAdd(&s_hist[31 - __clz(max(e.y, 1))], 1);
     }
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        int start = 0;
+        for (int c = 31; c > (int)threadIdx.x; --c) start += s_hist[c];
+        s_cur[threadIdx.x] = start;
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < n; i += 1024) s_k[atomicAdd(&s_cur[31 - __clz(max(s_e[i].y, 1))], 1)] = (unsigned long long)i;
+    __syncthreads();
     // written back interleaved: the sweepers claim four consecutive entries at a time, so claim k gets the entries k,
     // k + n/4, k + n/2, k + 3n/4 of the sorted order - one of the heaviest with three lighter ones, not the four heaviest
     const int n4 = n & ~3, q = n4 >> 2;
-    for (int i = threadIdx.x; i < n; i += 1024) c_desc[lo + i] = s_e[i < n4 ? (i & 3) * q + (i >> 2) : i];
+    for (int i = threadIdx.x; i < n; i += 1024) {
+        const int src = i < n4 ? (i & 3) * q + (i >> 2) : i;
+        c_desc[lo + i] = s_e[(int)(s_k[src] & 0xffffffffu)];
+    }
 }
 
 // ------------------------------------------------------------------------------------------------ main kernel
@@ -1364,10 +1366,11 @@ bool launch_chanws(Plan* p, const float* vis, const float* w, long long n_vis, i
         int per_block = (int)(((P.n_items + k6OrderBlocksMax - 1) / k6OrderBlocksMax + 1023) / 1024) * 1024;
         const int oblocks = (int)((P.n_items + per_block - 1) / per_block);
         chan_order_kernel<<<oblocks, 1024, 0, st>>>(ws.d_list_cnt, ws.d_list_off, (int)P.n_items, per_block, (int4*)ws.d_c_desc,
-                                                    ws.d_z_list, ws.d_misc + 14, ws.d_misc + 11, ws.d_misc + kMiscOrderState, dispatch, 1);
-        if (!cuda_ok(cudaFuncSetAttribute(chan_tail_sort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, k6TailMax * 16), "tail sort smem attribute"))
+                                                    ws.d_z_list, ws.d_misc + 14, ws.d_misc + 11, (P.n_groups - 1) * P.ntx * P.nty, ws.d_misc + kMiscTailStart,
+                                                    ws.d_misc + kMiscOrderState, dispatch, 1);
+        if (!cuda_ok(cudaFuncSetAttribute(chan_tail_sort_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, k6TailMax * 24), "tail sort smem attribute"))
             return false;
-        chan_tail_sort_kernel<<<1, 1024, k6TailMax * 16, st>>>((int4*)ws.d_c_desc, ws.d_misc + 14, (P.n_groups - 1) * P.ntx * P.nty, dispatch, 1);
+        chan_tail_sort_kernel<<<1, 1024, k6TailMax * 24, st>>>((int4*)ws.d_c_desc, ws.d_misc + 14, ws.d_misc + kMiscTailStart, dispatch, 1);
     }
     const size_t smem = k6_layout(P.n_tu, P.n_tv).total;
     auto kern = w ? chanws_kernel<true> : chanws_kernel<false>;

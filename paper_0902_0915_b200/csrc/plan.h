@@ -14,6 +14,7 @@ constexpr int kChanMinChannels = 8; // AUTO picks a channel-SIMD kernel (K6 / K5
 constexpr int kTile = 16;           // gridding tile side in cells (one warp owns one tile of one channel)
 // d_misc (ints, zeroed by every call's binning step): [0..3] work counters, [4..11] diagnostics, [12..13] hit-list pool
 // cursor (u64), [14..15] K6 item counts, [16..] tile-weight histogram (4096), then the block states of chan_order_kernel
+constexpr int kMiscTailStart = 16 + 4080;    // [1] first entry of the last channel group in K6's list of items with hits
 constexpr int kMiscOrderState = 16 + 4096;
 constexpr int kMiscScanState = kMiscOrderState + 2048;   // block states of bin_scan_kernel (<= 1024 blocks: 4 M buckets)
 constexpr int kMiscBigList = kMiscScanState + 1024;    // [0] number of big buckets of bin_order_kernel, [1..1023] their ids
