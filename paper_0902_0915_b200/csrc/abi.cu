@@ -376,12 +376,6 @@ int mwa_grid_probe_smem_atomics(mwa_grid_plan* plan, double* out_rate, void* str
     return probe_smem_atomics(reinterpret_cast<Plan*>(plan), out_rate, reinterpret_cast<cudaStream_t>(stream)) ? MWA_GRID_OK : MWA_GRID_ERR_CUDA;
 }
 
-#ifdef K6_TRACE
-extern "C" int mwa_grid_debug_trace(mwa_grid_plan* plan, unsigned long long* out, int n) {   // diagnostics build only
-    Plan* p = reinterpret_cast<Plan*>(plan);
-    return cudaMemcpy(out, (const char*)p->ws.d_lists + (size_t)34000000 * 8, (size_t)n * 8, cudaMemcpyDeviceToHost) == cudaSuccess ? 0 : -3;
-}
-#endif
 
 int mwa_grid_plan_set_list_pool(mwa_grid_plan* plan, long long entries) {
     if (!plan || entries < 0) { set_error("bad argument"); return MWA_GRID_ERR_INVALID; }

@@ -605,13 +605,6 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
         if (threadIdx.x == 0 && P.stats) atomicMax(P.stats, 100);
         return;
     }
-#ifdef K6_TRACE
-    if (threadIdx.x == 0) {
-        unsigned long long t;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-        reinterpret_cast<unsigned long long*>(const_cast<uint2*>(P.lists) + 34000000)[512 + blockIdx.x] = t;
-    }
-#endif
     const K6Layout L = k6_layout(P.n_tu, P.n_tv);
     float* tu = reinterpret_cast<float*>(base + L.tu);
     float* tv = reinterpret_cast<float*>(base + L.tv);
@@ -786,13 +779,6 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
                 K6_TOC(t_wo, c3);
             }
         }
-#ifdef K6_TRACE
-        if (warp == 0 && lane == 0) {
-            unsigned long long t;
-            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-            reinterpret_cast<unsigned long long*>(const_cast<uint2*>(P.lists) + 34000000)[256 + blockIdx.x] = t;
-        }
-#endif
         K6_ADD(0, t_full); K6_ADD(1, t_visit); K6_ADD(2, t_woe); K6_ADD(3, t_wo); K6_ADD(4, n_vis_cnt); K6_ADD(5, n_bat);
     } else {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
@@ -1245,14 +1231,6 @@ chanws_kernel(const __grid_constant__ K6Params P, const __grid_constant__ CUtens
     }
     __syncthreads();
     if (tid == 0 && S.abort && P.stats) atomicMax(P.stats, S.abort);
-#ifdef K6_TRACE
-    // diagnostics build only: per-CTA end time and the time its consumers finished, in the unused tail of the list pool
-    if (tid == 0) {
-        unsigned long long t;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-        reinterpret_cast<unsigned long long*>(const_cast<uint2*>(P.lists) + 34000000)[blockIdx.x] = t;
-    }
-#endif
 }
 
 // ------------------------------------------------------------------------------------------------ host side
