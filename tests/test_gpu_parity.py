@@ -593,3 +593,26 @@ def test_multi_frequency_synthesis_sums_the_channels_onto_one_grid(lib, design):
         p.set_mfs(False)
         back = p.grid(g.uv, g.freqs, g.vis, g.weights)                      # and back to one grid per channel
         assert tuple(back.shape) == (12, 4, 250, 250)
+
+
+# ---------------------------------------------------------------------------- K6 stress: many shapes, repeated calls
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_chanws_random_shapes_repeated_calls(lib, seed):
+    """compute-sanitizer is not available on the GPU pool, so races in K6's mbarrier pipeline are hunted by repetition: random
+    grid sizes (ragged edges), antenna counts (sparse to dense tiles) and channel counts (ragged last group, many
+    groups), each gridded three times on one plan - bit-identical every time and within tolerance of the oracle."""
+    rs = np.random.RandomState(100 + seed)
+    for _ in range(4):
+        n_ant = int(rs.choice([12, 40, 90, 180]))
+        kw = dict(n_ant=n_ant, core_ant=n_ant // 2, n_chan=int(rs.choice([8, 31, 32, 45, 96, 130])),
+                  grid_n=int(rs.choice([64, 96, 250, 256, 384])))
+        g = generate(_fine(kw))
+        G, A, _ = _oracle(g)
+        _to_dev(g)
+        with _plan(lib, g, "chanws") as p:
+            first = p.grid(g.uv, g.freqs, g.vis, g.weights).clone()
+            for k in range(2):
+                again = p.grid(g.uv, g.freqs, g.vis, g.weights)
+                assert torch.equal(first.view(torch.float32), again.view(torch.float32)), (kw, k)
+            assert lib.mwa_grid_plan_last_stats(p.handle)["error"] == 0
+        assert_parity(first.cpu().numpy(), G, A, f"K6 stress {kw}")
