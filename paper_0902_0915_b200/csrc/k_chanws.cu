@@ -335,6 +335,15 @@ __device__ __forceinline__ K6Item k6_describe(const K6Params& P, int X0, int Y0,
 // slower).  The items of the LAST group are re-ordered heaviest first by chan_tail_sort_kernel.
 __device__ __forceinline__ void k6_item_decode(const K6Params& P, int item, int& tx, int& ty, int& grp) {
     tx = item % P.ntx; ty = (item / P.ntx) % P.nty; grp = item / (P.ntx * P.nty);
+#ifndef K6_NO_TX_INTERLEAVE
+    // The four items of a claim run one after the other on one SM; horizontally adjacent tiles share halo rows, which L2
+    // keeps for tens of microseconds only.  Within a tile row the columns are therefore taken in the order 0, 4, 8, ...,
+    // 1, 5, 9, ...: neighbouring tiles go to different SMs at about the same time.
+    if ((P.ntx & 3) == 0 && P.ntx >= 16) {
+        const int q = P.ntx >> 2;
+        tx = (tx % q) * 4 + tx / q;
+    }
+#endif
 }
 
 // One warp walks the sorted rows of the item's bucket window (lane = candidate, 128 candidates' bounding boxes in
