@@ -94,6 +94,14 @@ int mwa_grid_visibilities_host(mwa_grid_plan* plan, const double* uv_f64, const 
 int mwa_grid_compute_indices(mwa_grid_plan* plan, const double* uv_f64, const double* freqs,
                              long long n_vis, int n_chan, int* out_idx, void* stream);
 
+/* Companion weights grid: wgrid_out[c][y][x] = sum over the samples of channel c of
+ * T[rv][tv] * T[ru][tu] * w - the gridded sampling density (what imaging weights and the normalisation of a dirty image are
+ * derived from); it equals the real part of the XX grid of unit visibilities.
+ *   wgrid_out [n_chan][N][N] float, DEVICE, overwritten; weights [n_vis][n_chan] or NULL = ones; other arguments as in
+ *   mwa_grid_visibilities.  A by-product, written in scatter form (memset + one red.global.add.f32 per tap).  Asynchronous. */
+int mwa_grid_weights_grid(mwa_grid_plan* plan, const double* uv_f64, const double* freqs, const float* weights, long long n_vis,
+                          int n_chan, float* wgrid_out, void* stream);
+
 /* Dropped-sample counter: the number of (row, channel) samples mwa_grid_visibilities would
  * drop for these coordinates (R11: a tap outside the grid, |x| >= N/2, or a non-finite coordinate), counted with the same
  * index function.  out_count is a HOST pointer.  Synchronous (it reads the count back). */

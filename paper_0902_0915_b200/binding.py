@@ -32,6 +32,8 @@ _lib.mwa_grid_visibilities_host.argtypes = [_P, _P, _P, _P, _P, _LL, _I, _P, _P]
 _lib.mwa_grid_visibilities_host.restype = _I
 _lib.mwa_grid_compute_indices.argtypes = [_P, _P, _P, _LL, _I, _P, _P]
 _lib.mwa_grid_compute_indices.restype = _I
+_lib.mwa_grid_weights_grid.argtypes = [_P, _P, _P, _P, _LL, _I, _P, _P]
+_lib.mwa_grid_weights_grid.restype = _I
 _lib.mwa_grid_count_dropped.argtypes = [_P, _P, _P, _LL, _I, _P, _P]
 _lib.mwa_grid_count_dropped.restype = _I
 _lib.mwa_grid_plan_set_mfs.argtypes = [_P, _I]
@@ -68,7 +70,7 @@ _lib.mwa_grid_last_error.restype = ctypes.c_char_p
 EXPORTS = ["mwa_grid_plan_create", "mwa_grid_plan_destroy", "mwa_grid_visibilities", "mwa_grid_visibilities_host",
            "mwa_grid_compute_indices", "mwa_grid_plan_set_design", "mwa_grid_plan_set_profiling",
            "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_plan_last_design", "mwa_grid_plan_last_stats", "mwa_grid_plan_set_list_pool", "mwa_grid_probe_fp32", "mwa_grid_last_error",
-           "mwa_image_from_grid", "mwa_image_correction", "mwa_image_stokes", "mwa_grid_probe_smem_atomics", "mwa_grid_count_dropped", "mwa_grid_plan_set_accumulate", "mwa_grid_plan_set_mfs"]
+           "mwa_image_from_grid", "mwa_image_correction", "mwa_image_stokes", "mwa_grid_probe_smem_atomics", "mwa_grid_count_dropped", "mwa_grid_plan_set_accumulate", "mwa_grid_plan_set_mfs", "mwa_grid_weights_grid"]
 
 
 class MwaGridError(RuntimeError):
@@ -149,6 +151,13 @@ def mwa_grid_compute_indices(plan, uv_f64, freqs, n_vis, n_chan, out_idx, stream
     _check(_lib.mwa_grid_compute_indices(plan, _ptr(uv_f64, torch.float64, "cuda", "uv_f64"),
                                          _ptr(freqs, torch.float64, "cuda", "freqs"), int(n_vis), int(n_chan),
                                          _ptr(out_idx, torch.int32, "cuda", "out_idx"), _stream_ptr(stream)))
+
+
+def mwa_grid_weights_grid(plan, uv_f64, freqs, weights, n_vis, n_chan, wgrid_out, stream=None) -> None:
+    """f3: companion weights grid, float32 [n_chan, N, N] = sum of tap * weight per cell."""
+    _check(_lib.mwa_grid_weights_grid(plan, _ptr(uv_f64, torch.float64, "cuda", "uv_f64"), _ptr(freqs, torch.float64, "cuda", "freqs"),
+                                      _ptr(weights, torch.float32, "cuda", "weights"), int(n_vis), int(n_chan),
+                                      _ptr(wgrid_out, torch.float32, "cuda", "wgrid_out"), _stream_ptr(stream)))
 
 
 def mwa_grid_count_dropped(plan, uv_f64, freqs, n_vis, n_chan, stream=None) -> int:

@@ -428,6 +428,22 @@ int mwa_grid_compute_indices(mwa_grid_plan* plan, const double* uv_f64, const do
     return MWA_GRID_OK;
 }
 
+int mwa_grid_weights_grid(mwa_grid_plan* plan, const double* uv_f64, const double* freqs, const float* weights, long long n_vis,
+                          int n_chan, float* wgrid_out, void* stream) {
+    g_last_error.clear();
+    Plan* p = reinterpret_cast<Plan*>(plan);
+    int rc = check_common(p, uv_f64, freqs, n_vis, n_chan);
+    if (rc != MWA_GRID_OK) return rc;
+    if (n_chan == 0) { p->last_launches = 0; return MWA_GRID_OK; }
+    if (!wgrid_out || !aligned(wgrid_out, 4) || !aligned(weights, 4)) { set_error("wgrid_out must be non-NULL; wgrid_out and weights 4-byte aligned"); return MWA_GRID_ERR_INVALID; }
+    rc = ensure_workspace(p, n_vis, n_chan);
+    if (rc != MWA_GRID_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+    p->last_launches = 0;
+    if (!launch_scale(p, freqs, n_chan, st)) return MWA_GRID_ERR_CUDA;
+    return launch_weights_grid(p, uv_f64, weights, n_vis, n_chan, wgrid_out, st) ? MWA_GRID_OK : MWA_GRID_ERR_CUDA;
+}
+
 int mwa_grid_count_dropped(mwa_grid_plan* plan, const double* uv_f64, const double* freqs, long long n_vis, int n_chan,
                            long long* out_count, void* stream) {
     g_last_error.clear();

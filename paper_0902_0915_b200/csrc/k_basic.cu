@@ -90,6 +90,43 @@ __global__ void indices_kernel(GridGeom g, const double2* __restrict__ uv, const
     }
 }
 
+// ---------------------------------------------------------------- companion weights grid
+// wgrid[c][y][x] = sum over samples of T[rv][tv] T[ru][tu] w  - the gridded sampling density that imaging weights and the
+// normalisation of a dirty image are derived from; equal to the real part of the XX grid of unit visibilities.  One thread
+// per (sample, tap row), one red.global.add.f32 per tap (K0's scatter form: this grid is a by-product, not the hot path).
+__global__ void weights_grid_kernel(GridGeom g, const double2* __restrict__ uv, const double* __restrict__ scale,
+                                    const float* __restrict__ weights, const float* __restrict__ table, long long n_vis,
+                                    int n_chan, float* __restrict__ wgrid) {
+    const long long total = n_vis * (long long)n_chan * g.W;
+    const size_t plane = (size_t)g.N * g.N;
+    for (long long k = blockIdx.x * (long long)blockDim.x + threadIdx.x; k < total; k += (long long)gridDim.x * blockDim.x) {
+        const long long sample = k / g.W;
+        const int tv = (int)(k - sample * g.W);
+        const long long n = sample / n_chan;
+        const int c = (int)(sample - n * n_chan);
+        const double2 p = uv[n];
+        SampleIndex s;
+        if (!sample_index(p.x, p.y, scale[c], g, s)) continue;
+        const float wt = weights ? weights[sample] : 1.0f;
+        const float kv = table[s.rv * g.W + tv] * wt;
+        float* base = wgrid + (size_t)c * plane + (size_t)(s.iv + tv - g.h) * g.N + (size_t)(s.iu - g.h);
+        for (int tu = 0; tu < g.W; ++tu) atomicAdd(base + tu, kv * table[s.ru * g.W + tu]);
+    }
+}
+
+bool launch_weights_grid(Plan* p, const double* uv, const float* w, long long n_vis, int n_chan, float* wgrid, cudaStream_t st) {
+    const size_t bytes = (size_t)n_chan * p->geom.N * p->geom.N * 4;
+    if (!cuda_ok(cudaMemsetAsync(wgrid, 0, bytes, st), "memset weights grid")) return false;
+    p->last_launches += 1;
+    const long long total = n_vis * (long long)n_chan * p->geom.W;
+    if (total == 0) return true;
+    long long blocks = (total + 255) / 256;
+    if (blocks > (long long)p->sm_count * 32) blocks = (long long)p->sm_count * 32;
+    weights_grid_kernel<<<(unsigned)blocks, 256, 0, st>>>(p->geom, (const double2*)uv, p->ws.d_scale, w, p->d_table, n_vis, n_chan, wgrid);
+    p->last_launches += 1;
+    return cuda_ok(cudaGetLastError(), "weights_grid_kernel");
+}
+
 // ---------------------------------------------------------------- dropped-sample counter
 __global__ void count_dropped_kernel(GridGeom g, const double2* __restrict__ uv, const double* __restrict__ scale, long long n_vis,
                                      int n_chan, unsigned long long* __restrict__ count) {

@@ -88,6 +88,7 @@ bool cuda_ok(cudaError_t e, const char* what);
 
 // launchers (each returns false after set_error on failure and adds its launches to plan->last_launches)
 bool launch_scale(Plan* p, const double* freqs, int n_chan, cudaStream_t st);
+bool launch_weights_grid(Plan* p, const double* uv, const float* w, long long n_vis, int n_chan, float* wgrid, cudaStream_t st);
 bool launch_count_dropped(Plan* p, const double* uv, long long n_vis, int n_chan, unsigned long long* d_count, cudaStream_t st);
 bool launch_indices(Plan* p, const double* uv, long long n_vis, int n_chan, int* out_idx, cudaStream_t st);
 bool launch_atomic(Plan* p, const double* uv, const float* vis, const float* w, long long n_vis, int n_chan,

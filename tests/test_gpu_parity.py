@@ -616,3 +616,24 @@ def test_chanws_random_shapes_repeated_calls(lib, seed):
                 assert torch.equal(first.view(torch.float32), again.view(torch.float32)), (kw, k)
             assert lib.mwa_grid_plan_last_stats(p.handle)["error"] == 0
         assert_parity(first.cpu().numpy(), G, A, f"K6 stress {kw}")
+
+
+# ---------------------------------------------------------------------------- f3: companion weights grid
+def test_weights_grid_equals_the_grid_of_unit_visibilities(lib):
+    g = generate(scaled(CONFIGS["C5"], n_ant=24, core_ant=12, n_chan=3, grid_n=250))        # random weights, W = 15
+    ones = np.ones((g.cfg.n_vis, g.cfg.n_chan, 4), dtype=np.complex64)
+    G, A, _ = oracle.grid(g.uv, g.freqs, ones, g.weights, g.cfg.grid_n, g.cell_du, g.cfg.support_W, g.cfg.oversample_O,
+                          g.kernel_table)
+    _to_dev(g)
+    with _plan(lib, g) as p:
+        wg = torch.full((g.cfg.n_chan, 250, 250), float("nan"), dtype=torch.float32, device="cuda")
+        lib.mwa_grid_weights_grid(p.handle, g.uv, g.freqs, g.weights, g.cfg.n_vis, g.cfg.n_chan, wg)
+        got = wg.cpu().numpy().astype(np.float64)
+        wg1 = torch.empty_like(wg)
+        lib.mwa_grid_weights_grid(p.handle, g.uv, g.freqs, None, g.cfg.n_vis, g.cfg.n_chan, wg1)   # NULL weights = ones
+    want, bound = G[:, 0].real, 1e-5 * A[:, 0] + 1e-7                    # the XX plane of the unit-visibility grid
+    assert np.all(np.abs(got - want) <= bound), float(np.max(np.abs(got - want) / bound))
+    assert np.count_nonzero(got[A[:, 0] == 0]) == 0
+    G1, A1, _ = oracle.grid(g.uv.cpu(), g.freqs.cpu(), ones, None, g.cfg.grid_n, g.cell_du, g.cfg.support_W, g.cfg.oversample_O,
+                            g.kernel_table)
+    assert np.all(np.abs(wg1.cpu().numpy() - G1[:, 0].real) <= 1e-5 * A1[:, 0] + 1e-7)
