@@ -45,6 +45,8 @@ def _load():
         lib.oracle_grid.argtypes = [P, P, P, P, ctypes.c_longlong, ctypes.c_int, ctypes.c_int,
                                     ctypes.c_double, ctypes.c_int, ctypes.c_int, P, P, P, ctypes.c_int]
         lib.oracle_grid.restype = ctypes.c_int
+        lib.oracle_grid_2d.argtypes = lib.oracle_grid.argtypes
+        lib.oracle_grid_2d.restype = ctypes.c_int
         _lib = lib
     return _lib
 
@@ -93,4 +95,30 @@ def grid(uv, freqs, vis, weights, grid_n, cell_du, support_W, oversample_O, kern
     used = _load().oracle_grid(uv.ctypes.data, freqs.ctypes.data, vis.ctypes.data, w_ptr, n_vis, n_chan,
                                grid_n, float(cell_du), support_W, oversample_O, table.ctypes.data,
                                G.ctypes.data, A.ctypes.data if want_abs else None, n_threads)
+    return G, A, used
+
+
+def grid_2d(uv, freqs, vis, weights, grid_n, cell_du, support_W, oversample_O, kernel_table_2d,
+            want_abs: bool = True, n_threads: int = 0):
+    """Gridding with a general 2-D complex kernel table [O+1, O+1, W, W] complex64 ([rv][ru][tv][tu]); SURVEY.md 8(f)-3.
+    Returns (G complex128 [n_chan,4,N,N], A float64 or None, threads)."""
+    uv, freqs = _np(uv, np.float64), _np(freqs, np.float64)
+    vis = _np(vis, np.complex64)
+    n_vis, n_chan = uv.shape[0], freqs.shape[0]
+    assert vis.shape == (n_vis, n_chan, 4), vis.shape
+    w_ptr = None
+    if weights is not None:
+        weights = _np(weights, np.float32)
+        assert weights.shape == (n_vis, n_chan)
+        w_ptr = weights.ctypes.data
+    table = _np(kernel_table_2d, np.complex64)
+    O1 = oversample_O + 1
+    assert table.shape == (O1, O1, support_W, support_W), table.shape
+    G = np.empty((n_chan, 4, grid_n, grid_n), dtype=np.complex128)
+    A = np.empty((n_chan, 4, grid_n, grid_n), dtype=np.float64) if want_abs else None
+    if n_threads <= 0:
+        n_threads = os.cpu_count() or 1
+    used = _load().oracle_grid_2d(uv.ctypes.data, freqs.ctypes.data, vis.ctypes.data, w_ptr, n_vis, n_chan,
+                                  grid_n, float(cell_du), support_W, oversample_O, table.ctypes.data,
+                                  G.ctypes.data, A.ctypes.data if want_abs else None, n_threads)
     return G, A, used

@@ -119,3 +119,50 @@ int oracle_grid(const double *uv, const double *freqs, const float *vis, const f
     }
     return n_threads;
 }
+
+/* The same gridder for a general 2-D COMPLEX kernel table ("general 2-D / complex kernel tables
+ * [O+1][O+1][W][W] (w-projection-style, 4 FMA per tap)"):
+ *     G[c][p][iv+tv-h][iu+tu-h] += K[rv][ru][tv][tu] * (w * V_p)          (complex * complex, fp64)
+ *     A[c][p][..]               += |K[rv][ru][tv][tu]| * |w| * |V_p|
+ * table2d [(O+1)][(O+1)][W][W][2] f32 (re, im), indexed [rv][ru][tv][tu]; everything else as oracle_grid (same index
+ * function, same drop rule R11, same layouts).  A separable real table K = T[rv][tv] * T[ru][tu] gives oracle_grid. */
+int oracle_grid_2d(const double *uv, const double *freqs, const float *vis, const float *weights,
+                   long long n_vis, int n_chan, int N, double cell_du, int W, int O, const float *table2d,
+                   double *G, double *A, int n_threads)
+{
+    int h = (W - 1) / 2, O1 = O + 1;
+    double inv_du = 1.0 / cell_du;
+    size_t plane = (size_t)N * N;
+    if (n_threads < 1) n_threads = 1;
+    if (n_threads > n_chan) n_threads = n_chan > 0 ? n_chan : 1;
+#pragma omp parallel for num_threads(n_threads) schedule(dynamic, 1)
+    for (int c = 0; c < n_chan; ++c) {
+        double *Gc = G + (size_t)c * 4 * plane * 2;
+        double *Ac = A ? A + (size_t)c * 4 * plane : NULL;
+        for (size_t k = 0; k < 4 * plane * 2; ++k) Gc[k] = 0.0;
+        if (Ac) for (size_t k = 0; k < 4 * plane; ++k) Ac[k] = 0.0;
+        double s = freqs[c] / ORACLE_C_LIGHT;
+        for (long long n = 0; n < n_vis; ++n) {
+            int id[4];
+            if (!sample_index(uv[2 * n], uv[2 * n + 1], s, inv_du, N, W, O, id)) continue;
+            int iu = id[0], iv = id[1], ru = id[2], rv = id[3];
+            const float *v = vis + ((size_t)n * n_chan + c) * 8;
+            double wt = weights ? (double)weights[(size_t)n * n_chan + c] : 1.0;
+            const float *K = table2d + (((size_t)rv * O1 + ru) * W * W) * 2;
+            for (int tv = 0; tv < W; ++tv) {
+                size_t row = (size_t)(iv + tv - h) * N;
+                for (int tu = 0; tu < W; ++tu) {
+                    double kr = (double)K[(tv * W + tu) * 2], ki = (double)K[(tv * W + tu) * 2 + 1];
+                    size_t cell = row + (size_t)(iu + tu - h);
+                    for (int p = 0; p < 4; ++p) {
+                        double zr = wt * (double)v[2 * p], zi = wt * (double)v[2 * p + 1];
+                        Gc[(p * plane + cell) * 2] += kr * zr - ki * zi;
+                        Gc[(p * plane + cell) * 2 + 1] += kr * zi + ki * zr;
+                        if (Ac) Ac[p * plane + cell] += hypot(kr, ki) * fabs(wt) * hypot((double)v[2 * p], (double)v[2 * p + 1]);
+                    }
+                }
+            }
+        }
+    }
+    return n_threads;
+}

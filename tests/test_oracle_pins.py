@@ -247,3 +247,41 @@ def test_stokes_oracle_against_the_textbook_definitions():
     q, p = 3, 11
     M = stokes_matrix_field(N).astype(np.complex128)
     assert np.allclose(imaging.stokes(measured, M)[1, :, q, p], M[q, p] @ measured[1, :, q, p])
+
+
+# ------------------------------------------------------------------ f3: general 2-D complex kernel tables
+def _table_2d(T, phase=None):
+    """[rv][ru][tv][tu] complex64 from the separable table T[(O+1)][W] (optionally times a per-tap phase screen)."""
+    K = (T[:, None, :, None].astype(np.float64) * T[None, :, None, :].astype(np.float64)).astype(np.complex128)
+    if phase is not None:
+        K = K * np.exp(1j * phase)
+    return K.astype(np.complex64)
+
+
+def test_oracle_2d_tables_against_the_pinned_separable_gridder():
+    N, W, O = 64, 7, 8
+    T = make_kernel_table(W, O)
+    rs = np.random.RandomState(8)
+    n_vis, n_chan = 300, 2
+    fr = np.array([299792458.0, 1.1 * 299792458.0])
+    uv = rs.uniform(-24, 24, (n_vis, 2))
+    vis = (rs.standard_normal((n_vis, n_chan, 4)) + 1j * rs.standard_normal((n_vis, n_chan, 4))).astype(np.complex64)
+    wts = rs.uniform(0.5, 1.5, (n_vis, n_chan)).astype(np.float32)
+    G1, A1, _ = oracle.grid(uv, fr, vis, wts, N, 1.0, W, O, T)
+    # (1) a separable real table reproduces the 1-D gridder (up to the fp32 rounding of the stored products)
+    G2, A2, _ = oracle.grid_2d(uv, fr, vis, wts, N, 1.0, W, O, _table_2d(T))
+    assert np.all(np.abs(G2 - G1) <= 2e-7 * A1 + 1e-12) and np.allclose(A2, A1, rtol=2e-7)
+    # (2) a constant phase factor on the kernel rotates the whole grid; (3) linearity in V
+    G3, _, _ = oracle.grid_2d(uv, fr, vis, wts, N, 1.0, W, O, _table_2d(T, phase=0.7))
+    assert np.all(np.abs(G3 - np.exp(0.7j) * G1) <= 4e-7 * A1 + 1e-12)
+    G4, _, _ = oracle.grid_2d(uv, fr, (2 * vis).astype(np.complex64), wts, N, 1.0, W, O, _table_2d(T, phase=0.7))
+    assert np.allclose(G4, 2 * G3, rtol=1e-12, atol=1e-14)
+    # (4) one visibility stamps the [rv][ru] slice of a NON-separable complex table, tv along rows and tu along columns
+    K = (rs.standard_normal((O + 1, O + 1, W, W)) + 1j * rs.standard_normal((O + 1, O + 1, W, W))).astype(np.complex64)
+    uv1 = np.array([[10.0625, -10.25]])                              # pin P1: (iu, ru) = (42, 5), (iv, rv) = (22, 2) at N = 64
+    v1 = np.zeros((1, 1, 4), dtype=np.complex64); v1[0, 0] = [1, 2j, -3, 0.5 - 0.25j]
+    G5, A5, _ = oracle.grid_2d(uv1, fr[:1], v1, None, N, 1.0, W, O, K)
+    h = 3
+    for p in range(4):
+        assert np.allclose(G5[0, p, 22 - h:22 + h + 1, 42 - h:42 + h + 1], K[2, 5].astype(np.complex128) * complex(v1[0, 0, p]), rtol=1e-15)
+    assert np.count_nonzero(G5[0, 0]) == W * W and np.allclose(A5[0, 1, 22 - h:22 + h + 1, 42 - h:42 + h + 1], 2 * np.abs(K[2, 5]))
