@@ -59,6 +59,15 @@ enum {
 mwa_grid_plan* mwa_grid_plan_create(int grid_n, double cell_du, int support_W, int oversample_O,
                                     const float* kernel_table);
 
+/* f3 - a plan with a general 2-D COMPLEX kernel table (w-projection-style kernels, 4 FMA per tap):
+ *   grid[c][p][iv+tv-h][iu+tu-h] += K[rv][ru][tv][tu] * w[n][c] * V[n][c][p]          (complex * complex, fp32 accumulate)
+ *   kernel_table_2d  HOST pointer, (O+1)*(O+1)*W*W*2 floats, [rv][ru][tv][tu] (re, im); copied.  oversample_O <= 62.
+ * Index function, drop rule and all layouts are those of mwa_grid_plan_create / mwa_grid_visibilities.  Such a plan grids
+ * with one tile-owned register kernel (csrc/k_gather2d.cu; designs AUTO / GATHER) and does not take accumulate-into, MFS,
+ * the imaging calls or the weights grid (they are defined for separable tables).  Returns NULL on failure. */
+mwa_grid_plan* mwa_grid_plan_create_2d(int grid_n, double cell_du, int support_W, int oversample_O,
+                                       const float* kernel_table_2d);
+
 /* Grid one visibility set (hot path: SURVEY.md section 8(a) rows a1-a5).
  *   uv_f64   [n_vis][2]            double, metres (u_m, v_m)                 16-byte aligned
  *   freqs    [n_chan]              double, Hz

@@ -24,6 +24,8 @@ _P, _I, _LL, _D = ctypes.c_void_p, ctypes.c_int, ctypes.c_longlong, ctypes.c_dou
 
 _lib.mwa_grid_plan_create.argtypes = [_I, _D, _I, _I, _P]
 _lib.mwa_grid_plan_create.restype = _P
+_lib.mwa_grid_plan_create_2d.argtypes = [_I, _D, _I, _I, _P]
+_lib.mwa_grid_plan_create_2d.restype = _P
 _lib.mwa_grid_plan_destroy.argtypes = [_P]
 _lib.mwa_grid_plan_destroy.restype = None
 _lib.mwa_grid_visibilities.argtypes = [_P, _P, _P, _P, _P, _LL, _I, _P, _P]
@@ -70,7 +72,7 @@ _lib.mwa_grid_last_error.restype = ctypes.c_char_p
 EXPORTS = ["mwa_grid_plan_create", "mwa_grid_plan_destroy", "mwa_grid_visibilities", "mwa_grid_visibilities_host",
            "mwa_grid_compute_indices", "mwa_grid_plan_set_design", "mwa_grid_plan_set_profiling",
            "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_plan_last_design", "mwa_grid_plan_last_stats", "mwa_grid_plan_set_list_pool", "mwa_grid_probe_fp32", "mwa_grid_last_error",
-           "mwa_image_from_grid", "mwa_image_correction", "mwa_image_stokes", "mwa_grid_probe_smem_atomics", "mwa_grid_count_dropped", "mwa_grid_plan_set_accumulate", "mwa_grid_plan_set_mfs", "mwa_grid_weights_grid"]
+           "mwa_image_from_grid", "mwa_image_correction", "mwa_image_stokes", "mwa_grid_probe_smem_atomics", "mwa_grid_count_dropped", "mwa_grid_plan_set_accumulate", "mwa_grid_plan_set_mfs", "mwa_grid_weights_grid", "mwa_grid_plan_create_2d"]
 
 
 class MwaGridError(RuntimeError):
@@ -115,6 +117,17 @@ def mwa_grid_plan_create(grid_n: int, cell_du: float, support_W: int, oversample
     if tab.numel() != (int(oversample_O) + 1) * int(support_W):
         raise ValueError("kernel_table must hold (O+1)*W floats")
     h = _lib.mwa_grid_plan_create(int(grid_n), float(cell_du), int(support_W), int(oversample_O), tab.data_ptr())
+    if not h:
+        raise MwaGridError(-1, mwa_grid_last_error())
+    return h
+
+
+def mwa_grid_plan_create_2d(grid_n: int, cell_du: float, support_W: int, oversample_O: int, kernel_table_2d) -> int:
+    """kernel_table_2d: CPU complex64 tensor / array of shape [O+1, O+1, W, W] ([rv][ru][tv][tu]).  Returns the plan handle."""
+    tab = torch.as_tensor(kernel_table_2d, dtype=torch.complex64, device="cpu").contiguous()
+    if tuple(tab.shape) != (int(oversample_O) + 1, int(oversample_O) + 1, int(support_W), int(support_W)):
+        raise ValueError("kernel_table_2d must be complex64 [O+1, O+1, W, W]")
+    h = _lib.mwa_grid_plan_create_2d(int(grid_n), float(cell_du), int(support_W), int(oversample_O), tab.data_ptr())
     if not h:
         raise MwaGridError(-1, mwa_grid_last_error())
     return h
@@ -254,10 +267,11 @@ def mwa_grid_probe_fp32(plan, stream=None):
 class Plan:
     """Owns a plan handle; `grid()` allocates the output on the inputs' device and calls the ABI."""
 
-    def __init__(self, grid_n, cell_du, support_W, oversample_O, kernel_table, design="auto"):
+    def __init__(self, grid_n, cell_du, support_W, oversample_O, kernel_table, design="auto", table_2d=False):
         self.grid_n, self.support_W, self.oversample_O = int(grid_n), int(support_W), int(oversample_O)
         self.mfs = False
-        self.handle = mwa_grid_plan_create(grid_n, cell_du, support_W, oversample_O, kernel_table)
+        create = mwa_grid_plan_create_2d if table_2d else mwa_grid_plan_create
+        self.handle = create(grid_n, cell_du, support_W, oversample_O, kernel_table)
         if design != "auto":
             mwa_grid_plan_set_design(self.handle, design)
 

@@ -177,6 +177,13 @@ static int grid_device(Plan* p, const double* uv, const double* freqs, const flo
             set_error("accumulate-into is implemented by the designs AUTO, GATHER, CHANWS, ATOMIC and ROMEIN only");
             return MWA_GRID_ERR_INVALID;
         }
+        if (p->d_table2d) {                           // plans of mwa_grid_plan_create_2d: one kernel (k_gather2d.cu)
+            if ((design != MWA_GRID_DESIGN_AUTO && design != MWA_GRID_DESIGN_GATHER) || p->accumulate || p->mfs) {
+                set_error("a plan with a 2-D kernel table grids with the design AUTO / GATHER only, without accumulate-into or MFS");
+                return MWA_GRID_ERR_INVALID;
+            }
+            ok = launch_gather2d(p, vis, weights, n_vis, n_chan, grid, st);
+        } else
         switch (design) {
             case MWA_GRID_DESIGN_ATOMIC: ok = launch_atomic(p, uv, vis, weights, n_vis, n_chan, grid, st); break;
             case MWA_GRID_DESIGN_SMEM: ok = launch_smem(p, vis, weights, n_vis, n_chan, grid, st); break;
@@ -220,13 +227,14 @@ extern "C" {
 
 const char* mwa_grid_last_error(void) { return g_last_error.c_str(); }
 
-mwa_grid_plan* mwa_grid_plan_create(int grid_n, double cell_du, int support_W, int oversample_O,
-                                    const float* kernel_table) {
+static mwa_grid_plan* plan_create_common(int grid_n, double cell_du, int support_W, int oversample_O, const float* kernel_table,
+                                         bool two_d) {
     g_last_error.clear();
     if (grid_n < 16 || grid_n > 16384 || (grid_n & 1)) { set_error("grid_n must be even and in [16, 16384]"); return nullptr; }
     if (support_W < 1 || support_W > 15 || !(support_W & 1)) { set_error("support_W must be odd and in [1, 15]"); return nullptr; }
     if (grid_n < 2 * support_W) { set_error("grid_n must be >= 2 * support_W"); return nullptr; }
     if (oversample_O < 2 || oversample_O > 64 || (oversample_O & 1)) { set_error("oversample_O must be even and in [2, 64]"); return nullptr; }
+    if (two_d && oversample_O > 62) { set_error("2-D tables: oversample_O must be <= 62"); return nullptr; }
     if (!(cell_du > 0.0) || !std::isfinite(cell_du)) { set_error("cell_du must be finite and > 0"); return nullptr; }
     if (!kernel_table) { set_error("kernel_table is NULL"); return nullptr; }
     Plan* p = new (std::nothrow) Plan();
@@ -240,25 +248,39 @@ mwa_grid_plan* mwa_grid_plan_create(int grid_n, double cell_du, int support_W, i
         if ((1 << k) == oversample_O) p->geom.o_shift = k;
     p->geom.inv_du = 1.0 / cell_du;
     p->cell_du = cell_du;
-    const size_t n = (size_t)(oversample_O + 1) * support_W;
-    p->h_table = new (std::nothrow) float[n];
-    if (!p->h_table) { set_error("out of host memory"); delete p; return nullptr; }
-    std::memcpy(p->h_table, kernel_table, n * sizeof(float));
+    const size_t O1 = (size_t)oversample_O + 1;
+    const size_t n = two_d ? O1 * O1 * support_W * support_W * 2 : O1 * support_W;
+    float** d_dst = two_d ? &p->d_table2d : &p->d_table;
+    if (!two_d) {
+        p->h_table = new (std::nothrow) float[n];
+        if (!p->h_table) { set_error("out of host memory"); delete p; return nullptr; }
+        std::memcpy(p->h_table, kernel_table, n * sizeof(float));
+    }
     if (!cuda_ok(cudaGetDevice(&p->device), "cudaGetDevice") ||
         !cuda_ok(cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, p->device), "sm count") ||
-        !cuda_ok(cudaMalloc((void**)&p->d_table, n * sizeof(float)), "cudaMalloc table") ||
-        !cuda_ok(cudaMemcpy(p->d_table, kernel_table, n * sizeof(float), cudaMemcpyHostToDevice), "copy table")) {
+        !cuda_ok(cudaMalloc((void**)d_dst, n * sizeof(float)), "cudaMalloc table") ||
+        !cuda_ok(cudaMemcpy(*d_dst, kernel_table, n * sizeof(float), cudaMemcpyHostToDevice), "copy table")) {
         mwa_grid_plan_destroy(reinterpret_cast<mwa_grid_plan*>(p));
         return nullptr;
     }
     return reinterpret_cast<mwa_grid_plan*>(p);
 }
 
+mwa_grid_plan* mwa_grid_plan_create(int grid_n, double cell_du, int support_W, int oversample_O,
+                                    const float* kernel_table) {
+    return plan_create_common(grid_n, cell_du, support_W, oversample_O, kernel_table, false);
+}
+
+mwa_grid_plan* mwa_grid_plan_create_2d(int grid_n, double cell_du, int support_W, int oversample_O,
+                                       const float* kernel_table_2d) {
+    return plan_create_common(grid_n, cell_du, support_W, oversample_O, kernel_table_2d, true);
+}
+
 void mwa_grid_plan_destroy(mwa_grid_plan* plan) {
     if (!plan) return;
     Plan* p = reinterpret_cast<Plan*>(plan);
     Workspace& ws = p->ws;
-    void* ptrs[] = {p->d_table, ws.d_scale, ws.d_group, ws.d_scale_ref, ws.d_bucket_count, ws.d_bucket_cursor, ws.d_perm, ws.d_perm_tmp,
+    void* ptrs[] = {p->d_table, p->d_table2d, ws.d_scale, ws.d_group, ws.d_scale_ref, ws.d_bucket_count, ws.d_bucket_cursor, ws.d_perm, ws.d_perm_tmp,
                     ws.d_uv_sorted, ws.d_row_sorted, ws.d_tile_order, ws.d_tile_weight, ws.d_misc, ws.d_dispatch, ws.d_stage,
                     ws.d_pre, ws.d_bb, ws.d_list_cnt, ws.d_list_off, ws.d_c_desc, ws.d_z_list, ws.d_lists};
     for (void* q : ptrs)
@@ -276,6 +298,7 @@ int mwa_image_from_grid(mwa_grid_plan* plan, const float* grid, float* image, lo
     g_last_error.clear();
     Plan* p = reinterpret_cast<Plan*>(plan);
     if (!p) { set_error("plan is NULL"); return MWA_GRID_ERR_INVALID; }
+    if (!p->d_table) { set_error("the convolution correction is defined for separable 1-D tables only"); return MWA_GRID_ERR_INVALID; }
     if (n_planes < 0) { set_error("n_planes must be >= 0"); return MWA_GRID_ERR_INVALID; }
     p->last_launches = 0;
     if (n_planes == 0) return MWA_GRID_OK;
@@ -317,6 +340,7 @@ int mwa_image_correction(mwa_grid_plan* plan, double* out_corr, int n) {
     g_last_error.clear();
     Plan* p = reinterpret_cast<Plan*>(plan);
     if (!p || !out_corr || n < 0) { set_error("bad argument"); return MWA_GRID_ERR_INVALID; }
+    if (!p->d_table) { set_error("the convolution correction is defined for separable 1-D tables only"); return MWA_GRID_ERR_INVALID; }
     const double* c = image_correction_host(p, nullptr);
     if (!c) return MWA_GRID_ERR_CUDA;
     const int k = n < p->geom.N ? n : p->geom.N;
@@ -435,6 +459,7 @@ int mwa_grid_weights_grid(mwa_grid_plan* plan, const double* uv_f64, const doubl
     int rc = check_common(p, uv_f64, freqs, n_vis, n_chan);
     if (rc != MWA_GRID_OK) return rc;
     if (n_chan == 0) { p->last_launches = 0; return MWA_GRID_OK; }
+    if (!p->d_table) { set_error("the weights grid is implemented for separable 1-D tables only"); return MWA_GRID_ERR_INVALID; }
     if (!wgrid_out || !aligned(wgrid_out, 4) || !aligned(weights, 4)) { set_error("wgrid_out must be non-NULL; wgrid_out and weights 4-byte aligned"); return MWA_GRID_ERR_INVALID; }
     rc = ensure_workspace(p, n_vis, n_chan);
     if (rc != MWA_GRID_OK) return rc;

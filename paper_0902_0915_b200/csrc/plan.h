@@ -62,6 +62,7 @@ struct Plan {
     double cell_du = 0.0;
     float* d_table = nullptr;        // [(O+1)][W] as given
     float* h_table = nullptr;        // host copy
+    float* d_table2d = nullptr;      // f3: general 2-D complex table [(O+1)][(O+1)][W][W][2] (plans of mwa_grid_plan_create_2d), else null
     int design = 0;
     int device = 0;
     int sm_count = 148;
@@ -111,6 +112,7 @@ bool launch_image(Plan* p, const float* grid, float* image, long long n_planes, 
 const double* image_correction_host(Plan* p, cudaStream_t st);
 bool launch_stokes(Plan* p, const float* image, const float* matrix, float* out, int n_chan, cudaStream_t st);
 void image_release(Plan* p);
+bool launch_gather2d(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid, cudaStream_t st);
 bool launch_romein(Plan* p, const double* uv, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                    const int* perm, cudaStream_t st);
 

@@ -637,3 +637,30 @@ def test_weights_grid_equals_the_grid_of_unit_visibilities(lib):
     G1, A1, _ = oracle.grid(g.uv.cpu(), g.freqs.cpu(), ones, None, g.cfg.grid_n, g.cell_du, g.cfg.support_W, g.cfg.oversample_O,
                             g.kernel_table)
     assert np.all(np.abs(wg1.cpu().numpy() - G1[:, 0].real) <= 1e-5 * A1[:, 0] + 1e-7)
+
+
+# ---------------------------------------------------------------------------- f3: general 2-D complex kernel tables
+@pytest.mark.parametrize("name,kw", [
+    ("C2", dict(n_ant=48, n_chan=5, grid_n=250)),                          # W = 7, O = 8, ragged grid edge
+    ("C5", dict(n_ant=20, core_ant=10, n_chan=2, grid_n=256)),             # W = 15, O = 16, random weights
+])
+def test_2d_complex_kernel_table(lib, name, kw):
+    g = generate(scaled(CONFIGS[name], **kw))
+    cfg = g.cfg
+    W, O = cfg.support_W, cfg.oversample_O
+    rs = np.random.RandomState(13)
+    T = g.kernel_table.numpy().astype(np.float64)
+    # a non-separable complex kernel: the separable one times a tap- and row-dependent phase screen, plus a small random part
+    K = T[:, None, :, None] * T[None, :, None, :] * np.exp(1j * rs.uniform(-1.5, 1.5, (O + 1, O + 1, W, W)))
+    K = (K + 0.01 * (rs.standard_normal(K.shape) + 1j * rs.standard_normal(K.shape)) * np.abs(K).max()).astype(np.complex64)
+    G, A, _ = oracle.grid_2d(g.uv, g.freqs, g.vis, g.weights, cfg.grid_n, g.cell_du, W, O, K)
+    _to_dev(g)
+    with lib.Plan(cfg.grid_n, g.cell_du, W, O, K, table_2d=True) as p:
+        out = p.grid(g.uv, g.freqs, g.vis, g.weights)
+        again = p.grid(g.uv, g.freqs, g.vis, g.weights)
+        assert torch.equal(out.view(torch.float32), again.view(torch.float32))
+        assert_parity(out.cpu().numpy(), G, A, f"2-D table {name}")
+        idx = p.indices(g.uv, g.freqs).cpu().numpy()                        # the same index function
+        with pytest.raises(lib.MwaGridError):
+            p.image(out)
+    assert np.array_equal(idx, oracle.compute_indices(g.uv.cpu(), g.freqs.cpu(), cfg.grid_n, g.cell_du, W, O))
