@@ -98,6 +98,32 @@ int mwa_grid_visibilities_host(mwa_grid_plan* plan, const double* uv_f64, const 
                                const float* vis_c64, const float* weights, long long n_vis, int n_chan,
                                float* grid_out, void* stream);
 
+/* The gridding call for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): no plan, and no cudaMalloc / cudaFree / allocating library routine inside, on any call.
+ * It runs the GATHER design (K3c: scale, binning, tile-owned register gridder - the kernels of the plan path) with the
+ * binning workspace in a static device array of the library (csrc/k_noalloc.cu: about 7.6 MB of every GPU that loads
+ * the library, held until exit), which fixes the maximum sizes of a call: */
+#define MWA_GRID_NOALLOC_MAX_VIS 131072    /* rows per call (C4's 130,816 baselines fit)          */
+#define MWA_GRID_NOALLOC_MAX_CHAN 1024     /* channels per call                                   */
+#define MWA_GRID_NOALLOC_MAX_GRID_N 2048   /* grid cells per side                                 */
+/* A call beyond any of them returns MWA_GRID_ERR_INVALID with a message naming the limit; nothing is enqueued.
+ *   grid_n, cell_du, support_W, oversample_O   as in mwa_grid_plan_create (and grid_n <= the limit above)
+ *   kernel_table_dev  DEVICE pointer, (O+1)*W floats, row-major [ru][t] as in mwa_grid_plan_create; read by the
+ *                     kernels, not copied: it is the caller's and must stay valid until the stream reaches the end of
+ *                     the call
+ *   all other arguments: layouts, alignment, drop rule, finite-input contract and asynchrony of mwa_grid_visibilities;
+ *   grid_out is overwritten entirely.
+ * Values: those of a plan with MWA_GRID_DESIGN_GATHER, bit for bit (same kernels, same order of summation).
+ * The first call on a device resolves the array's device address (cudaGetSymbolAddress) and loads the kernels: make it
+ * before any region that forbids such set-up.  ALL calls on a device share the one array, which keeps the contents of
+ * the call before (each call clears what it needs zeroed): calls that overlap on the GPU - two streams without an
+ * ordering between them, two host threads - race on it and give wrong grids; order them on one stream or with events.
+ * The current device must be the one the pointers live on.  Errors: MWA_GRID_ERR_INVALID / MWA_GRID_ERR_CUDA. */
+int mwa_grid_visibilities_noalloc(int grid_n, double cell_du, int support_W, int oversample_O,
+                                  const float* kernel_table_dev, const double* uv_f64, const double* freqs,
+                                  const float* vis_c64, const float* weights, long long n_vis, int n_chan,
+                                  float* grid_out, void* stream);
+
 /* Test hook for "indices bit-exact": runs the SAME __device__ index function the gridders use.
  *   out_idx [n_vis][n_chan][4] int32 = (iu, iv, ru, rv), or (-1,-1,-1,-1) for a dropped sample. */
 int mwa_grid_compute_indices(mwa_grid_plan* plan, const double* uv_f64, const double* freqs,

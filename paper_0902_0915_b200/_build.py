@@ -5,7 +5,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmwa_grid.so")
-SOURCES = ["abi.cu", "k_basic.cu", "k_bin.cu", "k_gather.cu", "k_chan.cu", "k_chanws.cu", "k_smem.cu", "k_romein.cu", "k_image.cu", "k_probe.cu", "k_gather2d.cu"]
+SOURCES = ["abi.cu", "k_basic.cu", "k_bin.cu", "k_gather.cu", "k_chan.cu", "k_chanws.cu", "k_smem.cu", "k_romein.cu", "k_image.cu", "k_probe.cu", "k_gather2d.cu", "k_noalloc.cu"]
 HEADERS = ["plan.h", "index.cuh", os.path.join("..", "..", "include", "mwa_grid.h")]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-ldl"]

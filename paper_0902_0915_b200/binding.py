@@ -32,6 +32,8 @@ _lib.mwa_grid_visibilities.argtypes = [_P, _P, _P, _P, _P, _LL, _I, _P, _P]
 _lib.mwa_grid_visibilities.restype = _I
 _lib.mwa_grid_visibilities_host.argtypes = [_P, _P, _P, _P, _P, _LL, _I, _P, _P]
 _lib.mwa_grid_visibilities_host.restype = _I
+_lib.mwa_grid_visibilities_noalloc.argtypes = [_I, _D, _I, _I, _P, _P, _P, _P, _P, _LL, _I, _P, _P]
+_lib.mwa_grid_visibilities_noalloc.restype = _I
 _lib.mwa_grid_compute_indices.argtypes = [_P, _P, _P, _LL, _I, _P, _P]
 _lib.mwa_grid_compute_indices.restype = _I
 _lib.mwa_grid_weights_grid.argtypes = [_P, _P, _P, _P, _LL, _I, _P, _P]
@@ -72,7 +74,8 @@ _lib.mwa_grid_last_error.restype = ctypes.c_char_p
 EXPORTS = ["mwa_grid_plan_create", "mwa_grid_plan_destroy", "mwa_grid_visibilities", "mwa_grid_visibilities_host",
            "mwa_grid_compute_indices", "mwa_grid_plan_set_design", "mwa_grid_plan_set_profiling",
            "mwa_grid_plan_stage_ms", "mwa_grid_plan_last_launches", "mwa_grid_plan_last_design", "mwa_grid_plan_last_stats", "mwa_grid_plan_set_list_pool", "mwa_grid_probe_fp32", "mwa_grid_last_error",
-           "mwa_image_from_grid", "mwa_image_correction", "mwa_image_stokes", "mwa_grid_probe_smem_atomics", "mwa_grid_count_dropped", "mwa_grid_plan_set_accumulate", "mwa_grid_plan_set_mfs", "mwa_grid_weights_grid", "mwa_grid_plan_create_2d"]
+           "mwa_image_from_grid", "mwa_image_correction", "mwa_image_stokes", "mwa_grid_probe_smem_atomics", "mwa_grid_count_dropped", "mwa_grid_plan_set_accumulate", "mwa_grid_plan_set_mfs", "mwa_grid_weights_grid", "mwa_grid_plan_create_2d",
+           "mwa_grid_visibilities_noalloc"]
 
 
 class MwaGridError(RuntimeError):
@@ -157,6 +160,26 @@ def mwa_grid_visibilities_host(plan, uv_f64, freqs, vis_c64, weights, n_vis, n_c
                                            _ptr(weights, torch.float32, "cpu", "weights"),
                                            int(n_vis), int(n_chan), _ptr(grid_out, torch.complex64, "cpu", "grid_out"),
                                            _stream_ptr(stream)))
+
+
+NOALLOC_MAX_VIS, NOALLOC_MAX_CHAN, NOALLOC_MAX_GRID_N = 131072, 1024, 2048      # MWA_GRID_NOALLOC_MAX_* of the header
+
+
+def mwa_grid_visibilities_noalloc(grid_n, cell_du, support_W, oversample_O, kernel_table_dev, uv_f64, freqs, vis_c64, weights,
+                                  n_vis, n_chan, grid_out, stream=None) -> None:
+    """The gridding call that allocates nothing (no plan; GATHER design on a static device scratch array of the library).
+    kernel_table_dev: DEVICE float32 [O+1, W]; the other tensors as in mwa_grid_visibilities.  Limits: NOALLOC_MAX_*.
+    Calls that overlap on the GPU race on the shared scratch.  Asynchronous."""
+    if kernel_table_dev is not None and kernel_table_dev.numel() != (int(oversample_O) + 1) * int(support_W):
+        raise ValueError("kernel_table_dev must hold (O+1)*W floats")
+    _check(_lib.mwa_grid_visibilities_noalloc(int(grid_n), float(cell_du), int(support_W), int(oversample_O),
+                                              _ptr(kernel_table_dev, torch.float32, "cuda", "kernel_table_dev"),
+                                              _ptr(uv_f64, torch.float64, "cuda", "uv_f64"),
+                                              _ptr(freqs, torch.float64, "cuda", "freqs"),
+                                              _ptr(vis_c64, torch.complex64, "cuda", "vis_c64"),
+                                              _ptr(weights, torch.float32, "cuda", "weights"),
+                                              int(n_vis), int(n_chan), _ptr(grid_out, torch.complex64, "cuda", "grid_out"),
+                                              _stream_ptr(stream)))
 
 
 def mwa_grid_compute_indices(plan, uv_f64, freqs, n_vis, n_chan, out_idx, stream=None) -> None:
