@@ -139,6 +139,7 @@ static int check_common(Plan* p, const double* uv, const double* freqs, long lon
 static int grid_device(Plan* p, const double* uv, const double* freqs, const float* vis, const float* weights,
                        long long n_vis, int n_chan, float* grid, cudaStream_t st) {
     p->last_launches = 0;
+    p->pdl_next = false;
     if (n_chan == 0) return MWA_GRID_OK;
     int dev = -1;
     if (!cuda_ok(cudaGetDevice(&dev), "cudaGetDevice")) return MWA_GRID_ERR_CUDA;
@@ -155,10 +156,21 @@ static int grid_device(Plan* p, const double* uv, const double* freqs, const flo
             if (!e && !cuda_ok(cudaEventCreate(&e), "cudaEventCreate")) return MWA_GRID_ERR_CUDA;
         cudaEventRecord(p->ev[0], st);
     }
-    if (!launch_scale(p, freqs, n_chan, st)) return MWA_GRID_ERR_CUDA;
     const int design = p->design;
-    if (design != MWA_GRID_DESIGN_ATOMIC && design != MWA_GRID_DESIGN_ROMEIN && n_vis > 0)
-        if (!launch_binning(p, uv, n_vis, n_chan, st)) return MWA_GRID_ERR_CUDA;
+    const bool bins = design != MWA_GRID_DESIGN_ATOMIC && design != MWA_GRID_DESIGN_ROMEIN && n_vis > 0;
+    if (bins && binning_is_small(p, n_vis)) {              // launch-bound calls: a1 + a3 in one launch
+        if (!launch_small_prepass(p, uv, freqs, n_vis, n_chan, st)) return MWA_GRID_ERR_CUDA;
+        // only a gather kernel that DIRECTLY follows the pre-pass may be launched as its programmatic dependent
+        const bool direct = !prof && !p->d_table2d && (design == MWA_GRID_DESIGN_GATHER ||
+                                                      (design == MWA_GRID_DESIGN_AUTO && (n_chan < kChanMinChannels || p->mfs)));
+        p->pdl_next = direct && !(p->mfs && !p->accumulate);     // MFS puts a memset between the two
+#ifdef MWA_NO_PDL
+        p->pdl_next = false;                                     // A/B measurement build only
+#endif
+    } else {
+        if (!launch_scale(p, freqs, n_chan, st)) return MWA_GRID_ERR_CUDA;
+        if (bins && !launch_binning(p, uv, n_vis, n_chan, st)) return MWA_GRID_ERR_CUDA;
+    }
     if (prof) cudaEventRecord(p->ev[1], st);
     bool ok = false;
     const int out_chan = p->mfs ? 1 : n_chan;              // grids the call writes

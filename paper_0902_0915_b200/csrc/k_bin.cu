@@ -6,6 +6,7 @@
 // that overlap it, and decides membership with the exact index function; the buckets only have to be
 // conservative.  n_vis items are sorted, not n_vis * n_chan.
 #include "plan.h"
+#include "scale.cuh"
 
 namespace mwa {
 
@@ -220,12 +221,16 @@ __global__ void tile_order_scatter_kernel(const int* __restrict__ weight, int n_
 // histogram, scan, scatter, ascending row order inside every bucket, tile weights and the heaviest-first tile order - and
 // writes the same arrays (bucket_start, perm, uv_sorted, row_sorted, tile_weight, tile_order) with the same contents,
 // except that equal-weight tiles are ordered by index here (the multi-kernel path orders them as its atomics fall).
+// With freqs != null the block first does a1 (scale.cuh) and clears the call's counters itself: the whole pre-pass of a
+// small call is then ONE launch instead of scale_kernel + memset + this kernel (launch_small_prepass).
 constexpr int kSmallRows = 4096, kSmallBuckets = 2048, kSmallTiles = 1024;   // 36 KB of static shared memory
 
 __global__ void __launch_bounds__(1024)
 bin_small_kernel(GridGeom g, const double2* __restrict__ uv, const double* __restrict__ s_ref_p, int n_vis, int nb, int nt,
                  int* __restrict__ bucket_start, int* __restrict__ perm, double2* __restrict__ uv_sorted,
-                 double4* __restrict__ row_sorted, int* __restrict__ tile_weight, int* __restrict__ tile_order) {
+                 double4* __restrict__ row_sorted, int* __restrict__ tile_weight, int* __restrict__ tile_order,
+                 const double* __restrict__ freqs, int n_chan, int chan_ok, double* __restrict__ scale,
+                 double* __restrict__ scale_ref, int* __restrict__ dispatch, double4* __restrict__ group, int* __restrict__ misc) {
     __shared__ int s_start[kSmallBuckets + 1];      // counts, then exclusive starts
     __shared__ int s_cursor[kSmallBuckets];
     __shared__ unsigned short s_tmp[kSmallRows];    // rows in bucket order, arbitrary inside a bucket
@@ -234,7 +239,16 @@ bin_small_kernel(GridGeom g, const double2* __restrict__ uv, const double* __res
     __shared__ int s_tw[kSmallTiles];
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int n_buckets = nb * nb, n_tiles = nt * nt;
-    const double s_ref = *s_ref_p;
+    double s_ref;
+    if (freqs != nullptr) {                         // fused pre-pass: a1 and the memset of the counters
+        // a gridder launched with programmatic stream serialisation may start its prologue now (it waits for this grid's
+        // completion before it reads anything written here); without such a launch the instruction does nothing
+        asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+        s_ref = scale_block(freqs, n_chan, g.N / 2, chan_ok, scale, scale_ref, dispatch, group);
+        for (int k = tid; k < kMiscInts; k += 1024) misc[k] = 0;
+    } else {
+        s_ref = *s_ref_p;
+    }
     for (int b = tid; b <= n_buckets; b += 1024) s_start[b] = 0;
     __syncthreads();
     for (int n = tid; n < n_vis; n += 1024) {
@@ -314,6 +328,24 @@ bin_small_kernel(GridGeom g, const double2* __restrict__ uv, const double* __res
     }
 }
 
+bool binning_is_small(const Plan* p, long long n_vis) {
+    const int nb = (p->geom.N + kBucketCells - 1) / kBucketCells, nt = (p->geom.N + kTile - 1) / kTile;
+    return n_vis > 0 && n_vis <= kSmallRows && nb * nb <= kSmallBuckets && nt * nt <= kSmallTiles;
+}
+
+// a1 + a3 of a small call (binning_is_small) in one launch; writes what launch_scale + launch_binning write
+bool launch_small_prepass(Plan* p, const double* uv, const double* freqs, long long n_vis, int n_chan, cudaStream_t st) {
+    Workspace& ws = p->ws;
+    const int nb = (p->geom.N + kBucketCells - 1) / kBucketCells, nt = (p->geom.N + kTile - 1) / kTile;
+    bin_small_kernel<<<1, 1024, 0, st>>>(p->geom, (const double2*)uv, nullptr, (int)n_vis, nb, nt, ws.d_bucket_count, ws.d_perm,
+                                         ws.d_uv_sorted, (double4*)ws.d_row_sorted, ws.d_tile_weight, ws.d_tile_order, freqs, n_chan,
+                                         (chan_supported(p, n_chan) || chanws_supported(p, n_chan)) ? 1 : 0, ws.d_scale, ws.d_scale_ref,
+                                         ws.d_dispatch, (double4*)ws.d_group, ws.d_misc);
+    p->last_launches += 1;
+    p->pdl_next = true;
+    return cuda_ok(cudaGetLastError(), "bin_small_kernel (fused pre-pass)");
+}
+
 bool launch_binning(Plan* p, const double* uv, long long n_vis, int /*n_chan*/, cudaStream_t st) {
     Workspace& ws = p->ws;
     const int nb = (p->geom.N + kBucketCells - 1) / kBucketCells;
@@ -322,7 +354,8 @@ bool launch_binning(Plan* p, const double* uv, long long n_vis, int /*n_chan*/, 
     if (!cuda_ok(cudaMemsetAsync(ws.d_misc, 0, (size_t)kMiscInts * sizeof(int), st), "memset misc")) return false;
     if (n_vis <= kSmallRows && n_buckets <= kSmallBuckets && nt * nt <= kSmallTiles) {
         bin_small_kernel<<<1, 1024, 0, st>>>(p->geom, (const double2*)uv, ws.d_scale_ref, (int)n_vis, nb, nt, ws.d_bucket_count,
-                                             ws.d_perm, ws.d_uv_sorted, (double4*)ws.d_row_sorted, ws.d_tile_weight, ws.d_tile_order);
+                                             ws.d_perm, ws.d_uv_sorted, (double4*)ws.d_row_sorted, ws.d_tile_weight, ws.d_tile_order,
+                                             nullptr, 0, 0, nullptr, nullptr, nullptr, nullptr, nullptr);
         p->last_launches += 2;
         return cuda_ok(cudaGetLastError(), "bin_small_kernel");
     }

@@ -55,6 +55,9 @@ struct GatherParams {
     int mfs;                    // 1: all channels add into ONE grid [4][N][N] (f3 multi-frequency synthesis): the write-out of a
                                 //    (tile, channel) item is a reduction (red.global.add.v4.f32) into the zero-filled shared grid
     int chunk;                  // consecutive work items per claim (1..8; amortises the round trip of the work counter)
+    int pdl;                    // 1: launched with programmatic stream serialisation behind the fused pre-pass of a small call
+                                //    (bin_small_kernel): the table copies are built while the pre-pass still runs, and
+                                //    griddepcontrol.wait comes before the first read of anything the pre-pass writes
 };
 
 typedef unsigned long long u64;
@@ -98,7 +101,7 @@ constexpr int kBiasU = 16, kBiasV = 16;   // floats; keep the stored offsets non
 
 __global__ void __launch_bounds__(kWarpsPerCta * 32, 4)
 gather_kernel(const GatherParams P) {
-    if (P.dispatch != nullptr && *P.dispatch != 0) return;
+    if (!P.pdl && P.dispatch != nullptr && *P.dispatch != 0) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const GridGeom g = P.g;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -121,6 +124,10 @@ gather_kernel(const GatherParams P) {
         tv[k] = (t >= 0 && t < g.W) ? P.table[r * g.W + t] : 0.0f;
     }
     __syncthreads();
+    if (P.pdl) {                                             // the pre-pass has completed and its writes are visible from here on
+        asm volatile("griddepcontrol.wait;" ::: "memory");
+        if (P.dispatch != nullptr && *P.dispatch != 0) return;
+    }
 
     const int bx = lane & 3, by = lane >> 2;
     const unsigned tu_s = (unsigned)__cvta_generic_to_shared(tu);
@@ -490,6 +497,22 @@ bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, i
     // items per claim: up to 8 while every warp still gets at least ~16 claims (small problems keep 1)
     long long chunk = P.n_items / (blocks * kWarpsPerCta * 16);
     P.chunk = (int)(chunk < 1 ? 1 : chunk > 8 ? 8 : chunk);
+    P.pdl = p->pdl_next ? 1 : 0;
+    p->pdl_next = false;
+    if (P.pdl) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)blocks);
+        cfg.blockDim = dim3(kWarpsPerCta * 32);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        p->last_launches += 1;
+        return cuda_ok(cudaLaunchKernelEx(&cfg, gather_kernel, P), "gather_kernel (dependent launch)");
+    }
     gather_kernel<<<(unsigned)blocks, kWarpsPerCta * 32, smem, st>>>(P);
     p->last_launches += 1;
     return cuda_ok(cudaGetLastError(), "gather_kernel");

@@ -82,6 +82,8 @@ struct Plan {
     bool accumulate = false;         // f3: grid_out += instead of = (mwa_grid_plan_set_accumulate)
     long long pool_limit = 0;        // diagnostics: cap on K6's hit-list pool in entries (0 = default sizing)
     bool last_chanws = false;        // AUTO: the channel-SIMD kernel enqueued by the last call was K6 (else K5)
+    bool pdl_next = false;           // the kernel enqueued last was the fused pre-pass of a small call (it releases its dependents
+                                     // at once): launch_gather, if it comes next, launches with programmatic stream serialisation
 };
 
 void set_error(const std::string& msg);
@@ -95,6 +97,8 @@ bool launch_indices(Plan* p, const double* uv, long long n_vis, int n_chan, int*
 bool launch_atomic(Plan* p, const double* uv, const float* vis, const float* w, long long n_vis, int n_chan,
                    float* grid, cudaStream_t st);
 bool launch_binning(Plan* p, const double* uv, long long n_vis, int n_chan, cudaStream_t st);
+bool binning_is_small(const Plan* p, long long n_vis);     // the call's a1 + a3 fit one CTA: launch_small_prepass replaces
+bool launch_small_prepass(Plan* p, const double* uv, const double* freqs, long long n_vis, int n_chan, cudaStream_t st);   // launch_scale + launch_binning
 bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                    const int* dispatch, cudaStream_t st);
 bool probe_fp32(Plan* p, double* tflops_ffma, double* tflops_ffma2, cudaStream_t st);
