@@ -185,11 +185,12 @@ int mwa_grid_probe_fp32(mwa_grid_plan* plan, double* out_tflops, void* stream);
 int mwa_grid_probe_smem_atomics(mwa_grid_plan* plan, double* out_rate, void* stream);
 
 /* Test / diagnostics query (synchronises with the device): counters the last K6 gridding call left behind, written
- * into HOST array `out` (up to 8 values): [0] pipeline error code (0 = none; non-zero means a bounded wait inside the
+ * into HOST array `out` (up to 32 values): [0] pipeline error code (0 = none; non-zero means a bounded wait inside the
  * kernel expired and the grid is incomplete), [1] work items, [2] items at least one sample reaches, [3] staged batches
  * of up to 16 hits, [4] largest number of hits of one item, [5] items whose hit list did not fit the pre-pass pool and
- * were swept inside the gridding kernel, [6] work items K5 served through its dense-tile path.  Returns the number of
- * values written. */
+ * were swept inside the gridding kernel, [6] work items K5 served through its dense-tile path; with n >= 32 also [31]
+ * work items of heavy tiles that K3c gridded with the four warps of a CTA (calls with few items per warp).  Returns the
+ * number of values written. */
 int mwa_grid_plan_last_stats(mwa_grid_plan* plan, long long* out, int n);
 
 /* Test / diagnostics: caps the pool that holds K6's per-item hit lists at `entries` list entries (0 = default sizing,

@@ -245,7 +245,8 @@ def mwa_grid_plan_last_stats(plan):
     buf = (ctypes.c_longlong * 32)()
     _check(_lib.mwa_grid_plan_last_stats(plan, ctypes.cast(buf, ctypes.c_void_p), 32))
     return {"error": int(buf[0]), "items": int(buf[1]), "items_with_hits": int(buf[2]), "batches": int(buf[3]),
-            "max_hits": int(buf[4]), "swept_items": int(buf[5]), "k5_dense_items": int(buf[6]), "timing": [int(x) for x in buf[8:32]]}
+            "max_hits": int(buf[4]), "swept_items": int(buf[5]), "k5_dense_items": int(buf[6]), "timing": [int(x) for x in buf[8:32]],
+            "k3c_heavy_items": int(buf[31])}
 
 
 def mwa_grid_probe_smem_atomics(plan, stream=None) -> float:

@@ -174,7 +174,6 @@ bin_order_large_kernel(const double2* __restrict__ uv, const int* __restrict__ b
 
 // Tile weights (rows whose reference-scale bucket lies under the tile) and a heaviest-first tile order by a
 // counting sort on the clipped weight.  Only a scheduling heuristic: any order gives the same grid.
-constexpr int kWeightBins = 1024;
 
 __global__ void tile_weight_kernel(const int* __restrict__ bucket_start, int nb, int nt, int* __restrict__ weight,
                                    int* __restrict__ hist) {

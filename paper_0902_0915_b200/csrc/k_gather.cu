@@ -55,6 +55,9 @@ struct GatherParams {
     int mfs;                    // 1: all channels add into ONE grid [4][N][N] (f3 multi-frequency synthesis): the write-out of a
                                 //    (tile, channel) item is a reduction (red.global.add.v4.f32) into the zero-filled shared grid
     int chunk;                  // consecutive work items per claim (1..8; amortises the round trip of the work counter)
+    const int* heavy_tiles;     // null, or [1]: the first *heavy_tiles entries of tile_order are heavy tiles (weight >= kHeavyTileWeight):
+                                //    each of their items is gridded by the FOUR warps of a CTA together (see "heavy items" below)
+    int* heavy_counter;         // work counter of the heavy items
     int pdl;                    // 1: launched with programmatic stream serialisation behind the fused pre-pass of a small call
                                 //    (bin_small_kernel): the table copies are built while the pre-pass still runs, and
                                 //    griddepcontrol.wait comes before the first read of anything the pre-pass writes
@@ -99,7 +102,10 @@ struct WarpSmem {
 
 constexpr int kBiasU = 16, kBiasV = 16;   // floats; keep the stored offsets non-negative
 
-__global__ void __launch_bounds__(kWarpsPerCta * 32, 4)
+// kHeavy: the instantiation with the CTA-cooperative heavy items in front of the per-warp items (launched only for calls
+// with few items per warp; 3 CTAs per SM so that the second code path does not spill)
+template <bool kHeavy>
+__global__ void __launch_bounds__(kWarpsPerCta * 32, kHeavy ? 3 : 4)
 gather_kernel(const GatherParams P) {
     if (!P.pdl && P.dispatch != nullptr && *P.dispatch != 0) return;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -149,15 +155,47 @@ gather_kernel(const GatherParams P) {
     const size_t plane = (size_t)g.N * g.N;
     const unsigned lt_mask = (1u << lane) - 1u;
 
+    // ---- heavy items.  With few work items per warp (one channel, a large grid: C3) the call lasts as long as its
+    // heaviest tile takes ONE warp - thousands of hits against a mean of a hundred.  The items of the heavy tiles (the
+    // head of tile_order) are therefore taken first, one per CTA: warp k walks every fourth round of 32 candidates
+    // (slice k), the four register tiles are added in shared memory in the fixed order 0 + 1 + 2 + 3 (deterministic),
+    // and warp 0 writes the tile.  A CTA that finds no heavy item left goes on to the per-warp items below.
+    __shared__ long long s_heavy_item;
+    __shared__ int s_any_hit[kWarpsPerCta];
+    u64* red = reinterpret_cast<u64*>(wsm - warp + kWarpsPerCta);      // [3][32][32] u64 behind the WarpSmem array (heavy only)
+    bool heavy = kHeavy;                                                 // CTA-uniform; constant false in the plain instantiation
+    const long long n_heavy = heavy ? (long long)(*P.heavy_tiles) * P.n_chan : 0;   // normal items start here
+    if (kHeavy && blockIdx.x == 0 && threadIdx.x == 0)                   // diagnostics: mwa_grid_plan_last_stats()[31]
+        *reinterpret_cast<long long*>(P.heavy_counter - kMiscHeavyCounter + kMiscHeavyStat) = n_heavy;
+
     long long base = 0;
-    if (lane == 0) base = (long long)atomicAdd(P.counter, P.chunk);
-    base = __shfl_sync(0xffffffffu, base, 0);
     int sub = 0;
     long long next_base = 0;
+    if (!heavy) {
+        if (lane == 0) base = (long long)atomicAdd(P.counter, P.chunk);
+        base = __shfl_sync(0xffffffffu, base, 0);
+    }
 
-    while (base + sub < P.n_items) {
-        const long long item = base + sub;
-        if (sub == 0 && lane == 0) next_base = (long long)atomicAdd(P.counter, P.chunk);   // used P.chunk items from now
+    while (true) {
+        long long item;
+        if (heavy) {
+            __syncthreads();                                             // s_heavy_item and red[] of the item before are free
+            if (threadIdx.x == 0) s_heavy_item = (long long)atomicAdd(P.heavy_counter, 1);
+            __syncthreads();
+            item = s_heavy_item;
+            if (item >= n_heavy) {                                       // on to the per-warp items
+                heavy = false;
+                if (lane == 0) base = (long long)atomicAdd(P.counter, P.chunk);
+                base = __shfl_sync(0xffffffffu, base, 0);
+                sub = 0;
+                continue;
+            }
+        } else {
+            item = n_heavy + base + sub;
+            if (item >= P.n_items) break;
+            if (sub == 0 && lane == 0) next_base = (long long)atomicAdd(P.counter, P.chunk);   // used P.chunk items from now
+        }
+        const int nsl = heavy ? kWarpsPerCta : 1, slice = heavy ? warp : 0;
         const int trank = (int)(item / P.n_chan);
         const int c = (int)(item - (long long)trank * P.n_chan);
         const int tile = P.tile_order[trank];
@@ -310,8 +348,8 @@ gather_kernel(const GatherParams P) {
                     if (ga == 1) break;
                 }
             }
-            const int gstep = (int)(((long long)4 * S) % ng);
-            int gp = (int)(((long long)(lane >> 3) * S) % ng);               // the lane's current group
+            const int gstep = (int)(((long long)(4 * nsl) * S) % ng);          // a round of 32 candidates is 4 groups; every nsl-th round
+            int gp = (int)(((long long)((lane >> 3) + 4 * slice) * S) % ng);   // the lane's current group
             int f = gp * 8 + (lane & 7);
             auto locate = [&](int cb, int& row, double2& p) {
                 int lo = 0;                                                  // smallest bucket row with incl > f
@@ -331,12 +369,12 @@ gather_kernel(const GatherParams P) {
             };
             int row_nx;
             double2 p_nx;
-            locate(0, row_nx, p_nx);
-            for (int cb = 0; cb < ng * 8; cb += 32) {
+            locate(32 * slice, row_nx, p_nx);
+            for (int cb = 32 * slice; cb < ng * 8; cb += 32 * nsl) {
                 const int row = row_nx;
                 const bool in_range = row >= 0;
                 const double2 p = p_nx;
-                if (cb + 32 < ng * 8) locate(cb + 32, row_nx, p_nx);
+                if (cb + 32 * nsl < ng * 8) locate(cb + 32 * nsl, row_nx, p_nx);
                 bool hit = false;
                 unsigned geo = 0, mask = 0;
                 if (in_range) {
@@ -387,6 +425,30 @@ gather_kernel(const GatherParams P) {
             }
         }
         if (n_buf > 0) consume(n_buf);
+
+        if (heavy) {                                                       // add the four warps' register tiles, in warp order
+            if (warp > 0) {
+#pragma unroll
+                for (int i = 0; i < 2; ++i)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) red[((warp - 1) * 32 + (i * 16 + j * 4 + q)) * 32 + lane] = acc[i][j][q];
+            }
+            if (lane == 0) s_any_hit[warp] = any_hit ? 1 : 0;
+            __syncthreads();
+            if (warp > 0) continue;                                        // (the barrier at the head of the loop comes next)
+            const u64 ones = pack2(1.0f, 1.0f);
+            for (int w = 0; w < kWarpsPerCta - 1; ++w) {
+#pragma unroll
+                for (int i = 0; i < 2; ++i)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) ffma2(acc[i][j][q], ones, red[(w * 32 + (i * 16 + j * 4 + q)) * 32 + lane]);   // acc += 1 * partial
+            }
+            any_hit = (s_any_hit[0] | s_any_hit[1] | s_any_hit[2] | s_any_hit[3]) != 0;
+        }
 
         // ---- a5: write the lane's 4x2 block of all 4 planes, once
         if (P.mfs) {
@@ -446,13 +508,12 @@ gather_kernel(const GatherParams P) {
                 }
             }
         }
-        if (++sub == P.chunk) { sub = 0; base = __shfl_sync(0xffffffffu, next_base, 0); }
+        if (!heavy && ++sub == P.chunk) { sub = 0; base = __shfl_sync(0xffffffffu, next_base, 0); }
     }
 }
 
 bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
                    const int* dispatch, cudaStream_t st) {
-    (void)n_vis;
     GatherParams P;
     P.g = p->geom;
     P.scale = p->ws.d_scale;
@@ -480,13 +541,19 @@ bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, i
     P.rlv = (p->geom.W + 2 + 1) & ~1;
     P.n_items = (long long)P.nt * P.nt * n_chan;
     const size_t tbl = ((size_t)(4 * P.rlu + 2 * P.rlv) * (p->geom.O + 1) * 4 + 15) & ~size_t(15);
-    const size_t smem = tbl + sizeof(WarpSmem) * kWarpsPerCta;
+    // heavy items (see the kernel): only where a single warp's heaviest tile can be the critical path - few items per warp -
+    // and not behind the one-CTA pre-pass of small calls (it does not count the heavy tiles)
+    const bool use_heavy = !binning_is_small(p, n_vis) && P.n_items < (long long)p->sm_count * 16 * 32;
+    P.heavy_tiles = use_heavy ? p->ws.d_misc + kMiscHeavyTiles : nullptr;
+    P.heavy_counter = p->ws.d_misc + kMiscHeavyCounter;
+    const size_t smem = tbl + sizeof(WarpSmem) * kWarpsPerCta + (use_heavy ? (size_t)(kWarpsPerCta - 1) * 32 * 32 * 8 : 0);
     // a per-device setting: set on every launch (cheap), so a process that uses several GPUs gets it on each
-    if (!cuda_ok(cudaFuncSetAttribute(gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024),
+    void (*kern)(const GatherParams) = use_heavy ? gather_kernel<true> : gather_kernel<false>;
+    if (!cuda_ok(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024),
                  "gather smem attribute"))
         return false;
     int ctas_per_sm = 0;
-    if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, gather_kernel, kWarpsPerCta * 32, smem),
+    if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctas_per_sm, kern, kWarpsPerCta * 32, smem),
                  "gather occupancy"))
         return false;
     if (ctas_per_sm < 1) { set_error("gather kernel does not fit on an SM"); return false; }
@@ -511,9 +578,9 @@ bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, i
         cfg.attrs = attr;
         cfg.numAttrs = 1;
         p->last_launches += 1;
-        return cuda_ok(cudaLaunchKernelEx(&cfg, gather_kernel, P), "gather_kernel (dependent launch)");
+        return cuda_ok(cudaLaunchKernelEx(&cfg, kern, P), "gather_kernel (dependent launch)");
     }
-    gather_kernel<<<(unsigned)blocks, kWarpsPerCta * 32, smem, st>>>(P);
+    kern<<<(unsigned)blocks, kWarpsPerCta * 32, smem, st>>>(P);
     p->last_launches += 1;
     return cuda_ok(cudaGetLastError(), "gather_kernel");
 }

@@ -14,6 +14,16 @@ constexpr int kChanMinChannels = 8; // AUTO picks a channel-SIMD kernel (K6 / K5
 constexpr int kTile = 16;           // gridding tile side in cells (one warp owns one tile of one channel)
 // d_misc (ints, zeroed by every call's binning step): [0..3] work counters, [4..11] diagnostics, [12..13] hit-list pool
 // cursor (u64), [14..15] K6 item counts, [16..] tile-weight histogram (4096), then the block states of chan_order_kernel
+constexpr int kWeightBins = 1024;            // tile-weight histogram bins (weight clipped to kWeightBins - 1), heaviest first
+#ifndef MWA_HEAVY_TILE_WEIGHT
+#define MWA_HEAVY_TILE_WEIGHT 256
+#endif
+constexpr int kHeavyTileWeight = MWA_HEAVY_TILE_WEIGHT;        // a tile with this many rows in the buckets under it (~ 480 hits with the halo) is "heavy":
+                                             // K3c grids its items with the four warps of a CTA when items are few (k_gather.cu)
+constexpr int kMiscHeavyTiles = 16 + kWeightBins - 1 - kHeavyTileWeight;   // after tile_order_scatter_kernel: end of that weight bin
+                                             // in tile_order = the number of tiles at least that heavy
+constexpr int kMiscHeavyCounter = 16 + kWeightBins;   // [1] work counter of K3c's heavy items
+constexpr int kMiscHeavyStat = 2048 + 46;              // long long: heavy items of the last K3c call (last_stats()[31])
 constexpr int kMiscTailStart = 16 + 4080;    // [1] first entry of the last channel group in K6's list of items with hits
 constexpr int kMiscOrderState = 16 + 4096;
 constexpr int kMiscScanState = kMiscOrderState + 2048;   // block states of bin_scan_kernel (<= 1024 blocks: 4 M buckets)

@@ -595,6 +595,38 @@ def test_multi_frequency_synthesis_sums_the_channels_onto_one_grid(lib, design):
         assert tuple(back.shape) == (12, 4, 250, 250)
 
 
+# ---------------------------------------------------------------------------- K3c: heavy tiles gridded by four warps
+@pytest.mark.parametrize("mode", ["overwrite", "accumulate", "mfs"])
+def test_gather_heavy_tiles_are_gridded_by_the_four_warps_of_a_cta(lib, mode):
+    """Few items per warp and a dense core (C3's regime): K3c takes the items of the heavy tiles first, one per CTA, every warp
+    a quarter of the candidates, partial tiles added in a fixed order.  Observable through last_stats; bit-identical from
+    call to call; all three write-out modes."""
+    g = generate(scaled(CONFIGS["C3"], n_ant=128, core_ant=96, core_radius_m=300.0, n_chan=2, grid_n=500,
+                        f_lo_hz=150e6, f_hi_hz=152e6))             # 22 tiles of 256 - 1900 rows each
+    assert g.cfg.n_vis > 4096                                        # not the one-CTA pre-pass of small calls
+    G, A, _ = _oracle(g)
+    _to_dev(g)
+    with _plan(lib, g, "gather") as p:
+        if mode == "mfs":
+            p.set_mfs(True)
+            G, A = G.sum(axis=0, keepdims=True), A.sum(axis=0, keepdims=True)
+        out = p.grid(g.uv, g.freqs, g.vis, g.weights)
+        torch.cuda.synchronize()
+        st = lib.mwa_grid_plan_last_stats(p.handle)
+        assert st["k3c_heavy_items"] > 0, st
+        assert_parity(out.cpu().numpy(), G, A, f"heavy tiles {mode}")
+        for _ in range(3):
+            again = p.grid(g.uv, g.freqs, g.vis, g.weights)
+            if mode != "mfs":                                        # MFS adds the channels with reductions: order not fixed
+                assert torch.equal(again.view(torch.float32), out.view(torch.float32))
+        if mode == "accumulate":
+            lib.mwa_grid_plan_set_accumulate(p.handle, True)
+            p.grid(g.uv, g.freqs, g.vis, g.weights, out=out)
+            bound = 2 * (1e-5 * A + 1e-7) + 3 * 2.0 ** -24 * np.abs(2 * G)
+            assert np.all(np.abs(out.cpu().numpy().astype(np.complex128) - 2 * G) <= bound)
+            lib.mwa_grid_plan_set_accumulate(p.handle, False)
+
+
 # ---------------------------------------------------------------------------- K6 stress: many shapes, repeated calls
 @pytest.mark.parametrize("seed", [0, 1, 2])
 def test_chanws_random_shapes_repeated_calls(lib, seed):
