@@ -103,22 +103,57 @@ __global__ void bin_scatter_kernel(GridGeom g, const double2* __restrict__ uv, c
 // ~8 rows on average, a few hundred in the core) and writes the sorted copies.  With this the bucket-sorted order is a
 // pure function of the input, so K3c and K5 - which add the taps of a cell in list order, with no atomics - give
 // bit-identical grids from run to run.
-// A bucket of more than kOrderWarpMax rows (a degenerate input: a compact array, a coarse du, many rows at uv = 0) is
-// not ranked here - k^2 / 32 steps per lane would look like a hang - but put on a list for bin_order_large_kernel.
-constexpr int kOrderWarpMax = 2048;
-constexpr int kBigListCap = 1023;                      // n_vis / kOrderWarpMax big buckets at most: 2 M rows and more
+// A bucket of more than kOrderWarpMax rows (the core of a dense array; or a degenerate input: a compact array, a coarse
+// du, many rows at uv = 0) is not ranked here - k^2 / 32 steps per lane make one warp the critical path of the call -
+// but put on a list for bin_order_large_kernel, which gives it a whole block.
+constexpr int kOrderWarpMax = 256;                     // buckets up to this many rows are ranked by one warp, from shared memory
+constexpr int kOrderStage = kOrderWarpMax;
+constexpr int kOrderBlockRank = 2048;                  // bin_order_large_kernel: up to this many rows by counting, beyond by bitonic sort
+constexpr int kBigListCap = 1023;                      // buckets beyond the list are ranked by their warp of bin_order_kernel
 
 __global__ void bin_order_kernel(const double2* __restrict__ uv, const int* __restrict__ bucket_start, int n_buckets,
                                  const int* __restrict__ perm_tmp, int* __restrict__ perm,
                                  double2* __restrict__ uv_sorted, double4* __restrict__ row_sorted, int* __restrict__ big_list) {
+    __shared__ int s_stage[8][kOrderStage];                // blocks of 256 threads
     const int lane = threadIdx.x & 31;
+    int* stage = s_stage[(threadIdx.x >> 5) & 7];
     const int warps = (gridDim.x * blockDim.x) >> 5;
     for (int b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; b < n_buckets; b += warps) {
         const int k0 = bucket_start[b], k1 = bucket_start[b + 1];
         if (k1 - k0 > kOrderWarpMax) {
+            int slot = 0;
             if (lane == 0) {
-                const int slot = atomicAdd(big_list, 1);
+                slot = atomicAdd(big_list, 1);
                 if (slot < kBigListCap) big_list[1 + slot] = b;
+            }
+            if (__shfl_sync(0xffffffffu, slot, 0) < kBigListCap) continue;
+            // the list is full (more than 1023 such buckets): this warp ranks the bucket itself, slowly, below
+        }
+        const int k = k1 - k0;
+        if (k > 32 && k <= kOrderStage) {
+            // the dense buckets of a core (hundreds of rows) are what this kernel's time is made of: the bucket is staged in
+            // shared memory and a lane ranks four of its rows per pass over it (one broadcast LDS per four compares)
+            __syncwarp();
+            for (int i = lane; i < k; i += 32) stage[i] = perm_tmp[k0 + i];
+            __syncwarp();
+            for (int i0 = lane; i0 < k; i0 += 128) {
+                int row[4], rank[4] = {0, 0, 0, 0};
+#pragma unroll
+                for (int t = 0; t < 4; ++t) row[t] = i0 + 32 * t < k ? stage[i0 + 32 * t] : 0x7fffffff;
+                for (int j = 0; j < k; ++j) {
+                    const int v = stage[j];
+#pragma unroll
+                    for (int t = 0; t < 4; ++t) rank[t] += v < row[t];
+                }
+#pragma unroll
+                for (int t = 0; t < 4; ++t) {
+                    if (i0 + 32 * t < k) {
+                        const double2 p = uv[row[t]];
+                        perm[k0 + rank[t]] = row[t];
+                        uv_sorted[k0 + rank[t]] = p;
+                        row_sorted[k0 + rank[t]] = make_double4(p.x, p.y, (double)row[t], 0.0);
+                    }
+                }
             }
             continue;
         }
@@ -142,11 +177,39 @@ __global__ void __launch_bounds__(1024)
 bin_order_large_kernel(const double2* __restrict__ uv, const int* __restrict__ bucket_start, int* __restrict__ perm_tmp,
                        int* __restrict__ perm, double2* __restrict__ uv_sorted, double4* __restrict__ row_sorted,
                        const int* __restrict__ big_list) {
+    __shared__ int s_rows[kOrderBlockRank];
     const int n_big = min(big_list[0], kBigListCap);
     for (int q = blockIdx.x; q < n_big; q += gridDim.x) {
         const int b = big_list[1 + q];
         const int k0 = bucket_start[b], n = bucket_start[b + 1] - k0;
         int* a = perm_tmp + k0;
+        if (n <= kOrderBlockRank) {                          // the dense buckets of a core: rank by counting, from shared memory
+            for (int i = threadIdx.x; i < n; i += 1024) s_rows[i] = a[i];
+            __syncthreads();
+            for (int i0 = threadIdx.x; i0 < n; i0 += 2048) {
+                const int r0 = s_rows[i0], r1 = i0 + 1024 < n ? s_rows[i0 + 1024] : 0x7fffffff;
+                int rank0 = 0, rank1 = 0;
+                for (int j = 0; j < n; ++j) {
+                    const int v = s_rows[j];
+                    rank0 += v < r0;
+                    rank1 += v < r1;
+                }
+                {
+                    const double2 p = uv[r0];
+                    perm[k0 + rank0] = r0;
+                    uv_sorted[k0 + rank0] = p;
+                    row_sorted[k0 + rank0] = make_double4(p.x, p.y, (double)r0, 0.0);
+                }
+                if (i0 + 1024 < n) {
+                    const double2 p = uv[r1];
+                    perm[k0 + rank1] = r1;
+                    uv_sorted[k0 + rank1] = p;
+                    row_sorted[k0 + rank1] = make_double4(p.x, p.y, (double)r1, 0.0);
+                }
+            }
+            __syncthreads();
+            continue;
+        }
         for (int k = 2; (k >> 1) < n; k <<= 1) {
             for (int i = threadIdx.x; i < n; i += 1024) {            // mirror step
                 const int j = i ^ (k - 1);
@@ -177,8 +240,13 @@ bin_order_large_kernel(const double2* __restrict__ uv, const int* __restrict__ b
 
 __global__ void tile_weight_kernel(const int* __restrict__ bucket_start, int nb, int nt, int* __restrict__ weight,
                                    int* __restrict__ hist) {
-    const int per = kTile / kBucketCells;
-    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < nt * nt; t += gridDim.x * blockDim.x) {
+    const int per = kTile / kBucketCells, lane = threadIdx.x & 31;
+    // a warp walks 32 consecutive tiles per pass (the loop bound is uniform in the warp: the warp-wide votes below are safe)
+    for (int t0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31; t0 < nt * nt; t0 += gridDim.x * blockDim.x) {
+        const int t = t0 + lane;
+        const bool valid = t < nt * nt;
+        const unsigned act = __ballot_sync(0xffffffffu, valid);
+        if (!valid) continue;
         const int ty = t / nt, tx = t - ty * nt;
         int w = 0;
         for (int dy = 0; dy < per; ++dy) {
@@ -189,7 +257,10 @@ __global__ void tile_weight_kernel(const int* __restrict__ bucket_start, int nb,
             if (b0 < b1) w += bucket_start[b1] - bucket_start[b0];
         }
         weight[t] = w;
-        atomicAdd(&hist[kWeightBins - 1 - min(w, kWeightBins - 1)], 1);   // descending
+        // descending; one atomic per distinct bin of the warp (most tiles of a sparse grid are empty: one bin for all of them)
+        const int bin = kWeightBins - 1 - min(w, kWeightBins - 1);
+        const unsigned same = __match_any_sync(act, bin);
+        if (__ffs(same) - 1 == lane) atomicAdd(&hist[bin], __popc(same));
     }
 }
 
@@ -208,8 +279,18 @@ __global__ void tile_order_scan_kernel(int* __restrict__ hist) {   // one block 
 
 __global__ void tile_order_scatter_kernel(const int* __restrict__ weight, int n_tiles, int* __restrict__ hist,
                                           int* __restrict__ order) {
-    for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < n_tiles; t += gridDim.x * blockDim.x) {
-        const int pos = atomicAdd(&hist[kWeightBins - 1 - min(weight[t], kWeightBins - 1)], 1);
+    const int lane = threadIdx.x & 31;
+    for (int t0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31; t0 < n_tiles; t0 += gridDim.x * blockDim.x) {
+        const int t = t0 + lane;
+        const bool valid = t < n_tiles;
+        const unsigned act = __ballot_sync(0xffffffffu, valid);
+        if (!valid) continue;
+        const int bin = kWeightBins - 1 - min(weight[t], kWeightBins - 1);
+        const unsigned same = __match_any_sync(act, bin);                 // the lanes of one bin take consecutive places
+        const int leader = __ffs(same) - 1;
+        int pos = 0;
+        if (lane == leader) pos = atomicAdd(&hist[bin], __popc(same));
+        pos = __shfl_sync(same, pos, leader) + __popc(same & ((1u << lane) - 1u));
         order[pos] = t;
     }
 }
@@ -374,7 +455,7 @@ bool launch_binning(Plan* p, const double* uv, long long n_vis, int /*n_chan*/, 
         bin_order_kernel<<<(unsigned)oblocks, 256, 0, st>>>((const double2*)uv, ws.d_bucket_count, n_buckets, ws.d_perm_tmp, ws.d_perm,
                                                             ws.d_uv_sorted, (double4*)ws.d_row_sorted, ws.d_misc + kMiscBigList);
         if (n_vis > kOrderWarpMax) {                           // else no bucket can be big
-            bin_order_large_kernel<<<p->sm_count < 64 ? p->sm_count : 64, 1024, 0, st>>>((const double2*)uv, ws.d_bucket_count, ws.d_perm_tmp, ws.d_perm,
+            bin_order_large_kernel<<<p->sm_count, 1024, 0, st>>>((const double2*)uv, ws.d_bucket_count, ws.d_perm_tmp, ws.d_perm,
                                                                                          ws.d_uv_sorted, (double4*)ws.d_row_sorted,
                                                                                          ws.d_misc + kMiscBigList);
             p->last_launches += 1;
