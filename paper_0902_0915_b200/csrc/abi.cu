@@ -160,16 +160,19 @@ static int grid_device(Plan* p, const double* uv, const double* freqs, const flo
     const bool bins = design != MWA_GRID_DESIGN_ATOMIC && design != MWA_GRID_DESIGN_ROMEIN && n_vis > 0;
     if (bins && binning_is_small(p, n_vis)) {              // launch-bound calls: a1 + a3 in one launch
         if (!launch_small_prepass(p, uv, freqs, n_vis, n_chan, st)) return MWA_GRID_ERR_CUDA;
-        // only a gather kernel that DIRECTLY follows the pre-pass may be launched as its programmatic dependent
-        const bool direct = !prof && !p->d_table2d && (design == MWA_GRID_DESIGN_GATHER ||
-                                                      (design == MWA_GRID_DESIGN_AUTO && (n_chan < kChanMinChannels || p->mfs)));
-        p->pdl_next = direct && !(p->mfs && !p->accumulate);     // MFS puts a memset between the two
-#ifdef MWA_NO_PDL
-        p->pdl_next = false;                                     // A/B measurement build only
-#endif
     } else {
         if (!launch_scale(p, freqs, n_chan, st)) return MWA_GRID_ERR_CUDA;
         if (bins && !launch_binning(p, uv, n_vis, n_chan, st)) return MWA_GRID_ERR_CUDA;
+    }
+    {
+        // the pre-pass kernels form a chain of programmatic dependent launches; only a gather kernel that DIRECTLY follows
+        // the chain joins it (nothing may sit between the two: no stage timer, no memset of the MFS grid, no other kernel)
+        const bool direct = !prof && !p->d_table2d && (design == MWA_GRID_DESIGN_GATHER ||
+                                                      (design == MWA_GRID_DESIGN_AUTO && (n_chan < kChanMinChannels || p->mfs)));
+        p->pdl_next = p->pdl_next && direct && !(p->mfs && !p->accumulate);
+#ifdef MWA_NO_PDL
+        p->pdl_next = false;                                     // A/B measurement build only
+#endif
     }
     if (prof) cudaEventRecord(p->ev[1], st);
     bool ok = false;

@@ -19,6 +19,8 @@ __device__ __forceinline__ int bucket_coord(double metres, double s_ref, double 
 
 __global__ void bin_count_kernel(GridGeom g, const double2* __restrict__ uv, const double* __restrict__ s_ref_p,
                                  int n_vis, int nb, int* __restrict__ count) {
+    pdl_wait();                                         // chain of dependent launches (plan.h)
+    pdl_release();
     const double s_ref = *s_ref_p;
     for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < n_vis; n += gridDim.x * blockDim.x) {
         const double2 p = uv[n];
@@ -37,6 +39,8 @@ constexpr int kScanFlag = 1 << 30;
 
 __global__ void __launch_bounds__(1024)
 bin_scan_kernel(int* __restrict__ count, int n, int* __restrict__ cursor, volatile int* blk_state) {
+    pdl_wait();                                         // chain of dependent launches (plan.h)
+    pdl_release();
     __shared__ int warp_sum[32];
     __shared__ int prefix_s;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, b = blockIdx.x;
@@ -90,6 +94,8 @@ bin_scan_kernel(int* __restrict__ count, int n, int* __restrict__ cursor, volati
 
 __global__ void bin_scatter_kernel(GridGeom g, const double2* __restrict__ uv, const double* __restrict__ s_ref_p,
                                    int n_vis, int nb, int* __restrict__ cursor, int* __restrict__ perm_tmp) {
+    pdl_wait();                                         // chain of dependent launches (plan.h)
+    pdl_release();
     const double s_ref = *s_ref_p;
     for (int n = blockIdx.x * blockDim.x + threadIdx.x; n < n_vis; n += gridDim.x * blockDim.x) {
         const double2 p = uv[n];
@@ -114,6 +120,8 @@ constexpr int kBigListCap = 1023;                      // buckets beyond the lis
 __global__ void bin_order_kernel(const double2* __restrict__ uv, const int* __restrict__ bucket_start, int n_buckets,
                                  const int* __restrict__ perm_tmp, int* __restrict__ perm,
                                  double2* __restrict__ uv_sorted, double4* __restrict__ row_sorted, int* __restrict__ big_list) {
+    pdl_wait();                                         // chain of dependent launches (plan.h)
+    pdl_release();
     __shared__ int s_stage[8][kOrderStage];                // blocks of 256 threads
     const int lane = threadIdx.x & 31;
     int* stage = s_stage[(threadIdx.x >> 5) & 7];
@@ -177,6 +185,8 @@ __global__ void __launch_bounds__(1024)
 bin_order_large_kernel(const double2* __restrict__ uv, const int* __restrict__ bucket_start, int* __restrict__ perm_tmp,
                        int* __restrict__ perm, double2* __restrict__ uv_sorted, double4* __restrict__ row_sorted,
                        const int* __restrict__ big_list) {
+    pdl_wait();                                         // chain of dependent launches (plan.h)
+    pdl_release();
     __shared__ int s_rows[kOrderBlockRank];
     const int n_big = min(big_list[0], kBigListCap);
     for (int q = blockIdx.x; q < n_big; q += gridDim.x) {
@@ -240,6 +250,8 @@ bin_order_large_kernel(const double2* __restrict__ uv, const int* __restrict__ b
 
 __global__ void tile_weight_kernel(const int* __restrict__ bucket_start, int nb, int nt, int* __restrict__ weight,
                                    int* __restrict__ hist) {
+    pdl_wait();                                         // chain of dependent launches (plan.h)
+    pdl_release();
     const int per = kTile / kBucketCells, lane = threadIdx.x & 31;
     // a warp walks 32 consecutive tiles per pass (the loop bound is uniform in the warp: the warp-wide votes below are safe)
     for (int t0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31; t0 < nt * nt; t0 += gridDim.x * blockDim.x) {
@@ -265,6 +277,8 @@ __global__ void tile_weight_kernel(const int* __restrict__ bucket_start, int nb,
 }
 
 __global__ void tile_order_scan_kernel(int* __restrict__ hist) {   // one block of kWeightBins threads
+    pdl_wait();                                         // chain of dependent launches (plan.h)
+    pdl_release();
     __shared__ int s[kWeightBins];
     s[threadIdx.x] = hist[threadIdx.x];
     __syncthreads();
@@ -279,6 +293,8 @@ __global__ void tile_order_scan_kernel(int* __restrict__ hist) {   // one block 
 
 __global__ void tile_order_scatter_kernel(const int* __restrict__ weight, int n_tiles, int* __restrict__ hist,
                                           int* __restrict__ order) {
+    pdl_wait();                                         // chain of dependent launches (plan.h)
+    pdl_release();
     const int lane = threadIdx.x & 31;
     for (int t0 = (blockIdx.x * blockDim.x + threadIdx.x) & ~31; t0 < n_tiles; t0 += gridDim.x * blockDim.x) {
         const int t = t0 + lane;
@@ -445,28 +461,39 @@ bool launch_binning(Plan* p, const double* uv, long long n_vis, int /*n_chan*/, 
     if (blocks > p->sm_count * 8) blocks = p->sm_count * 8;
     bin_count_kernel<<<blocks, 256, 0, st>>>(p->geom, (const double2*)uv, ws.d_scale_ref, (int)n_vis, nb,
                                              ws.d_bucket_count);
-    bin_scan_kernel<<<(n_buckets + kScanPerBlock - 1) / kScanPerBlock, 1024, 0, st>>>(ws.d_bucket_count, n_buckets, ws.d_bucket_cursor,
-                                                                                     ws.d_misc + kMiscScanState);
-    bin_scatter_kernel<<<blocks, 256, 0, st>>>(p->geom, (const double2*)uv, ws.d_scale_ref, (int)n_vis, nb,
-                                               ws.d_bucket_cursor, ws.d_perm_tmp);
+    // from here on every kernel is launched as a programmatic dependent of the one before it: it becomes resident while
+    // its predecessor drains and waits (pdl_wait) for the predecessor's completion before its first read
+    cudaError_t e = launch_dependent(bin_scan_kernel, dim3((n_buckets + kScanPerBlock - 1) / kScanPerBlock), dim3(1024), 0, st,
+                                     ws.d_bucket_count, n_buckets, ws.d_bucket_cursor, ws.d_misc + kMiscScanState);
+    if (e == cudaSuccess)
+        e = launch_dependent(bin_scatter_kernel, dim3(blocks), dim3(256), 0, st, p->geom, (const double2*)uv, (const double*)ws.d_scale_ref,
+                             (int)n_vis, nb, ws.d_bucket_cursor, ws.d_perm_tmp);
     {
         long long oblocks = ((long long)n_buckets * 32 + 255) / 256;
         if (oblocks > p->sm_count * 16) oblocks = p->sm_count * 16;
-        bin_order_kernel<<<(unsigned)oblocks, 256, 0, st>>>((const double2*)uv, ws.d_bucket_count, n_buckets, ws.d_perm_tmp, ws.d_perm,
-                                                            ws.d_uv_sorted, (double4*)ws.d_row_sorted, ws.d_misc + kMiscBigList);
+        if (e == cudaSuccess)
+            e = launch_dependent(bin_order_kernel, dim3((unsigned)oblocks), dim3(256), 0, st, (const double2*)uv, (const int*)ws.d_bucket_count,
+                                 n_buckets, (const int*)ws.d_perm_tmp, ws.d_perm, ws.d_uv_sorted, (double4*)ws.d_row_sorted,
+                                 ws.d_misc + kMiscBigList);
         if (n_vis > kOrderWarpMax) {                           // else no bucket can be big
-            bin_order_large_kernel<<<p->sm_count, 1024, 0, st>>>((const double2*)uv, ws.d_bucket_count, ws.d_perm_tmp, ws.d_perm,
-                                                                                         ws.d_uv_sorted, (double4*)ws.d_row_sorted,
-                                                                                         ws.d_misc + kMiscBigList);
+            if (e == cudaSuccess)
+                e = launch_dependent(bin_order_large_kernel, dim3(p->sm_count), dim3(1024), 0, st, (const double2*)uv,
+                                     (const int*)ws.d_bucket_count, ws.d_perm_tmp, ws.d_perm, ws.d_uv_sorted, (double4*)ws.d_row_sorted,
+                                     (const int*)(ws.d_misc + kMiscBigList));
             p->last_launches += 1;
         }
     }
     int* hist = ws.d_misc + 16;
     int tblocks = (nt * nt + 255) / 256;
     if (tblocks > p->sm_count * 8) tblocks = p->sm_count * 8;
-    tile_weight_kernel<<<tblocks, 256, 0, st>>>(ws.d_bucket_count, nb, nt, ws.d_tile_weight, hist);
-    tile_order_scan_kernel<<<1, kWeightBins, 0, st>>>(hist);
-    tile_order_scatter_kernel<<<tblocks, 256, 0, st>>>(ws.d_tile_weight, nt * nt, hist, ws.d_tile_order);
+    if (e == cudaSuccess)
+        e = launch_dependent(tile_weight_kernel, dim3(tblocks), dim3(256), 0, st, (const int*)ws.d_bucket_count, nb, nt, ws.d_tile_weight, hist);
+    if (e == cudaSuccess) e = launch_dependent(tile_order_scan_kernel, dim3(1), dim3(kWeightBins), 0, st, hist);
+    if (e == cudaSuccess)
+        e = launch_dependent(tile_order_scatter_kernel, dim3(tblocks), dim3(256), 0, st, (const int*)ws.d_tile_weight, nt * nt, hist,
+                             ws.d_tile_order);
+    if (!cuda_ok(e, "binning kernels (dependent launches)")) return false;
+    p->pdl_next = true;                                        // a gridder that comes next may join the chain
     p->last_launches += 9;
     return cuda_ok(cudaGetLastError(), "binning kernels");
 }

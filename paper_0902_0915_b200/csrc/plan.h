@@ -96,6 +96,29 @@ struct Plan {
                                      // at once): launch_gather, if it comes next, launches with programmatic stream serialisation
 };
 
+// ---- programmatic dependent launch (the kernels of one call's pre-pass chain)
+// A kernel launched with launch_dependent may become resident while the kernel before it on the stream still runs; it
+// must execute pdl_wait() before it touches anything that kernel (or any kernel before that) writes - every kernel of a
+// chain does so first thing, in every thread, so completion is transitive - and pdl_release() lets the next kernel of
+// the chain become resident in turn.  Both are no-ops in a kernel that was launched the plain way.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_release() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_dependent(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 void set_error(const std::string& msg);
 bool cuda_ok(cudaError_t e, const char* what);
 
