@@ -160,13 +160,20 @@ def run_ours(args):
         from gen import baseline_major
         g = baseline_major(g)
     plan = lib.Plan(cfg.grid_n, g.cell_du, cfg.support_W, cfg.oversample_O, g.kernel_table, design=args.design)
-    lib.mwa_grid_plan_set_profiling(plan.handle, False)       # the timed steps run without the plan's internal stage timers
+    lib.mwa_grid_plan_set_profiling(plan.handle, True)        # the plan's stage timers (CUDA events on the call's stream); see below
     if args.mfs:                                  # comparison runs only: all channels onto one shared grid (f3)
         plan.set_mfs(True)
     grid = torch.empty((1 if args.mfs else cfg.n_chan, 4, cfg.grid_n, cfg.grid_n), dtype=torch.complex64, device=dev)
     alg_bytes = cfg.algorithmic_bytes()
     small = alg_bytes < 512e6                     # fits (mostly) in the 126 MB L2: flush between iterations
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if small else None
+
+    # Stage timers: on during the timed steps (the roofline's kernel time then comes from the timed region itself), except on
+    # the launch-bound configs (C1 - C3, a call of 0.02 - 0.4 ms): there the event records between the kernels cost
+    # microseconds and keep the gridding kernel from being launched as a programmatic dependent of its pre-pass, so the
+    # timed steps run without them and a second pass of the same steps measures the split.
+    inline_timers = not small
+    lib.mwa_grid_plan_set_profiling(plan.handle, inline_timers)
 
     def step():
         if flush is not None:
@@ -197,21 +204,20 @@ def run_ours(args):
         ev1.record()
         ev1.synchronize()
         tot_ms += ev0.elapsed_time(ev1)
+        if inline_timers:
+            stage.append(lib.mwa_grid_plan_stage_ms(plan.handle))
         launches += lib.mwa_grid_plan_last_launches(plan.handle)
     barrier()
-    # second pass, same steps, with the plan's stage timers on (CUDA events on the call's stream around a1 + a3 and around the
-    # gridding kernels): the per-stage split and the roofline of the gridding stage.  Kept out of the timed steps above because
-    # the event records sit between the kernels (they cost microseconds on the launch-bound configs and keep the gridding
-    # kernel of a small call from being launched as a programmatic dependent of its pre-pass).
-    lib.mwa_grid_plan_set_profiling(plan.handle, True)
-    for _ in range(args.steps):
-        if flush is not None:
-            flush.fill_(1)
-        lib.mwa_grid_visibilities(plan.handle, g.uv, g.freqs, g.vis, g.weights, cfg.n_vis, cfg.n_chan, grid)
-        torch.cuda.synchronize()
-        stage.append(lib.mwa_grid_plan_stage_ms(plan.handle))
-    lib.mwa_grid_plan_set_profiling(plan.handle, False)
-    barrier()
+    if not inline_timers:                         # second pass, same steps, stage timers on: the per-stage split and the roofline
+        lib.mwa_grid_plan_set_profiling(plan.handle, True)
+        for _ in range(args.steps):
+            if flush is not None:
+                flush.fill_(1)
+            lib.mwa_grid_visibilities(plan.handle, g.uv, g.freqs, g.vis, g.weights, cfg.n_vis, cfg.n_chan, grid)
+            torch.cuda.synchronize()
+            stage.append(lib.mwa_grid_plan_stage_ms(plan.handle))
+        lib.mwa_grid_plan_set_profiling(plan.handle, False)
+        barrier()
     ran = lib.mwa_grid_plan_last_design(plan.handle)           # resolves AUTO (device-side choice)
     clocks = sampler.stop() if rank == 0 else None
     t = torch.tensor([tot_ms], dtype=torch.float64, device=dev)
@@ -266,7 +272,8 @@ def run_ours(args):
                                f"grid {cfg.grid_n}^2 per channel and pol, kernel {cfg.support_W}x{cfg.support_W} "
                                f"oversampling {cfg.oversample_O}",
                    "design": args.design, "design_ran": ran, "row_order": args.row_order, "mfs": bool(args.mfs), "per_gpu": "one full snapshot per rank",
-                   "stage_split": "stage_ms and roofline come from a second pass of the same steps with the plan's stage timers on",
+                   "stage_split": "stage timers on during the timed steps" if inline_timers else
+                                  "launch-bound config: timed steps without stage timers; stage_ms and roofline from a second pass of the same steps with them on",
                    "cache": "256 MB L2 flush before every step" if small else
                             f"inputs+outputs {alg_bytes / 1e9:.1f} GB >> 126 MB L2, no flush"},
         "kernel_tap_updates_per_sec": value * cfg.support_W ** 2,
