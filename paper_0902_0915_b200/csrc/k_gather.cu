@@ -24,6 +24,9 @@
 //            onto one grid) a red.global.add.v4.f32 per 16 B.
 //
 // Work items (tile, channel) are taken from a global counter up to 8 at a time, channel fastest, tiles heaviest first.
+// Calls with few items per warp run the instantiation gather_kernel<true>: the items of the heavy tiles come first and
+// are gridded by the four warps of a CTA together ("heavy items" in the kernel).  Behind a pre-pass chain of programmatic
+// dependent launches (plan.h) the kernel builds its table copies before griddepcontrol.wait (GatherParams::pdl).
 // profiles/r02_gather_c5.md: C5 in 23.0 ms (round 1: 36.4 ms); bound by the shared-memory pipe (the LDS of phase B are
 // lane-scattered by construction).
 #include "plan.h"
