@@ -48,3 +48,10 @@ def test_product_does_not_import_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in src and "from oracle" not in src and "oracle/" not in src, f
+
+
+def test_noalloc_limits_in_the_binding_match_the_header():
+    import paper_0902_0915_b200 as m
+    text = open(os.path.join(ROOT, "include", "mwa_grid.h")).read()
+    lim = {k: int(v) for k, v in re.findall(r"#define\s+MWA_GRID_NOALLOC_(MAX_[A-Z_]+)\s+(\d+)", text)}
+    assert lim == {"MAX_VIS": m.NOALLOC_MAX_VIS, "MAX_CHAN": m.NOALLOC_MAX_CHAN, "MAX_GRID_N": m.NOALLOC_MAX_GRID_N}
