@@ -29,6 +29,8 @@
 // dependent launches (plan.h) the kernel builds its table copies before griddepcontrol.wait (GatherParams::pdl).
 // profiles/r02_gather_c5.md: C5 in 23.0 ms (round 1: 36.4 ms); bound by the shared-memory pipe (the LDS of phase B are
 // lane-scattered by construction).
+#include <cstdint>
+
 #include "plan.h"
 
 namespace mwa {
@@ -61,6 +63,7 @@ struct GatherParams {
     const int* heavy_tiles;     // null, or [1]: the first *heavy_tiles entries of tile_order are heavy tiles (weight >= kHeavyTileWeight):
                                 //    each of their items is gridded by the FOUR warps of a CTA together (see "heavy items" below)
     int* heavy_counter;         // work counter of the heavy items
+    int v8;                     // 1: N % 4 == 0 and grid 32-byte aligned: the write-out uses 256-bit stores (one full sector per lane)
     int pdl;                    // 1: launched with programmatic stream serialisation behind the fused pre-pass of a small call
                                 //    (bin_small_kernel): the table copies are built while the pre-pass still runs, and
                                 //    griddepcontrol.wait comes before the first read of anything the pre-pass writes
@@ -479,6 +482,35 @@ gather_kernel(const GatherParams P) {
                     }
                 }
             }
+        } else if (P.v8) {
+            // N is a multiple of 4 and the grid 32-byte aligned: a lane's 4 cells of a row are one aligned 32-byte sector,
+            // written by ONE 256-bit store (the four lanes of a block row fill a 128-byte line per instruction; two 128-bit
+            // stores would write every sector in two halves, two instructions apart)
+            const int x = X0 + 4 * bx;
+            if (x < g.N) {
+#pragma unroll
+                for (int i = 0; i < 2; ++i) {
+                    const int y = Y0 + 2 * by + i;
+                    if (y < g.N) {
+#pragma unroll
+                        for (int p = 0; p < 4; ++p) {
+                            float* dst = P.grid + (((size_t)c * 4 + p) * plane + (size_t)y * g.N + x) * 2;
+                            float a0, a1, a2, a3, a4, a5, a6, a7;
+                            unpack2(acc[i][0][p], a0, a1);
+                            unpack2(acc[i][1][p], a2, a3);
+                            unpack2(acc[i][2][p], a4, a5);
+                            unpack2(acc[i][3][p], a6, a7);
+                            if (P.accumulate) {                         // the warp owns these cells: a plain read-modify-write
+                                const float4 o0 = *reinterpret_cast<const float4*>(dst), o1 = *reinterpret_cast<const float4*>(dst + 4);
+                                a0 += o0.x; a1 += o0.y; a2 += o0.z; a3 += o0.w;
+                                a4 += o1.x; a5 += o1.y; a6 += o1.z; a7 += o1.w;
+                            }
+                            asm volatile("st.global.cs.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(dst), "f"(a0), "f"(a1), "f"(a2),
+                                         "f"(a3), "f"(a4), "f"(a5), "f"(a6), "f"(a7) : "memory");
+                        }
+                    }
+                }
+            }
         } else {
             const int x = X0 + 4 * bx;
 #pragma unroll
@@ -534,6 +566,7 @@ bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, i
     P.n_chan = n_chan;
     P.accumulate = p->accumulate ? 1 : 0;
     P.mfs = p->mfs ? 1 : 0;
+    P.v8 = (p->geom.N % 4 == 0 && (reinterpret_cast<uintptr_t>(grid) & 31) == 0) ? 1 : 0;
     if (p->mfs && !p->accumulate) {                             // the reductions need a zeroed grid
         if (!cuda_ok(cudaMemsetAsync(grid, 0, (size_t)4 * p->geom.N * p->geom.N * 8, st), "memset grid")) return false;
         p->last_launches += 1;
