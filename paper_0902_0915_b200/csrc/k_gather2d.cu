@@ -208,6 +208,7 @@ gather2d_kernel(const Gather2dParams P) {
         if (n_buf > 0) consume(n_buf);
 
         const int x = X0 + 4 * bx;
+        const bool v8 = (g.N & 3) == 0 && (reinterpret_cast<unsigned long long>(P.grid) & 31ull) == 0ull;
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
             const int y = Y0 + 2 * by + i;
@@ -216,6 +217,18 @@ gather2d_kernel(const Gather2dParams P) {
                 for (int p = 0; p < 4; ++p) {
                     float* dst = P.grid + (((size_t)c * 4 + p) * plane + (size_t)y * g.N + x) * 2;
                     float a0, a1, a2, a3;
+                    if (v8) {                                    // one aligned 32-byte sector per lane: one 256-bit store (as K3c)
+                        if (x < g.N) {
+                            float a4, a5, a6, a7;
+                            g2_unpack(acc[i][0][p], a0, a1);
+                            g2_unpack(acc[i][1][p], a2, a3);
+                            g2_unpack(acc[i][2][p], a4, a5);
+                            g2_unpack(acc[i][3][p], a6, a7);
+                            asm volatile("st.global.cs.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(dst), "f"(a0), "f"(a1), "f"(a2),
+                                         "f"(a3), "f"(a4), "f"(a5), "f"(a6), "f"(a7) : "memory");
+                        }
+                        continue;
+                    }
                     if (x + 1 < g.N) {
                         g2_unpack(acc[i][0][p], a0, a1);
                         g2_unpack(acc[i][1][p], a2, a3);

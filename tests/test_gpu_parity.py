@@ -595,6 +595,25 @@ def test_multi_frequency_synthesis_sums_the_channels_onto_one_grid(lib, design):
         assert tuple(back.shape) == (12, 4, 250, 250)
 
 
+def test_grid_out_aligned_to_16_but_not_32_bytes(lib):
+    """The ABI asks for a 16-byte aligned grid_out; K3c's 256-bit stores need 32 and must fall back to 128-bit stores."""
+    g = generate(scaled(CONFIGS["C2"], n_ant=48, n_chan=3, grid_n=256))
+    cfg = g.cfg
+    G, A, _ = _oracle(g)
+    _to_dev(g)
+    n = cfg.n_chan * 4 * cfg.grid_n * cfg.grid_n
+    buf = torch.full((n + 2,), complex(float("nan"), float("nan")), dtype=torch.complex64, device="cuda")
+    out = buf[2:].view(cfg.n_chan, 4, cfg.grid_n, cfg.grid_n)              # 16 bytes past a 512-byte aligned allocation
+    assert out.data_ptr() % 32 == 16
+    with _plan(lib, g, "gather") as p:
+        lib.mwa_grid_visibilities(p.handle, g.uv, g.freqs, g.vis, g.weights, cfg.n_vis, cfg.n_chan, out)
+        torch.cuda.synchronize()
+        assert_parity(out.cpu().numpy(), G, A, "gather, grid_out 16-byte aligned")
+        ref = p.grid(g.uv, g.freqs, g.vis, g.weights)                         # 32-byte aligned: the 256-bit path
+        assert torch.equal(ref.view(torch.float32), out.contiguous().view(torch.float32))
+    assert torch.isnan(buf[:2].real).all()                                   # nothing written in front of the grid
+
+
 # ---------------------------------------------------------------------------- K3c: heavy tiles gridded by four warps
 @pytest.mark.parametrize("mode", ["overwrite", "accumulate", "mfs"])
 def test_gather_heavy_tiles_are_gridded_by_the_four_warps_of_a_cta(lib, mode):
