@@ -161,8 +161,10 @@ static int grid_device(Plan* p, const double* uv, const double* freqs, const flo
     if (bins && binning_is_small(p, n_vis)) {              // launch-bound calls: a1 + a3 in one launch
         if (!launch_small_prepass(p, uv, freqs, n_vis, n_chan, st)) return MWA_GRID_ERR_CUDA;
     } else {
+        // the memsets of the binning step go first, so that its first kernel can follow scale_kernel as a dependent launch
+        if (bins && !launch_binning_clear(p, st)) return MWA_GRID_ERR_CUDA;
         if (!launch_scale(p, freqs, n_chan, st)) return MWA_GRID_ERR_CUDA;
-        if (bins && !launch_binning(p, uv, n_vis, n_chan, st)) return MWA_GRID_ERR_CUDA;
+        if (bins && !launch_binning(p, uv, n_vis, n_chan, st, true)) return MWA_GRID_ERR_CUDA;
     }
     {
         // the pre-pass kernels form a chain of programmatic dependent launches; only a gather kernel that DIRECTLY follows

@@ -12,6 +12,7 @@ namespace mwa {
 __global__ void scale_kernel(const double* __restrict__ freqs, int n_chan, int half_n, int chan_ok,
                              double* __restrict__ scale, double* __restrict__ scale_ref, int* __restrict__ dispatch,
                              double4* __restrict__ group) {
+    pdl_release();                                      // bin_count_kernel may follow as a programmatic dependent (it waits for this grid)
     scale_block(freqs, n_chan, half_n, chan_ok, scale, scale_ref, dispatch, group);     // one block
 }
 

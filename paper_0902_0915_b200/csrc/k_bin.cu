@@ -446,28 +446,44 @@ bool launch_small_prepass(Plan* p, const double* uv, const double* freqs, long l
     return cuda_ok(cudaGetLastError(), "bin_small_kernel (fused pre-pass)");
 }
 
-bool launch_binning(Plan* p, const double* uv, long long n_vis, int /*n_chan*/, cudaStream_t st) {
+// The two memsets of the multi-kernel binning path, for callers that enqueue them BEFORE scale_kernel: bin_count_kernel
+// can then be launched as scale_kernel's programmatic dependent (launch_binning with cleared = true).
+bool launch_binning_clear(Plan* p, cudaStream_t st) {
+    Workspace& ws = p->ws;
+    const int nb = (p->geom.N + kBucketCells - 1) / kBucketCells;
+    if (!cuda_ok(cudaMemsetAsync(ws.d_misc, 0, (size_t)kMiscInts * sizeof(int), st), "memset misc")) return false;
+    if (!cuda_ok(cudaMemsetAsync(ws.d_bucket_count, 0, ((size_t)nb * nb + 1) * sizeof(int), st), "memset buckets")) return false;
+    p->last_launches += 2;
+    return true;
+}
+
+bool launch_binning(Plan* p, const double* uv, long long n_vis, int /*n_chan*/, cudaStream_t st, bool cleared) {
     Workspace& ws = p->ws;
     const int nb = (p->geom.N + kBucketCells - 1) / kBucketCells;
     const int n_buckets = nb * nb;
     const int nt = (p->geom.N + kTile - 1) / kTile;
-    if (!cuda_ok(cudaMemsetAsync(ws.d_misc, 0, (size_t)kMiscInts * sizeof(int), st), "memset misc")) return false;
-    if (n_vis <= kSmallRows && n_buckets <= kSmallBuckets && nt * nt <= kSmallTiles) {
+    if (!cleared && !cuda_ok(cudaMemsetAsync(ws.d_misc, 0, (size_t)kMiscInts * sizeof(int), st), "memset misc")) return false;
+    if (!cleared && n_vis <= kSmallRows && n_buckets <= kSmallBuckets && nt * nt <= kSmallTiles) {
         bin_small_kernel<<<1, 1024, 0, st>>>(p->geom, (const double2*)uv, ws.d_scale_ref, (int)n_vis, nb, nt, ws.d_bucket_count,
                                              ws.d_perm, ws.d_uv_sorted, (double4*)ws.d_row_sorted, ws.d_tile_weight, ws.d_tile_order,
                                              nullptr, 0, 0, nullptr, nullptr, nullptr, nullptr, nullptr);
         p->last_launches += 2;
         return cuda_ok(cudaGetLastError(), "bin_small_kernel");
     }
-    if (!cuda_ok(cudaMemsetAsync(ws.d_bucket_count, 0, ((size_t)n_buckets + 1) * sizeof(int), st), "memset buckets"))
+    if (!cleared && !cuda_ok(cudaMemsetAsync(ws.d_bucket_count, 0, ((size_t)n_buckets + 1) * sizeof(int), st), "memset buckets"))
         return false;
     int blocks = (int)((n_vis + 255) / 256);
     if (blocks > p->sm_count * 8) blocks = p->sm_count * 8;
-    bin_count_kernel<<<blocks, 256, 0, st>>>(p->geom, (const double2*)uv, ws.d_scale_ref, (int)n_vis, nb,
-                                             ws.d_bucket_count);
-    // from here on every kernel is launched as a programmatic dependent of the one before it: it becomes resident while
-    // its predecessor drains and waits (pdl_wait) for the predecessor's completion before its first read
-    cudaError_t e = launch_dependent(bin_scan_kernel, dim3((n_buckets + kScanPerBlock - 1) / kScanPerBlock), dim3(1024), 0, st,
+    // every kernel is launched as a programmatic dependent of the one before it: it becomes resident while its predecessor
+    // drains and waits (pdl_wait) for the predecessor's completion before its first read.  bin_count_kernel joins the chain
+    // behind scale_kernel when the memsets were enqueued before that kernel (cleared), else it follows the memsets plainly.
+    cudaError_t e = cudaSuccess;
+    if (cleared)
+        e = launch_dependent(bin_count_kernel, dim3(blocks), dim3(256), 0, st, p->geom, (const double2*)uv, (const double*)ws.d_scale_ref,
+                             (int)n_vis, nb, ws.d_bucket_count);
+    else
+        bin_count_kernel<<<blocks, 256, 0, st>>>(p->geom, (const double2*)uv, ws.d_scale_ref, (int)n_vis, nb, ws.d_bucket_count);
+    if (e == cudaSuccess) e = launch_dependent(bin_scan_kernel, dim3((n_buckets + kScanPerBlock - 1) / kScanPerBlock), dim3(1024), 0, st,
                                      ws.d_bucket_count, n_buckets, ws.d_bucket_cursor, ws.d_misc + kMiscScanState);
     if (e == cudaSuccess)
         e = launch_dependent(bin_scatter_kernel, dim3(blocks), dim3(256), 0, st, p->geom, (const double2*)uv, (const double*)ws.d_scale_ref,
@@ -498,7 +514,7 @@ bool launch_binning(Plan* p, const double* uv, long long n_vis, int /*n_chan*/, 
                              ws.d_tile_order);
     if (!cuda_ok(e, "binning kernels (dependent launches)")) return false;
     p->pdl_next = true;                                        // a gridder that comes next may join the chain
-    p->last_launches += 9;
+    p->last_launches += cleared ? 7 : 9;
     return cuda_ok(cudaGetLastError(), "binning kernels");
 }
 

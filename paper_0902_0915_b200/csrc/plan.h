@@ -129,7 +129,8 @@ bool launch_count_dropped(Plan* p, const double* uv, long long n_vis, int n_chan
 bool launch_indices(Plan* p, const double* uv, long long n_vis, int n_chan, int* out_idx, cudaStream_t st);
 bool launch_atomic(Plan* p, const double* uv, const float* vis, const float* w, long long n_vis, int n_chan,
                    float* grid, cudaStream_t st);
-bool launch_binning(Plan* p, const double* uv, long long n_vis, int n_chan, cudaStream_t st);
+bool launch_binning(Plan* p, const double* uv, long long n_vis, int n_chan, cudaStream_t st, bool cleared = false);
+bool launch_binning_clear(Plan* p, cudaStream_t st);       // the memsets of launch_binning, to be enqueued before launch_scale (then cleared = true)
 bool binning_is_small(const Plan* p, long long n_vis);     // the call's a1 + a3 fit one CTA: launch_small_prepass replaces
 bool launch_small_prepass(Plan* p, const double* uv, const double* freqs, long long n_vis, int n_chan, cudaStream_t st);   // launch_scale + launch_binning
 bool launch_gather(Plan* p, const float* vis, const float* w, long long n_vis, int n_chan, float* grid,
