@@ -6,8 +6,8 @@
 // that overlap it, and decides membership with the exact index function; the buckets only have to be
 // conservative.  n_vis items are sorted, not n_vis * n_chan.
 //
-// Launches: bin_count, then - each as a programmatic dependent of the one before (plan.h: launch_dependent; every kernel
-// starts with pdl_wait / pdl_release) - bin_scan, bin_scatter, bin_order, bin_order_large, tile_weight, tile_order_scan,
+// Launches: the two memsets, scale_kernel (k_basic.cu), then - each as a programmatic dependent of the one before (plan.h:
+// launch_dependent; every kernel starts with pdl_wait / pdl_release) - bin_count, bin_scan, bin_scatter, bin_order, bin_order_large, tile_weight, tile_order_scan,
 // tile_order_scatter.  Small calls (<= 4096 rows) do all of it, and a1, in the single CTA of bin_small_kernel.
 #include "plan.h"
 #include "scale.cuh"
